@@ -1,0 +1,79 @@
+// rc_oracle.cpp -- ORACLE (test infrastructure, not the product).
+//
+// Plain single-threaded C++17 statement of what the claim-scoped KV offload /
+// restore path computes.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may load this library.  It shares no
+// source, header, table or helper with paper_2606_01387_b200/csrc (constants
+// are restated here on purpose).
+//
+// Passages followed (P:Lnnn = /root/reference/PAPER.md line nnn):
+//   P:L25-27   running example: accept(C,P,leading-prefix-at-least-448),
+//              materialized(C), offloaded(C), restore-required(C), same-claim
+//              load failure, restoration_failed(C),
+//              active_request_refused(blocking_claim_ids=[C]).
+//   P:L333     "accepted" precedes lifecycle events; "refused" is emitted after
+//              the same-claim restoration failure and before terminal handling.
+//   P:L337     failure injection: off by default, CPU->GPU only, claim-id
+//              filter, unclaimed failures need a separate flag.
+//   P:L358-380 witness paths A (success) and B (same-claim failure).
+//   P:L384     path C: only the target claim is attributed.
+//   P:L199     ambiguity fails closed: an error status emits no event.
+// Everything the paper leaves open (byte layout, checksum, allocator, codes) is
+// build-defined: DESIGN.md "Readings" R1..R21.  Pins: tests/test_oracle_*.py.
+// Parity unpinned (beyond GPU==oracle): status-code numbering, aux/arg payload
+// choice, one-shot fault consumption, NO_FREE_BLOCKS / NO_HOST_SPACE policy.
+#include <cstdint>
+#include <cstring>
+#include <cstdlib>
+#include <vector>
+#include <map>
+#include <algorithm>
+
+typedef uint64_t u64;
+typedef uint32_t u32;
+typedef uint8_t u8;
+
+// ---- checksum (build-defined) -------------------------
+static const u64 K1 = 0x9E3779B97F4A7C15ull;  // 2^64/phi
+static const u64 K2 = 0x6A09E667F3BCC909ull;  // frac(sqrt 2) | 1
+static const u64 KA = 0xBB67AE8584CAA73Bull;  // frac(sqrt 3), odd
+static const u64 K3 = 0x3C6EF372FE94F82Bull;  // frac(sqrt 5)
+
+static u64 mixL(u64 x) { u64 y = x ^ (x >> 32); y *= K2; return y ^ (y >> 29); }
+static u64 mixF(u64 x) { u64 y = mixL(x); y *= K1; return y ^ (y >> 32); }
+
+static u64 load64le(const u8* p) {
+  u64 v = 0;
+  for (int i = 7; i >= 0; --i) v = (v << 8) | p[i];
+  return v;
+}
+
+// One page = V = page_bytes/16 vectors of two little-endian u64 words.
+// 256 lanes; lane t folds vectors t, t+256, t+512, ... in increasing order.
+static u64 page_digest(const u8* pg, u64 page_bytes) {
+  u64 V = page_bytes / 16, p = 0;
+  for (u64 lane = 0; lane < 256; ++lane) {
+    u64 h = (lane + 1) * K1;
+    for (u64 v = lane; v < V; v += 256) {
+      h = (h ^ load64le(pg + 16 * v)) * K2;
+      h = (h ^ load64le(pg + 16 * v + 8)) * K2;
+    }
+    p += mixL(h);
+  }
+  return p;
+}
+
+// A block in offload order: 2L pages, page g = l*2 + kv.
+static u64 block_digest(const u8* blk, u32 n_pages, u64 page_bytes) {
+  u64 s = 0;
+  for (u32 g = 0; g < n_pages; ++g)
+    s += mixL(page_digest(blk + (u64)g * page_bytes, page_bytes) ^ ((u64)(g + 1) * K3));
+  return mixF(s);
+}
+
+static u64 chain_seed(u64 claim_id) { return mixF(claim_id ^ K3); }
+static u64 chain_of(u64 claim_id, const u64* d, u32 nb) {
+  u64 h = chain_seed(claim_id);
+  for (u32 i = 0; i < nb; ++i) h = h * KA + d[i];
+  return h;
+}
