@@ -77,3 +77,44 @@ static u64 chain_of(u64 claim_id, const u64* d, u32 nb) {
   for (u32 i = 0; i < nb; ++i) h = h * KA + d[i];
   return h;
 }
+
+// ---- codes (restated; the ABI header of the product is not included) --------
+enum { EV_ACCEPTED = 1, EV_MATERIALIZED = 2, EV_OFFLOADED = 3, EV_RESTORE_REQUIRED = 4,
+       EV_LOAD_FAILED = 5, EV_RESTORED = 6, EV_RESTORATION_FAILED = 7,
+       EV_ACTIVE_REQUEST_REFUSED = 8 };
+enum { ST_OK = 0, ST_PRED_FALSE = 1, ST_UNKNOWN_CLAIM = 2, ST_BAD_STATE = 3, ST_DUPLICATE_ID = 4,
+       ST_BAD_TABLE = 5, ST_NO_FREE_BLOCKS = 6, ST_NO_HOST_SPACE = 7, ST_RESTORE_FAILED = 8 };
+enum { CS_ACCEPTED = 1, CS_MATERIALIZED = 2, CS_OFFLOADED = 3, CS_RESIDENT_AGAIN = 4, CS_REFUSED = 5 };
+enum { FK_XFER_ERROR = 1, FK_BITFLIP = 2 };
+enum { FF_ALLOW_UNCLAIMED = 1 };
+enum { E_OK = 0, E_INVALID = -1 };
+
+struct Event { u64 seq, claim_id; u32 code, aux; u64 arg; };   // 32 bytes
+struct Fault { u64 claim_id; u32 kind, param; };
+struct ClaimInfo { u64 claim_id, chain, host_bytes; u32 state, P, N, M, nb, n_table; };
+
+struct Claim {
+  u32 state = 0, P = 0, N = 0, M = 0, nb = 0;
+  std::vector<u32> bt;        // current block table
+  std::vector<u64> d;         // per-block digests recorded at offload
+  u64 chain = 0;
+  std::vector<u8> host;       // claim-scoped host copy (nb*blk bytes)
+};
+
+struct Ctx {
+  u32 L, H, D, e, BS, NB;
+  u64 page, blk, host_cap, host_used = 0;
+  u8* pool;                   // caller-owned host mirror [L][2][NB][page]
+  u8* fill;                   // caller-owned u8[NB]
+  std::vector<u8> used;
+  std::vector<u32> ref;
+  std::map<u64, Claim> claims;
+  std::vector<Fault> faults; u32 fault_flags = 0;
+  std::vector<Event> events; u64 drained = 0;
+  u64 generic_failures = 0;
+  void emit(u64 c, u32 code, u32 aux, u64 arg) {
+    Event ev; ev.seq = events.size(); ev.claim_id = c; ev.code = code; ev.aux = aux; ev.arg = arg;
+    events.push_back(ev);
+  }
+  u8* page_ptr(u32 g, u32 b) { return pool + ((u64)g * NB + b) * page; }
+};
