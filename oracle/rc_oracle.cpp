@@ -118,3 +118,80 @@ struct Ctx {
   }
   u8* page_ptr(u32 g, u32 b) { return pool + ((u64)g * NB + b) * page; }
 };
+
+static u32 ceil_div(u32 a, u32 b) { return (a + b - 1) / b; }
+
+// accept(C,P,N,bt): "first accepted by a mechanism that records C, P, and
+// the predicate"; P:L199 duplicate ownership / ambiguity -> no claim outcome.
+static int do_accept(Ctx* c, u64 id, u32 P, u32 N, const u32* bt, u32 nbt) {
+  if (id == 0) return ST_UNKNOWN_CLAIM;                 // 0 is reserved: "no claim"
+  if (c->claims.count(id)) return ST_DUPLICATE_ID;
+  if (P == 0 || N == 0 || N > P) return ST_BAD_TABLE;
+  if (nbt != ceil_div(P, c->BS)) return ST_BAD_TABLE;
+  for (u32 i = 0; i < nbt; ++i) {
+    if (bt[i] >= c->NB || !c->used[bt[i]]) return ST_BAD_TABLE;
+    for (u32 j = 0; j < i; ++j) if (bt[j] == bt[i]) return ST_BAD_TABLE;
+  }
+  Claim cl; cl.state = CS_ACCEPTED; cl.P = P; cl.N = N; cl.bt.assign(bt, bt + nbt);
+  for (u32 i = 0; i < nbt; ++i) c->ref[bt[i]]++;
+  c->claims[id] = cl;
+  c->emit(id, EV_ACCEPTED, N, P);
+  return ST_OK;
+}
+
+// Predicate by its token-level definition (DESIGN R2): token t of the prefix is
+// materialized iff (t mod BS) < fill[bt[t div BS]];  M = length of the leading
+// run of materialized tokens;  leading-prefix-at-least-N holds iff M >= N
+// (">=" because hit=448 with predicate 448 is served).
+static u32 leading_materialized(Ctx* c, const Claim& cl) {
+  u32 m = 0;
+  while (m < cl.P && (m % c->BS) < c->fill[cl.bt[m / c->BS]]) ++m;
+  return m;
+}
+
+static int do_materialize(Ctx* c, u64 id) {
+  auto it = c->claims.find(id);
+  if (it == c->claims.end()) return ST_UNKNOWN_CLAIM;   // post-hoc naming rejected
+  Claim& cl = it->second;
+  if (cl.state != CS_ACCEPTED) return ST_BAD_STATE;
+  u32 M = leading_materialized(c, cl);
+  if (M < cl.N) return ST_PRED_FALSE;                   // no event
+  cl.M = M; cl.nb = ceil_div(M, c->BS); cl.state = CS_MATERIALIZED;
+  c->emit(id, EV_MATERIALIZED, M, 0);
+  return ST_OK;
+}
+
+static void drop_refs(Ctx* c, Claim& cl) {
+  for (u32 b : cl.bt) { if (c->ref[b] > 0 && --c->ref[b] == 0) c->used[b] = 0; }
+  cl.bt.clear();
+}
+
+// offload: P:L343-346 (E2-E5).  Host bytes = concatenation, block-major,
+// then page g = l*2+kv.  Never failed by injection (CPU->GPU only).
+static void do_offload_one(Ctx* c, u64 id, Claim& cl) {
+  u32 G = 2 * c->L;
+  cl.host.resize((u64)cl.nb * c->blk);
+  for (u32 i = 0; i < cl.nb; ++i)
+    for (u32 g = 0; g < G; ++g)
+      memcpy(cl.host.data() + (u64)i * c->blk + (u64)g * c->page, c->page_ptr(g, cl.bt[i]), c->page);
+  cl.d.resize(cl.nb);
+  for (u32 i = 0; i < cl.nb; ++i) cl.d[i] = block_digest(cl.host.data() + (u64)i * c->blk, G, c->page);
+  cl.chain = chain_of(id, cl.d.data(), cl.nb);
+  c->host_used += cl.host.size();
+  drop_refs(c, cl);
+  cl.state = CS_OFFLOADED;
+  c->emit(id, EV_OFFLOADED, cl.nb, cl.chain);
+}
+
+static void do_offload(Ctx* c, u32 n, const u64* ids, int32_t* st) {
+  bool full = false;                                    // prefix rule (DESIGN R7)
+  for (u32 k = 0; k < n; ++k) {
+    auto it = c->claims.find(ids[k]);
+    if (it == c->claims.end()) { st[k] = ST_UNKNOWN_CLAIM; continue; }
+    Claim& cl = it->second;
+    if (cl.state != CS_MATERIALIZED && cl.state != CS_RESIDENT_AGAIN) { st[k] = ST_BAD_STATE; continue; }
+    if (full || c->host_used + (u64)cl.nb * c->blk > c->host_cap) { full = true; st[k] = ST_NO_HOST_SPACE; continue; }
+    do_offload_one(c, ids[k], cl);
+    st[k] = ST_OK;
+  }
+}
