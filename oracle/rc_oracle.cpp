@@ -195,3 +195,90 @@ static void do_offload(Ctx* c, u32 n, const u64* ids, int32_t* st) {
     st[k] = ST_OK;
   }
 }
+
+// restore: P:L347-351 (E6-E9) on success; P:L353-356, P:L376-380 on same-claim
+// failure.  The call works in the phases DESIGN R6/R7 fix:
+//   1. eligibility in batch order (state must be OFFLOADED: restore-after-use and
+//      double restore are BAD_STATE);
+//   2. free-block prefix rule against the free count at call entry;
+//   3. every served claim, in batch order, takes the next nb lowest free ids;
+//   4. per served claim, batch order: RESTORE_REQUIRED, fault decision (first armed
+//      entry whose id == C, one-shot; other ids have no effect: P:L25, P:L463,
+//      P:L493), write + re-digest + compare, verdict events;
+//   5. blocks of failed claims are freed after step 4 of that claim.
+static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st) {
+  u32 G = 2 * c->L;
+  std::vector<Claim*> served(n, nullptr);
+  u64 nfree = 0;
+  for (u32 b = 0; b < c->NB; ++b) nfree += !c->used[b];
+  u64 need = 0; bool full = false;
+  for (u32 k = 0; k < n; ++k) {
+    auto it = c->claims.find(ids[k]);
+    if (it == c->claims.end()) { st[k] = ST_UNKNOWN_CLAIM; continue; }
+    Claim& cl = it->second;
+    bool dup = false;
+    for (u32 j = 0; j < k; ++j) if (served[j] == &cl) dup = true;
+    if (cl.state != CS_OFFLOADED || dup) { st[k] = ST_BAD_STATE; continue; }
+    if (full || need + cl.nb > nfree) { full = true; st[k] = ST_NO_FREE_BLOCKS; continue; }
+    need += cl.nb; served[k] = &cl; st[k] = ST_OK;
+  }
+  u32 cursor = 0;                                       // step 3: lowest free ids, ascending
+  for (u32 k = 0; k < n; ++k) {
+    if (!served[k]) continue;
+    Claim& cl = *served[k];
+    cl.bt.clear();
+    while (cl.bt.size() < cl.nb) {
+      while (c->used[cursor]) ++cursor;
+      c->used[cursor] = 1; c->ref[cursor] = 1; cl.bt.push_back(cursor);
+    }
+  }
+  bool any_served = false;
+  for (u32 k = 0; k < n; ++k) {
+    if (!served[k]) continue;
+    any_served = true;
+    Claim& cl = *served[k]; u64 id = ids[k];
+    c->emit(id, EV_RESTORE_REQUIRED, cl.M, 0);          // lookup "hit"
+    int fi = -1;
+    for (size_t f = 0; f < c->faults.size(); ++f) if (c->faults[f].claim_id == id) { fi = (int)f; break; }
+    Fault flt{0, 0, 0};
+    if (fi >= 0) { flt = c->faults[fi]; c->faults.erase(c->faults.begin() + fi); }
+    bool ok; u32 bad = 0xFFFFFFFFu;
+    if (flt.kind == FK_XFER_ERROR) {
+      ok = false;                                       // nothing is written to the pool
+    } else {
+      std::vector<u8> staged(cl.host);                  // host copy itself stays intact
+      if (flt.kind == FK_BITFLIP && !staged.empty()) staged[flt.param % staged.size()] ^= 0x01;
+      std::vector<u64> d2(cl.nb);
+      for (u32 i = 0; i < cl.nb; ++i) {
+        for (u32 g = 0; g < G; ++g)
+          memcpy(c->page_ptr(g, cl.bt[i]), staged.data() + (u64)i * c->blk + (u64)g * c->page, c->page);
+        u32 rem = cl.M - i * c->BS;
+        c->fill[cl.bt[i]] = (u8)(rem < c->BS ? rem : c->BS);
+        d2[i] = block_digest(staged.data() + (u64)i * c->blk, G, c->page);
+      }
+      bool found = false;
+      for (u32 i = 0; i < cl.nb && !found; ++i) if (d2[i] != cl.d[i]) { bad = i; found = true; }
+      ok = !found && chain_of(id, d2.data(), cl.nb) == cl.chain;
+    }
+    c->host_used -= cl.host.size();
+    std::vector<u8>().swap(cl.host);
+    if (ok) {
+      cl.state = CS_RESIDENT_AGAIN;
+      c->emit(id, EV_RESTORED, cl.nb, cl.chain);
+      st[k] = ST_OK;
+    } else {
+      c->emit(id, EV_LOAD_FAILED, bad, 0);
+      c->emit(id, EV_RESTORATION_FAILED, 0, 0);
+      c->emit(id, EV_ACTIVE_REQUEST_REFUSED, 1, id);    // blocking_claim_ids=[C]: aux = count, arg = C
+      for (u32 b : cl.bt) { c->used[b] = 0; c->ref[b] = 0; c->fill[b] = 0; }
+      cl.bt.clear(); cl.d.clear();
+      cl.state = CS_REFUSED;                            // terminal
+      st[k] = ST_RESTORE_FAILED;
+    }
+  }
+  if (any_served && (c->fault_flags & FF_ALLOW_UNCLAIMED)) {   // P:L337; generic counter only
+    for (size_t f = 0; f < c->faults.size();)
+      if (c->faults[f].claim_id == 0) { c->generic_failures++; c->faults.erase(c->faults.begin() + f); }
+      else ++f;
+  }
+}
