@@ -282,3 +282,123 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st) {
       else ++f;
   }
 }
+
+// ---- C ABI (host pointers everywhere) ---------------------------------------
+struct rco_config { u32 layers, kv_heads, head_dim, elem_bytes, block_size, pool_blocks;
+                    u64 host_store_bytes; void* pool; u8* fill; };
+
+extern "C" {
+
+int rco_create(const rco_config* cfg, void** out) {
+  if (!cfg || !out || !cfg->pool || !cfg->fill) return E_INVALID;
+  u64 page = (u64)cfg->block_size * cfg->kv_heads * cfg->head_dim * cfg->elem_bytes;
+  if (page == 0 || page % 4096 != 0 || cfg->layers == 0 || cfg->pool_blocks == 0) return E_INVALID;
+  Ctx* c = new Ctx();
+  c->L = cfg->layers; c->H = cfg->kv_heads; c->D = cfg->head_dim; c->e = cfg->elem_bytes;
+  c->BS = cfg->block_size; c->NB = cfg->pool_blocks; c->page = page; c->blk = 2ull * c->L * page;
+  c->host_cap = cfg->host_store_bytes; c->pool = (u8*)cfg->pool; c->fill = cfg->fill;
+  c->used.assign(c->NB, 0); c->ref.assign(c->NB, 0);
+  *out = c; return E_OK;
+}
+int rco_destroy(void* h) { delete (Ctx*)h; return E_OK; }
+
+int rco_mark_used(void* h, u32 n, const u32* ids) {
+  Ctx* c = (Ctx*)h;
+  for (u32 i = 0; i < n; ++i) if (ids[i] >= c->NB) return E_INVALID;
+  for (u32 i = 0; i < n; ++i) c->used[ids[i]] = 1;
+  return E_OK;
+}
+int rco_mark_free(void* h, u32 n, const u32* ids) {      // claimed blocks (ref>0) are left alone
+  Ctx* c = (Ctx*)h;
+  for (u32 i = 0; i < n; ++i) if (ids[i] >= c->NB) return E_INVALID;
+  for (u32 i = 0; i < n; ++i) if (c->ref[ids[i]] == 0) c->used[ids[i]] = 0;
+  return E_OK;
+}
+int rco_accept(void* h, u32 n, const u64* id, const u32* P, const u32* N, const u32* bt_off,
+               const u32* bt_ids, int32_t* st) {
+  Ctx* c = (Ctx*)h;
+  for (u32 k = 0; k < n; ++k) {
+    if (bt_off[k + 1] < bt_off[k]) { st[k] = ST_BAD_TABLE; continue; }
+    st[k] = do_accept(c, id[k], P[k], N[k], bt_ids + bt_off[k], bt_off[k + 1] - bt_off[k]);
+  }
+  return E_OK;
+}
+int rco_materialize(void* h, u32 n, const u64* id, int32_t* st) {
+  for (u32 k = 0; k < n; ++k) st[k] = do_materialize((Ctx*)h, id[k]);
+  return E_OK;
+}
+int rco_offload(void* h, u32 n, const u64* id, int32_t* st) { do_offload((Ctx*)h, n, id, st); return E_OK; }
+int rco_restore(void* h, u32 n, const u64* id, int32_t* st) { do_restore((Ctx*)h, n, id, st); return E_OK; }
+int rco_release(void* h, u32 n, const u64* id, int32_t* st) {
+  Ctx* c = (Ctx*)h;
+  for (u32 k = 0; k < n; ++k) {
+    auto it = c->claims.find(id[k]);
+    if (it == c->claims.end()) { st[k] = ST_UNKNOWN_CLAIM; continue; }
+    drop_refs(c, it->second);
+    c->host_used -= it->second.host.size();
+    c->claims.erase(it); st[k] = ST_OK;
+  }
+  return E_OK;
+}
+int rco_outcomes(void* h, Event* buf, u64 cap, u64* n_out) {
+  Ctx* c = (Ctx*)h; u64 k = 0;
+  while (k < cap && c->drained < c->events.size()) buf[k++] = c->events[c->drained++];
+  *n_out = k; return E_OK;
+}
+int rco_set_faults(void* h, u32 n, const Fault* f, u32 flags) {
+  Ctx* c = (Ctx*)h;
+  for (u32 i = 0; i < n; ++i) {
+    if (f[i].kind != FK_XFER_ERROR && f[i].kind != FK_BITFLIP) return E_INVALID;
+    if (f[i].claim_id == 0 && !(flags & FF_ALLOW_UNCLAIMED)) return E_INVALID;  // P:L337 separate flag
+  }
+  c->faults.assign(f, f + n); c->fault_flags = flags;
+  return E_OK;
+}
+int rco_claim_info(void* h, u64 id, ClaimInfo* o) {
+  Ctx* c = (Ctx*)h; auto it = c->claims.find(id);
+  if (it == c->claims.end()) return E_INVALID;
+  const Claim& cl = it->second;
+  o->claim_id = id; o->chain = cl.chain; o->host_bytes = cl.host.size(); o->state = cl.state;
+  o->P = cl.P; o->N = cl.N; o->M = cl.M; o->nb = cl.nb; o->n_table = (u32)cl.bt.size();
+  return E_OK;
+}
+int rco_claim_blocks(void* h, u64 id, u32* ids, u32 cap, u32* n) {
+  Ctx* c = (Ctx*)h; auto it = c->claims.find(id);
+  if (it == c->claims.end()) return E_INVALID;
+  *n = (u32)it->second.bt.size();
+  for (u32 i = 0; i < *n && i < cap; ++i) ids[i] = it->second.bt[i];
+  return E_OK;
+}
+int rco_claim_digests(void* h, u64 id, u64* d, u32 cap, u32* n) {
+  Ctx* c = (Ctx*)h; auto it = c->claims.find(id);
+  if (it == c->claims.end()) return E_INVALID;
+  *n = (u32)it->second.d.size();
+  for (u32 i = 0; i < *n && i < cap; ++i) d[i] = it->second.d[i];
+  return E_OK;
+}
+int rco_host_read(void* h, u64 id, void* dst, u64 cap, u64* bytes) {
+  Ctx* c = (Ctx*)h; auto it = c->claims.find(id);
+  if (it == c->claims.end()) return E_INVALID;
+  *bytes = it->second.host.size();
+  if (dst && cap >= *bytes && *bytes) memcpy(dst, it->second.host.data(), *bytes);
+  return E_OK;
+}
+int rco_pool_state(void* h, u8* used, u32* ref) {       // copies used[NB], ref[NB]
+  Ctx* c = (Ctx*)h;
+  if (used) memcpy(used, c->used.data(), c->NB);
+  if (ref) memcpy(ref, c->ref.data(), 4ull * c->NB);
+  return E_OK;
+}
+int rco_stats(void* h, u64* out4) {                     // host_used, n_claims, n_events, generic_failures
+  Ctx* c = (Ctx*)h;
+  out4[0] = c->host_used; out4[1] = c->claims.size(); out4[2] = c->events.size(); out4[3] = c->generic_failures;
+  return E_OK;
+}
+// checksum primitives, exported so the pins can reach each one directly
+u64 rco_mixL(u64 x) { return mixL(x); }
+u64 rco_mixF(u64 x) { return mixF(x); }
+u64 rco_page_digest(const void* p, u64 page_bytes) { return page_digest((const u8*)p, page_bytes); }
+u64 rco_block_digest(const void* p, u32 n_pages, u64 page_bytes) { return block_digest((const u8*)p, n_pages, page_bytes); }
+u64 rco_chain_of(u64 id, const u64* d, u32 nb) { return chain_of(id, d, nb); }
+
+}  // extern "C"
