@@ -1,0 +1,106 @@
+"""Event-stream validator -- ORACLE side, test infrastructure only.
+
+The CPU restatement of the paper's artifact analyzer, which "supplies no runtime
+behavior; it only checks order, claim match, and controls after the run"
+(P:L331).  Input: a list of (seq, claim_id, code, aux, arg) tuples (or a numpy
+record array with those fields).  Two harness-only marker codes may appear:
+USE(C) = "the reuse request consumed the prefix" and REQUEST_FINISHED(C).
+
+Accepted language per claim:
+    ACCEPTED MATERIALIZED ( OFFLOADED RESTORE_REQUIRED
+        ( RESTORED USE* | LOAD_FAILED RESTORATION_FAILED REFUSED ) )*
+any prefix of it is valid; nothing but REQUEST_FINISHED follows REFUSED.
+Rules and the passages that fix them:
+  * seq strictly increasing;
+  * no event names a claim before its ACCEPTED (post-hoc naming P:L257);
+  * USE(C) while C is offloaded / restore-required is invalid: restore-after-use
+    (P:L23);
+  * REQUEST_FINISHED(C) between LOAD_FAILED and REFUSED is invalid: the outcome
+    precedes terminal handling (path B row 8);
+  * LOAD_FAILED / RESTORATION_FAILED / REFUSED without RESTORE_REQUIRED(C) in the
+    same cycle is invalid: generic, unclaimed or wrong-claim failure (P:L25, P:L48,
+    P:L463);
+  * REFUSED.arg (blocking_claim_ids) must be [C], the refused claim itself.
+"""
+ACCEPTED, MATERIALIZED, OFFLOADED, RESTORE_REQUIRED, LOAD_FAILED, RESTORED, RESTORATION_FAILED, REFUSED = range(1, 9)
+USE, REQUEST_FINISHED = 100, 101
+
+# per-claim automaton states
+_S0, _ACC, _MAT, _OFF, _RREQ, _LF, _RF, _REF, _RES, _FIN = range(10)
+
+_NEXT = {
+    (_S0, ACCEPTED): _ACC,
+    (_ACC, MATERIALIZED): _MAT,
+    (_MAT, OFFLOADED): _OFF,
+    (_RES, OFFLOADED): _OFF,
+    (_OFF, RESTORE_REQUIRED): _RREQ,
+    (_RREQ, RESTORED): _RES,
+    (_RREQ, LOAD_FAILED): _LF,
+    (_LF, RESTORATION_FAILED): _RF,
+    (_RF, REFUSED): _REF,
+    (_MAT, USE): _MAT,
+    (_RES, USE): _RES,
+    (_REF, REQUEST_FINISHED): _FIN,
+    (_ACC, REQUEST_FINISHED): _FIN,
+    (_MAT, REQUEST_FINISHED): _FIN,
+    (_RES, REQUEST_FINISHED): _FIN,
+}
+
+
+def _rows(events):
+    out = []
+    for ev in events:
+        if hasattr(ev, "dtype") and ev.dtype.names:
+            out.append((int(ev["seq"]), int(ev["claim_id"]), int(ev["code"]), int(ev["aux"]), int(ev["arg"])))
+        else:
+            s, c, code, aux, arg = ev
+            out.append((int(s), int(c), int(code), int(aux), int(arg)))
+    return out
+
+
+def validate(events):
+    """Returns (ok, reason).  ok is True iff the whole stream is in the accepted language."""
+    state = {}
+    last_seq = None
+    for seq, cid, code, aux, arg in _rows(events):
+        if last_seq is not None and seq <= last_seq:
+            return False, "seq not strictly increasing at %d" % seq
+        last_seq = seq
+        if cid == 0:
+            return False, "event names no claim (unclaimed) at seq %d" % seq
+        s = state.get(cid, _S0)
+        nxt = _NEXT.get((s, code))
+        if nxt is None:
+            return False, "claim %#x: code %d not allowed in state %d (seq %d)" % (cid, code, s, seq)
+        if code == REFUSED and (arg != cid or aux != 1):
+            return False, "claim %#x: blocking_claim_ids is not [C] (seq %d)" % (cid, seq)
+        state[cid] = nxt
+    return True, "ok"
+
+
+FAILURE_ORDER = [ACCEPTED, MATERIALIZED, OFFLOADED, RESTORE_REQUIRED, LOAD_FAILED, RESTORATION_FAILED, REFUSED]
+SUCCESS_ORDER = [ACCEPTED, MATERIALIZED, OFFLOADED, RESTORE_REQUIRED, RESTORED]
+
+
+def codes_of(events, cid):
+    return [code for _, c, code, _, _ in _rows(events) if c == cid]
+
+
+def failure_outcome_gate(events, cid):
+    """Same-claim failure outcome gate: the stream is valid and C's own subsequence
+    ends with the exact seven-step order printed at P:L27."""
+    ok, _ = validate(events)
+    codes = [c for c in codes_of(events, cid) if c not in (USE, REQUEST_FINISHED)]
+    if not ok or len(codes) < 7:
+        return False
+    tail = codes[-7:] if len(codes) == 7 else codes[:2] + codes[-5:]
+    return tail == FAILURE_ORDER
+
+
+def observation_gate(events, cid):
+    """Positive observation gate (path A): C's subsequence ends with
+    OFFLOADED RESTORE_REQUIRED RESTORED and no failure record names C."""
+    ok, _ = validate(events)
+    codes = [c for c in codes_of(events, cid) if c not in (USE, REQUEST_FINISHED)]
+    return bool(ok and len(codes) >= 5 and codes[:2] == SUCCESS_ORDER[:2] and codes[-3:] == SUCCESS_ORDER[-3:]
+                and LOAD_FAILED not in codes and REFUSED not in codes)
