@@ -1,0 +1,168 @@
+/* rc.h -- C ABI of librc: claim-scoped offload and restoration of paged KV-cache
+ * blocks on one B200 (sm_100a).
+ *
+ * What the path means is fixed by /root/reference/PAPER.md (P:Lnnn = line nnn):
+ *   P:L25-27   running example and the accepted order  accept(C,P,>=448),
+ *              materialized(C), offloaded(C), restore-required(C), same-claim
+ *              load failure, restoration_failed(C),
+ *              active_request_refused(blocking_claim_ids=[C]);
+ *   P:L333     acceptance precedes every lifecycle event; refusal follows the
+ *              same-claim restoration failure, before terminal handling;
+ *   P:L337     failure injection is off by default, hits only CPU->GPU transfers,
+ *              filters by claim id; unclaimed failures need a separate flag;
+ *   P:L199     ambiguity fails closed: an error emits no claim outcome.
+ * Byte layouts, checksum, allocator rule and code numbering are build-defined
+ * (DESIGN.md "Readings").
+ *
+ * Conventions.  Every function returns 0 (RC_OK) or a negative call-level error;
+ * nothing throws, nothing uses errno.  Batch calls also fill a caller-owned HOST
+ * array int32_t status[n] (RC_ST_*).  Any status other than RC_ST_OK and
+ * RC_ST_RESTORE_FAILED means: no event was emitted for that claim by that call and
+ * its state is unchanged.  All pointer arguments are HOST pointers unless marked
+ * DEVICE.  Calls are synchronous: on return the device work is complete.  One caller
+ * thread per context.  A CUDA error poisons the context: every later call returns
+ * RC_ERR_CUDA.  There is no CPU fallback anywhere behind this interface.
+ */
+#ifndef RC_H_
+#define RC_H_
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rc_ctx rc_ctx;
+
+enum { RC_OK = 0, RC_ERR_INVALID = -1, RC_ERR_CUDA = -2, RC_ERR_NOMEM = -3, RC_ERR_CAPACITY = -4 };
+
+/* per-claim status */
+enum { RC_ST_OK = 0, RC_ST_PRED_FALSE = 1, RC_ST_UNKNOWN_CLAIM = 2, RC_ST_BAD_STATE = 3,
+       RC_ST_DUPLICATE_ID = 4, RC_ST_BAD_TABLE = 5, RC_ST_NO_FREE_BLOCKS = 6,
+       RC_ST_NO_HOST_SPACE = 7, RC_ST_RESTORE_FAILED = 8 };
+
+/* event codes (the ordered claim-scoped outcome stream) */
+enum { RC_EV_ACCEPTED = 1,          /* aux = N (predicate threshold), arg = P (prefix tokens)      */
+       RC_EV_MATERIALIZED = 2,      /* aux = M (leading materialized tokens), arg = 0              */
+       RC_EV_OFFLOADED = 3,         /* aux = nb (blocks offloaded), arg = chain checksum           */
+       RC_EV_RESTORE_REQUIRED = 4,  /* aux = M (the lookup "hit"), arg = 0                 */
+       RC_EV_LOAD_FAILED = 5,       /* aux = first bad block index, 0xFFFFFFFF = transfer error    */
+       RC_EV_RESTORED = 6,          /* aux = nb, arg = chain checksum                              */
+       RC_EV_RESTORATION_FAILED = 7,
+       RC_EV_ACTIVE_REQUEST_REFUSED = 8 /* aux = 1 = |blocking_claim_ids|, arg = C                 */ };
+
+/* claim states */
+enum { RC_CS_ACCEPTED = 1, RC_CS_MATERIALIZED = 2, RC_CS_OFFLOADED = 3, RC_CS_RESIDENT_AGAIN = 4,
+       RC_CS_REFUSED = 5 };
+
+enum { RC_FAULT_XFER_ERROR = 1, RC_FAULT_BITFLIP = 2 };
+enum { RC_FAULT_ALLOW_UNCLAIMED = 1 };
+
+typedef struct rc_event { uint64_t seq; uint64_t claim_id; uint32_t code; uint32_t aux; uint64_t arg; } rc_event;
+typedef struct rc_fault { uint64_t claim_id; uint32_t kind; uint32_t param; } rc_fault;
+
+typedef struct rc_config {
+  uint32_t layers, kv_heads, head_dim, elem_bytes; /* elem_bytes: 1 (fp8) or 2 (bf16); bytes are never decoded */
+  uint32_t block_size;                 /* tokens per block (BS)                                       */
+  uint32_t pool_blocks;                /* NB                                                          */
+  uint32_t max_claims;                 /* claim-table slots                                           */
+  uint32_t max_table_entries;          /* total block-table entries over all live claims              */
+  uint32_t max_events;                 /* event ring capacity (records not yet drained)               */
+  uint32_t staging_chunks;             /* ring depth, >= 2                                            */
+  uint64_t staging_chunk_bytes;        /* rounded down to a multiple of blk = 2*L*page                */
+  uint64_t host_store_bytes;           /* pinned host store, rounded down to a multiple of blk        */
+  void*    pool_dev;   /* DEVICE, caller-owned: [layers][2][NB][BS][kv_heads][head_dim], 256-B aligned */
+  uint8_t* fill_dev;   /* DEVICE, caller-owned u8[NB]: tokens materialized in each physical block     */
+  void*    stream_compute;  /* cudaStream_t (caller-owned, e.g. torch): kernels                        */
+  void*    stream_d2h;      /* cudaStream_t: offload copies                                            */
+  void*    stream_h2d;      /* cudaStream_t: restore copies                                            */
+} rc_config;
+
+typedef struct rc_claim_info {
+  uint64_t claim_id, chain, host_bytes;
+  uint32_t state, P, N, M, nb, n_table;
+} rc_claim_info;
+
+typedef struct rc_stats {
+  uint64_t bytes_d2h, bytes_h2d;         /* payload bytes moved over the host link                    */
+  uint64_t claims_offloaded, claims_restored, claims_refused;
+  uint64_t generic_failures;             /* unclaimed injected failures: a counter, never an outcome   */
+  uint64_t host_used_bytes, free_blocks, events_emitted, kernel_launches;
+  float    ms_gather, ms_scatter;        /* summed device time of the gather / scatter kernels         */
+  float    ms_d2h, ms_h2d;               /* summed device time of the copies (copy-stream events)      */
+  uint64_t gather_launches, scatter_launches, gather_blocks, scatter_blocks;
+} rc_stats;
+
+/* Creates a context.  page = BS*kv_heads*head_dim*elem_bytes must be a multiple of 4096
+ * (checksum lanes).  The library owns: staging ring (device), pinned host store, claim
+ * table, digests, allocator state, event ring, fault table.  All pool blocks start free. */
+int rc_create(const rc_config* cfg, rc_ctx** out);
+int rc_destroy(rc_ctx* ctx);
+
+/* Allocator hand-over: blocks the caller already filled become "used" (ref 0), or go back
+ * to free if no claim references them (claimed blocks are left alone). */
+int rc_mark_used(rc_ctx* ctx, uint32_t n, const uint32_t* block_ids);
+int rc_mark_free(rc_ctx* ctx, uint32_t n, const uint32_t* block_ids);
+
+/* a0. Records (C, P, N, block table) before any lifecycle event.  Table k is
+ * bt_ids[bt_off[k] .. bt_off[k+1]) and must have ceil(P/BS) distinct in-range used blocks.
+ * Emits ACCEPTED.  Statuses: OK, UNKNOWN_CLAIM (id 0 is reserved), DUPLICATE_ID, BAD_TABLE. */
+int rc_accept(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, const uint32_t* prefix_tokens,
+              const uint32_t* pred_min_tokens, const uint32_t* bt_off, const uint32_t* bt_ids,
+              int32_t* status);
+
+/* a1. Evaluates leading-prefix-at-least-N on the device from fill_dev: token t is materialized
+ * iff (t mod BS) < fill[bt[t div BS]]; M = leading run; holds iff M >= N.
+ * Emits MATERIALIZED for claims whose predicate holds; PRED_FALSE leaves the claim ACCEPTED. */
+int rc_materialize(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
+
+/* a1-a4. Gathers the nb = ceil(M/BS) leading blocks of every eligible claim (block-major, then
+ * page g = layer*2 + kv) through the staging ring into the pinned host store, digests each
+ * block while it streams, chains the digests per claim, drops the claim's references to ALL
+ * its table blocks and emits OFFLOADED.  Host space is granted in batch order;
+ * the first claim that does not fit and every later one get NO_HOST_SPACE. */
+int rc_offload(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
+
+/* a5-a8. For OFFLOADED claims: free blocks are granted in batch order against the free count
+ * at entry (NO_FREE_BLOCKS for the first claim that does not fit and all later ones); served
+ * claims take the lowest free ids ascending; host bytes are copied back, scattered into the
+ * new blocks, re-digested and compared with the recorded digests and chain.  Emits, per claim
+ * and consecutively, RESTORE_REQUIRED then RESTORED, or RESTORE_REQUIRED, LOAD_FAILED,
+ * RESTORATION_FAILED, ACTIVE_REQUEST_REFUSED (status RESTORE_FAILED; the claim is terminal,
+ * its new blocks are freed). */
+int rc_restore(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
+
+/* Drains up to cap not-yet-returned events in seq order. */
+int rc_outcomes(rc_ctx* ctx, rc_event* buf, uint64_t cap, uint64_t* n_out);
+
+/* Replaces the armed fault set (n = 0 disarms; default is disarmed).  A fault fires only in
+ * rc_restore (CPU->GPU) and only for the claim it names, once.  Entries with claim_id 0 are
+ * rejected (RC_ERR_INVALID) unless flags has RC_FAULT_ALLOW_UNCLAIMED; they only bump
+ * rc_stats.generic_failures. */
+int rc_set_faults(rc_ctx* ctx, uint32_t n, const rc_fault* faults, uint32_t flags);
+
+/* Forgets claims in any state, dropping block references and host bytes.  Emits nothing. */
+int rc_release(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
+
+/* Introspection (tests, parity). */
+int rc_claim_info(rc_ctx* ctx, uint64_t claim_id, rc_claim_info* out);
+int rc_claim_blocks(rc_ctx* ctx, uint64_t claim_id, uint32_t* ids, uint32_t cap, uint32_t* n);
+int rc_claim_digests(rc_ctx* ctx, uint64_t claim_id, uint64_t* d, uint32_t cap, uint32_t* n);
+int rc_host_read(rc_ctx* ctx, uint64_t claim_id, void* dst, uint64_t cap, uint64_t* bytes);
+int rc_pool_state(rc_ctx* ctx, uint8_t* used /*NB*/, uint32_t* ref /*NB*/);
+int rc_stats_get(rc_ctx* ctx, rc_stats* out);
+int rc_stats_reset(rc_ctx* ctx);
+
+/* Host-link ceiling: best-of-`reps` cudaMemcpyAsync of `bytes` between the context's pinned
+ * store and its staging ring; direction 0 = D2H, 1 = H2D, 2 = both at once.  GB/s. */
+int rc_measure_link(rc_ctx* ctx, uint64_t bytes, int direction, int reps, double* gbs);
+
+/* Standalone checksum of `n_blocks` contiguous blocks at DEVICE address src (offload order):
+ * the read-only digest pass used to report the checksum against the HBM roofline. */
+int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64_t* digests /*HOST*/);
+
+const char* rc_strerror(int err);
+const char* rc_last_cuda_error(rc_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
