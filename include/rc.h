@@ -19,9 +19,12 @@
  * array int32_t status[n] (RC_ST_*).  Any status other than RC_ST_OK and
  * RC_ST_RESTORE_FAILED means: no event was emitted for that claim by that call and
  * its state is unchanged.  All pointer arguments are HOST pointers unless marked
- * DEVICE.  Calls are synchronous: on return the device work is complete.  One caller
- * thread per context.  A CUDA error poisons the context: every later call returns
- * RC_ERR_CUDA.  There is no CPU fallback anywhere behind this interface.
+ * DEVICE.  Calls without a _begin suffix are synchronous: on return the device work
+ * is complete.  One caller thread per context.  A CUDA error poisons the context:
+ * every later call returns RC_ERR_CUDA.  A call-level error (negative return) emits
+ * no event and changes no claim.  There is no CPU fallback anywhere behind this
+ * interface: every step of the path runs in the library's sm_100a kernels and its
+ * copy-engine transfers.
  */
 #ifndef RC_H_
 #define RC_H_
@@ -32,7 +35,8 @@ extern "C" {
 
 typedef struct rc_ctx rc_ctx;
 
-enum { RC_OK = 0, RC_ERR_INVALID = -1, RC_ERR_CUDA = -2, RC_ERR_NOMEM = -3, RC_ERR_CAPACITY = -4 };
+enum { RC_OK = 0, RC_ERR_INVALID = -1, RC_ERR_CUDA = -2, RC_ERR_NOMEM = -3, RC_ERR_CAPACITY = -4,
+       RC_ERR_BUSY = -5 };
 
 /* per-claim status */
 enum { RC_ST_OK = 0, RC_ST_PRED_FALSE = 1, RC_ST_UNKNOWN_CLAIM = 2, RC_ST_BAD_STATE = 3,
@@ -56,30 +60,38 @@ enum { RC_CS_ACCEPTED = 1, RC_CS_MATERIALIZED = 2, RC_CS_OFFLOADED = 3, RC_CS_RE
 enum { RC_FAULT_XFER_ERROR = 1, RC_FAULT_BITFLIP = 2 };
 enum { RC_FAULT_ALLOW_UNCLAIMED = 1 };
 
+/* which data mover the gather / scatter launches use */
+enum { RC_MOVER_AUTO = 0, RC_MOVER_LDG = 1 /* 16-byte register copies */, RC_MOVER_TMA = 2 /* bulk-copy smem ring */ };
+
 typedef struct rc_event { uint64_t seq; uint64_t claim_id; uint32_t code; uint32_t aux; uint64_t arg; } rc_event;
 typedef struct rc_fault { uint64_t claim_id; uint32_t kind; uint32_t param; } rc_fault;
 
 typedef struct rc_config {
   uint32_t layers, kv_heads, head_dim, elem_bytes; /* elem_bytes: 1 (fp8) or 2 (bf16); bytes are never decoded */
-  uint32_t block_size;                 /* tokens per block (BS)                                       */
+  uint32_t block_size;                 /* tokens per block (BS), <= 255                               */
   uint32_t pool_blocks;                /* NB                                                          */
-  uint32_t max_claims;                 /* claim-table slots                                           */
+  uint32_t max_claims;                 /* live claims                                                 */
   uint32_t max_table_entries;          /* total block-table entries over all live claims              */
   uint32_t max_events;                 /* event ring capacity (records not yet drained)               */
-  uint32_t staging_chunks;             /* ring depth, >= 2                                            */
+  uint32_t staging_chunks;             /* ring depth per direction, >= 2                              */
   uint64_t staging_chunk_bytes;        /* rounded down to a multiple of blk = 2*L*page                */
   uint64_t host_store_bytes;           /* pinned host store, rounded down to a multiple of blk        */
   void*    pool_dev;   /* DEVICE, caller-owned: [layers][2][NB][BS][kv_heads][head_dim], 256-B aligned */
   uint8_t* fill_dev;   /* DEVICE, caller-owned u8[NB]: tokens materialized in each physical block     */
-  void*    stream_compute;  /* cudaStream_t (caller-owned, e.g. torch): kernels                        */
-  void*    stream_d2h;      /* cudaStream_t: offload copies                                            */
-  void*    stream_h2d;      /* cudaStream_t: restore copies                                            */
+  /* cudaStream_t, caller-owned (e.g. torch); any may be NULL and is then created by the library.   */
+  void*    stream_meta;     /* metadata kernels: their order on this stream is the order of calls    */
+  void*    stream_gather;   /* offload: gather + digest kernels                                      */
+  void*    stream_d2h;      /* offload: staging -> pinned host copies                                */
+  void*    stream_scatter;  /* restore: scatter + digest kernels                                     */
+  void*    stream_h2d;      /* restore: pinned host -> staging copies                                */
+  uint32_t mover;           /* RC_MOVER_*                                                            */
+  uint32_t grid_ctas;       /* CTAs of a gather / scatter launch; 0 = library default                */
 } rc_config;
 
-typedef struct rc_claim_info {
+typedef struct rc_claim_info_t {
   uint64_t claim_id, chain, host_bytes;
   uint32_t state, P, N, M, nb, n_table;
-} rc_claim_info;
+} rc_claim_info_t;
 
 typedef struct rc_stats {
   uint64_t bytes_d2h, bytes_h2d;         /* payload bytes moved over the host link                    */
@@ -92,7 +104,7 @@ typedef struct rc_stats {
 } rc_stats;
 
 /* Creates a context.  page = BS*kv_heads*head_dim*elem_bytes must be a multiple of 4096
- * (checksum lanes).  The library owns: staging ring (device), pinned host store, claim
+ * (checksum lanes).  The library owns: staging rings (device), pinned host store, claim
  * table, digests, allocator state, event ring, fault table.  All pool blocks start free. */
 int rc_create(const rc_config* cfg, rc_ctx** out);
 int rc_destroy(rc_ctx* ctx);
@@ -130,7 +142,18 @@ int rc_offload(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* statu
  * its new blocks are freed). */
 int rc_restore(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
 
-/* Drains up to cap not-yet-returned events in seq order. */
+/* Split forms (BASELINE.json configs[4]: restore of batch k overlapped with the offload of
+ * batch k+1).  _begin validates, enqueues all device work and returns; the status array must
+ * stay valid until rc_wait fills it in.  At most one offload and one restore may be in flight;
+ * their data movement runs on separate stream pairs and overlaps; their metadata steps
+ * (allocation, reference drops, verdicts, event emission) execute in _begin order, so the
+ * result equals the synchronous calls made in that order.  rc_restore_begin blocks only until
+ * its allocation plan is known.  which: 0 = offload, 1 = restore. */
+int rc_offload_begin(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
+int rc_restore_begin(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
+int rc_wait(rc_ctx* ctx, int which);
+
+/* Drains up to cap not-yet-returned events of completed calls, in seq order. */
 int rc_outcomes(rc_ctx* ctx, rc_event* buf, uint64_t cap, uint64_t* n_out);
 
 /* Replaces the armed fault set (n = 0 disarms; default is disarmed).  A fault fires only in
@@ -143,7 +166,7 @@ int rc_set_faults(rc_ctx* ctx, uint32_t n, const rc_fault* faults, uint32_t flag
 int rc_release(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
 
 /* Introspection (tests, parity). */
-int rc_claim_info(rc_ctx* ctx, uint64_t claim_id, rc_claim_info* out);
+int rc_claim_info(rc_ctx* ctx, uint64_t claim_id, rc_claim_info_t* out);
 int rc_claim_blocks(rc_ctx* ctx, uint64_t claim_id, uint32_t* ids, uint32_t cap, uint32_t* n);
 int rc_claim_digests(rc_ctx* ctx, uint64_t claim_id, uint64_t* d, uint32_t cap, uint32_t* n);
 int rc_host_read(rc_ctx* ctx, uint64_t claim_id, void* dst, uint64_t cap, uint64_t* bytes);
@@ -152,12 +175,13 @@ int rc_stats_get(rc_ctx* ctx, rc_stats* out);
 int rc_stats_reset(rc_ctx* ctx);
 
 /* Host-link ceiling: best-of-`reps` cudaMemcpyAsync of `bytes` between the context's pinned
- * store and its staging ring; direction 0 = D2H, 1 = H2D, 2 = both at once.  GB/s. */
+ * store and its staging ring; direction 0 = D2H, 1 = H2D, 2 = both at once (sum).  GB/s. */
 int rc_measure_link(rc_ctx* ctx, uint64_t bytes, int direction, int reps, double* gbs);
 
 /* Standalone checksum of `n_blocks` contiguous blocks at DEVICE address src (offload order):
- * the read-only digest pass used to report the checksum against the HBM roofline. */
-int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64_t* digests /*HOST*/);
+ * the read-only digest pass used to report the checksum against the HBM roofline.  digests is
+ * a HOST array (may be NULL); ms (may be NULL) receives the device time of the digest kernel. */
+int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64_t* digests, float* ms);
 
 const char* rc_strerror(int err);
 const char* rc_last_cuda_error(rc_ctx* ctx);

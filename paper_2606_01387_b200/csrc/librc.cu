@@ -1,0 +1,1058 @@
+// librc.cu -- host side of librc: the C ABI of include/rc.h, the claim table, the extent
+// allocators (block-table arena, digest arena, pinned host store) and the transfer engine
+// (staging rings, gather/scatter streams, copy streams, events).  Every step of the path runs in
+// the kernels of rc_kernels.cuh or on the copy engines; the host only validates arguments,
+// orders the work and mirrors claim state.  There is no CPU fallback: without a CUDA device
+// rc_create fails with RC_ERR_CUDA.
+//
+// Ordering model: metadata kernels (accept, predicate, plan/allocation,
+// reference drops, verdicts, event emission) all run on ONE in-order stream, `meta`, in call
+// order; bulk movement runs on (gather, d2h) for offload and (scatter, h2d) for restore and is
+// fenced to `meta` with events.  So an offload and a restore may overlap their data movement
+// while every observable result equals the synchronous calls in _begin order.
+#include "../../include/rc.h"
+#include "rc_kernels.cuh"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include <unordered_map>
+#include <unordered_set>
+#include <vector>
+
+using namespace rck;
+
+namespace {
+
+// first-fit extent allocator over [0, cap) units; free extents kept merged in address order
+struct ExtAlloc {
+  std::map<u64, u64> fr;
+  u64 cap = 0, free_total = 0;
+  void init(u64 c) { fr.clear(); cap = free_total = c; if (c) fr[0] = c; }
+  bool alloc(u64 n, u64& off) {
+    if (n == 0) { off = 0; return true; }
+    for (auto it = fr.begin(); it != fr.end(); ++it)
+      if (it->second >= n) {
+        off = it->first;
+        const u64 rest = it->second - n;
+        fr.erase(it);
+        if (rest) fr[off + n] = rest;
+        free_total -= n;
+        return true;
+      }
+    return false;
+  }
+  // n units in as few pieces as the free list allows, lowest addresses first (never fails when
+  // free_total >= n: the host store is granted by byte count, not by contiguity)
+  bool alloc_split(u64 n, std::vector<std::pair<u64, u64>>& out) {
+    if (n > free_total) return false;
+    u64 o;
+    if (alloc(n, o)) { out.push_back({o, n}); return true; }
+    while (n) {
+      auto it = fr.begin();
+      const u64 take = std::min(n, it->second), at = it->first, rest = it->second - take;
+      fr.erase(it);
+      if (rest) fr[at + take] = rest;
+      free_total -= take;
+      out.push_back({at, take});
+      n -= take;
+    }
+    return true;
+  }
+  void release(u64 off, u64 n) {
+    if (!n) return;
+    auto nx = fr.lower_bound(off);
+    if (nx != fr.begin()) {
+      auto pv = std::prev(nx);
+      if (pv->first + pv->second == off) { off = pv->first; n += pv->second; fr.erase(pv); }
+    }
+    if (nx != fr.end() && off + n == nx->first) { n += nx->second; fr.erase(nx); }
+    fr[off] = n;
+    free_total += (n - 0);
+  }
+};
+
+struct Claim {
+  u64 id = 0, chain = 0;
+  u32 state = 0, P = 0, N = 0, M = 0, nb = 0;
+  u32 bt_off = 0, bt_len = 0;            // live table extent (bt_len == 0: no table)
+  u32 dg_off = 0, dg_len = 0;            // recorded digests
+  std::vector<std::pair<u64, u64>> host; // host-store extents in blk units
+  bool busy = false;
+};
+
+struct Seg { u64 w0, n, hoff; };          // n blocks at work position w0 <-> host-store block hoff
+
+struct Op {
+  bool active = false;
+  u32 n = 0;
+  int32_t* status = nullptr;
+  std::vector<Claim*> cl;                 // per batch entry: served claim or nullptr
+  std::vector<u32> new_bt;                // restore: new table extent offset per entry
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> t_kernel, t_copy;
+  u64 blocks = 0, copy_bytes = 0, launches = 0;
+  cudaEvent_t done = nullptr;
+};
+
+}  // namespace
+
+struct rc_ctx {
+  rc_config cfg;
+  u32 G = 0, vpp = 0, NB = 0, R = 0, sms = 0, grid = 0, tile = 0, mover = 0;
+  u64 page = 0, blk = 0, chunk_blocks = 0, host_blocks = 0, cap_entries = 0, desc_cap = 0;
+  cudaStream_t meta = 0, gather = 0, d2h = 0, scatter = 0, h2d = 0, util = 0;
+  bool own[5] = {false, false, false, false, false};
+  u8* pool = nullptr; u8* fill = nullptr;
+  u8* d_used = nullptr; u32* d_ref = nullptr; u32* d_bt = nullptr; u64* d_dg = nullptr;
+  Event* d_ring = nullptr; u64* d_evcount = nullptr; u32* d_bitmaps = nullptr; u32* d_up = nullptr;
+  u32* d_counters = nullptr; u32* d_alloc = nullptr; u64* d_flip = nullptr;
+  Desc* d_desc[3] = {}; Res* d_res[3] = {}; u32* d_off[3] = {};
+  Desc* h_desc[3] = {}; Res* h_res[3] = {};
+  u32* h_up = nullptr; u64* h_flip = nullptr; u32* h_counters = nullptr;
+  u32* d_phys[2] = {}; u64* d_dtmp[2] = {};
+  std::vector<u8*> staging[2]; std::vector<u64*> part[2];
+  std::vector<cudaEvent_t> ev_free[2], ev_ready[2];
+  std::vector<bool> slot_used[2];
+  cudaEvent_t ev_plan[2] = {}, ev_body_a[2] = {}, ev_body_b[2] = {};
+  std::vector<cudaEvent_t> ev_pool;
+  u8* h_store = nullptr;
+  ExtAlloc host_alloc, bt_alloc, dg_alloc;
+  u64 host_used = 0;
+  std::unordered_map<u64, Claim> claims;
+  std::vector<rc_fault> faults; u32 fault_flags = 0;
+  u64 ev_emitted = 0, ev_drained = 0, ev_reserved = 0;
+  rc_stats st;
+  Op ops[2];
+  bool poisoned = false;
+  std::string cuda_err;
+  int accept_ctas = 32;
+};
+
+#define CK(call)                                                                      \
+  do {                                                                                \
+    cudaError_t e_ = (call);                                                          \
+    if (e_ != cudaSuccess) {                                                          \
+      c->poisoned = true;                                                             \
+      c->cuda_err = std::string(#call) + ": " + cudaGetErrorString(e_);               \
+      return RC_ERR_CUDA;                                                             \
+    }                                                                                 \
+  } while (0)
+#define CKL() CK(cudaGetLastError())
+
+static inline u32 ceil_div(u32 a, u32 b) { return (a + b - 1) / b; }
+static inline u32 warps_grid(u32 n) { return (n * 32 + 255) / 256; }
+
+static cudaEvent_t get_event(rc_ctx* c) {
+  if (!c->ev_pool.empty()) { cudaEvent_t e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+
+// ---- data movers -----------------------------------------------------------------------------
+template <int MODE>
+static void launch_ldg(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
+  const u32 pages = n_items * c->G;
+  const u32 grid = std::min(pages, c->grid);
+  const u32 vpt = c->vpp / LANES;
+  if (vpt % 8 == 0)
+    k_move_hash<MODE, 8><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp);
+  else if (vpt % 4 == 0)
+    k_move_hash<MODE, 4><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp);
+  else
+    k_move_hash<MODE, 1><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp);
+}
+
+constexpr int TMA_STAGES = 4;
+template <int MODE, int TILE>
+static void launch_tma_t(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
+  const u32 pages = n_items * c->G;
+  const u32 grid = std::min(pages, c->grid);
+  k_move_hash_tma<MODE, TMA_STAGES, TILE><<<grid, LANES, TMA_STAGES * TILE, s>>>(c->pool, staging, phys, part, n_items,
+                                                                             c->G, c->NB, (u32)c->page);
+}
+template <int MODE>
+static void launch_tma(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
+  if (c->tile == 16384) launch_tma_t<MODE, 16384>(c, s, staging, phys, part, n_items);
+  else if (c->tile == 8192) launch_tma_t<MODE, 8192>(c, s, staging, phys, part, n_items);
+  else launch_tma_t<MODE, 4096>(c, s, staging, phys, part, n_items);
+}
+template <int MODE>
+static void launch_move(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
+  if (c->mover == RC_MOVER_TMA) launch_tma<MODE>(c, s, staging, phys, part, n_items);
+  else launch_ldg<MODE>(c, s, staging, phys, part, n_items);
+  c->st.kernel_launches++;
+}
+
+template <int MODE, int TILE>
+static cudaError_t tma_attr(int& occ) {
+  cudaError_t e = cudaFuncSetAttribute(k_move_hash_tma<MODE, TMA_STAGES, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       TMA_STAGES * TILE);
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hash_tma<MODE, TMA_STAGES, TILE>, LANES,
+                                                       TMA_STAGES * TILE);
+}
+
+// ---- create / destroy ------------------------------------------------------------------------
+extern "C" int rc_destroy(rc_ctx* c) {
+  if (!c) return RC_ERR_INVALID;
+  cudaDeviceSynchronize();
+  auto F = [](void* p) { if (p) cudaFree(p); };
+  auto FH = [](void* p) { if (p) cudaFreeHost(p); };
+  F(c->d_used); F(c->d_ref); F(c->d_bt); F(c->d_dg); F(c->d_ring); F(c->d_evcount); F(c->d_bitmaps); F(c->d_up);
+  F(c->d_counters); F(c->d_alloc); F(c->d_flip);
+  for (int i = 0; i < 3; ++i) { F(c->d_desc[i]); F(c->d_res[i]); F(c->d_off[i]); FH(c->h_desc[i]); FH(c->h_res[i]); }
+  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store);
+  for (int d = 0; d < 2; ++d) {
+    F(c->d_phys[d]); F(c->d_dtmp[d]);
+    for (auto p : c->staging[d]) F(p);
+    for (auto p : c->part[d]) F(p);
+    for (auto e : c->ev_free[d]) cudaEventDestroy(e);
+    for (auto e : c->ev_ready[d]) cudaEventDestroy(e);
+    if (c->ev_plan[d]) cudaEventDestroy(c->ev_plan[d]);
+    if (c->ev_body_a[d]) cudaEventDestroy(c->ev_body_a[d]);
+    if (c->ev_body_b[d]) cudaEventDestroy(c->ev_body_b[d]);
+    if (c->ops[d].done) cudaEventDestroy(c->ops[d].done);
+  }
+  for (auto e : c->ev_pool) cudaEventDestroy(e);
+  cudaStream_t* ss[5] = {&c->meta, &c->gather, &c->d2h, &c->scatter, &c->h2d};
+  for (int i = 0; i < 5; ++i) if (c->own[i] && *ss[i]) cudaStreamDestroy(*ss[i]);
+  if (c->util) cudaStreamDestroy(c->util);
+  delete c;
+  return RC_OK;
+}
+
+extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
+  if (!cfg || !out) return RC_ERR_INVALID;
+  *out = nullptr;
+  const u64 page = (u64)cfg->block_size * cfg->kv_heads * cfg->head_dim * cfg->elem_bytes;
+  if (!cfg->layers || !cfg->pool_blocks || page == 0 || page % 4096 != 0 || page > (1ull << 30)) return RC_ERR_INVALID;
+  if (cfg->elem_bytes != 1 && cfg->elem_bytes != 2) return RC_ERR_INVALID;
+  if (cfg->block_size > 255 || !cfg->pool_dev || !cfg->fill_dev || ((uintptr_t)cfg->pool_dev & 255)) return RC_ERR_INVALID;
+  if (!cfg->max_claims || !cfg->max_table_entries || !cfg->max_events || cfg->staging_chunks < 2) return RC_ERR_INVALID;
+  const u64 blk = 2ull * cfg->layers * page;
+  if (cfg->staging_chunk_bytes < blk || cfg->mover > RC_MOVER_TMA) return RC_ERR_INVALID;
+  if ((cfg->staging_chunk_bytes / blk) * (2ull * cfg->layers) > 0x7FFFFFFFull) return RC_ERR_INVALID;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return RC_ERR_CUDA;   // no device, no library
+  rc_ctx* c = new rc_ctx();
+  c->cfg = *cfg;
+  c->page = page; c->blk = blk; c->G = 2 * cfg->layers; c->vpp = (u32)(page / 16); c->NB = cfg->pool_blocks;
+  c->R = cfg->staging_chunks;
+  c->chunk_blocks = cfg->staging_chunk_bytes / blk;
+  c->host_blocks = cfg->host_store_bytes / blk;
+  c->cap_entries = cfg->max_table_entries;
+  c->desc_cap = 2ull * cfg->max_claims + 1024;
+  c->pool = (u8*)cfg->pool_dev; c->fill = cfg->fill_dev;
+  memset(&c->st, 0, sizeof(c->st));
+  c->host_alloc.init(c->host_blocks); c->bt_alloc.init(c->cap_entries); c->dg_alloc.init(c->cap_entries);
+  auto fail = [&](int code, const char* what, cudaError_t e) {
+    fprintf(stderr, "librc: rc_create failed at %s: %s\n", what, e == cudaSuccess ? "" : cudaGetErrorString(e));
+    rc_destroy(c);
+    return code;
+  };
+#define CC(call, code) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(code, #call, e_); } while (0)
+  cudaDeviceProp prop;
+  int dev = 0;
+  CC(cudaGetDevice(&dev), RC_ERR_CUDA);
+  CC(cudaGetDeviceProperties(&prop, dev), RC_ERR_CUDA);
+  c->sms = prop.multiProcessorCount;
+  void* given[5] = {cfg->stream_meta, cfg->stream_gather, cfg->stream_d2h, cfg->stream_scatter, cfg->stream_h2d};
+  cudaStream_t* ss[5] = {&c->meta, &c->gather, &c->d2h, &c->scatter, &c->h2d};
+  for (int i = 0; i < 5; ++i) {
+    if (given[i]) *ss[i] = (cudaStream_t)given[i];
+    else { CC(cudaStreamCreateWithFlags(ss[i], cudaStreamNonBlocking), RC_ERR_CUDA); c->own[i] = true; }
+  }
+  CC(cudaStreamCreateWithFlags(&c->util, cudaStreamNonBlocking), RC_ERR_CUDA);
+  const u64 NB = c->NB, cap = c->cap_entries, dc = c->desc_cap;
+  CC(cudaMalloc(&c->d_used, NB), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_ref, NB * 4), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_bt, cap * 4), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_dg, cap * 8), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_ring, (u64)cfg->max_events * sizeof(Event)), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_evcount, 8), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_bitmaps, (u64)c->accept_ctas * ((NB + 31) / 32) * 4), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_up, cap * 4), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_counters, 16), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_alloc, cap * 4), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_flip, dc * 8), RC_ERR_NOMEM);
+  CC(cudaMemset(c->d_used, 0, NB), RC_ERR_CUDA);
+  CC(cudaMemset(c->d_ref, 0, NB * 4), RC_ERR_CUDA);
+  CC(cudaMemset(c->d_evcount, 0, 8), RC_ERR_CUDA);
+  CC(cudaMemset(c->d_bitmaps, 0, (u64)c->accept_ctas * ((NB + 31) / 32) * 4), RC_ERR_CUDA);
+  for (int i = 0; i < 3; ++i) {
+    CC(cudaMalloc(&c->d_desc[i], dc * sizeof(Desc)), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_res[i], dc * sizeof(Res)), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_off[i], (dc + 1) * 4), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_desc[i], dc * sizeof(Desc), cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_res[i], dc * sizeof(Res), cudaHostAllocDefault), RC_ERR_NOMEM);
+  }
+  CC(cudaHostAlloc(&c->h_up, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
+  CC(cudaHostAlloc(&c->h_flip, dc * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
+  CC(cudaHostAlloc(&c->h_counters, 16, cudaHostAllocDefault), RC_ERR_NOMEM);
+  for (int d = 0; d < 2; ++d) {
+    CC(cudaMalloc(&c->d_phys[d], cap * 4), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_dtmp[d], cap * 8), RC_ERR_NOMEM);
+    c->staging[d].assign(c->R, nullptr); c->part[d].assign(c->R, nullptr);
+    c->ev_free[d].assign(c->R, nullptr); c->ev_ready[d].assign(c->R, nullptr);
+    c->slot_used[d].assign(c->R, false);
+    for (u32 r = 0; r < c->R; ++r) {
+      CC(cudaMalloc(&c->staging[d][r], c->chunk_blocks * blk), RC_ERR_NOMEM);
+      CC(cudaMalloc(&c->part[d][r], c->chunk_blocks * c->G * WPC * 8), RC_ERR_NOMEM);
+      CC(cudaEventCreateWithFlags(&c->ev_free[d][r], cudaEventDisableTiming), RC_ERR_CUDA);
+      CC(cudaEventCreateWithFlags(&c->ev_ready[d][r], cudaEventDisableTiming), RC_ERR_CUDA);
+    }
+    CC(cudaEventCreateWithFlags(&c->ev_plan[d], cudaEventDisableTiming), RC_ERR_CUDA);
+    CC(cudaEventCreateWithFlags(&c->ev_body_a[d], cudaEventDisableTiming), RC_ERR_CUDA);
+    CC(cudaEventCreateWithFlags(&c->ev_body_b[d], cudaEventDisableTiming), RC_ERR_CUDA);
+    CC(cudaEventCreateWithFlags(&c->ops[d].done, cudaEventDisableTiming), RC_ERR_CUDA);
+  }
+  if (c->host_blocks) CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocDefault), RC_ERR_NOMEM);
+  // launch geometry of the movers
+  c->mover = cfg->mover == RC_MOVER_AUTO ? RC_MOVER_TMA : cfg->mover;
+  c->tile = page % 16384 == 0 ? 16384 : (page % 8192 == 0 ? 8192 : 4096);
+  int occ = 0;
+  if (c->mover == RC_MOVER_TMA) {
+    int o2 = 0, o3 = 0;
+    if (c->tile == 16384) {
+      CC((tma_attr<MV_GATHER, 16384>(occ)), RC_ERR_CUDA); CC((tma_attr<MV_SCATTER, 16384>(o2)), RC_ERR_CUDA);
+      CC((tma_attr<MV_DIGEST, 16384>(o3)), RC_ERR_CUDA);
+    } else if (c->tile == 8192) {
+      CC((tma_attr<MV_GATHER, 8192>(occ)), RC_ERR_CUDA); CC((tma_attr<MV_SCATTER, 8192>(o2)), RC_ERR_CUDA);
+      CC((tma_attr<MV_DIGEST, 8192>(o3)), RC_ERR_CUDA);
+    } else {
+      CC((tma_attr<MV_GATHER, 4096>(occ)), RC_ERR_CUDA); CC((tma_attr<MV_SCATTER, 4096>(o2)), RC_ERR_CUDA);
+      CC((tma_attr<MV_DIGEST, 4096>(o3)), RC_ERR_CUDA);
+    }
+    occ = std::min(occ, std::min(o2, o3));
+  } else {
+    CC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hash<MV_GATHER, 8>, LANES, 0), RC_ERR_CUDA);
+  }
+  if (occ < 1) occ = 1;
+  c->grid = cfg->grid_ctas ? cfg->grid_ctas : c->sms * (u32)occ;
+#undef CC
+  *out = c;
+  return RC_OK;
+}
+
+// ---- small helpers -----------------------------------------------------------------------------
+static int ev_room(rc_ctx* c, u64 extra) {
+  return (c->ev_emitted - c->ev_drained) + c->ev_reserved + extra <= c->cfg.max_events;
+}
+static int upload_desc(rc_ctx* c, int set, u32 n) {
+  CK(cudaMemcpyAsync(c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc), cudaMemcpyHostToDevice, c->meta));
+  return RC_OK;
+}
+static int fetch_res(rc_ctx* c, int set, u32 n) {
+  CK(cudaMemcpyAsync(c->h_res[set], c->d_res[set], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
+  return RC_OK;
+}
+static int emit(rc_ctx* c, int set, u32 n, int mode) {
+  k_emit<<<1, 256, 0, c->meta>>>(c->d_desc[set], c->d_res[set], n, mode, c->d_ring, c->cfg.max_events, c->d_evcount);
+  CKL();
+  c->st.kernel_launches++;
+  return RC_OK;
+}
+#define GUARD()                                   \
+  if (!c) return RC_ERR_INVALID;                  \
+  if (c->poisoned) return RC_ERR_CUDA
+
+static int mark(rc_ctx* c, u32 n, const u32* ids, int val) {
+  GUARD();
+  if (n && !ids) return RC_ERR_INVALID;
+  for (u32 i = 0; i < n; ++i) if (ids[i] >= c->NB) return RC_ERR_INVALID;
+  for (u32 s = 0; s < n; s += (u32)c->cap_entries) {
+    const u32 m = (u32)std::min<u64>(n - s, c->cap_entries);
+    memcpy(c->h_up, ids + s, (u64)m * 4);
+    CK(cudaMemcpyAsync(c->d_up, c->h_up, (u64)m * 4, cudaMemcpyHostToDevice, c->meta));
+    k_mark<<<(m + 255) / 256, 256, 0, c->meta>>>(c->d_up, m, c->d_used, c->d_ref, val);
+    CKL();
+    c->st.kernel_launches++;
+    CK(cudaStreamSynchronize(c->meta));
+  }
+  return RC_OK;
+}
+extern "C" int rc_mark_used(rc_ctx* c, uint32_t n, const uint32_t* ids) { return mark(c, n, ids, 1); }
+extern "C" int rc_mark_free(rc_ctx* c, uint32_t n, const uint32_t* ids) { return mark(c, n, ids, 0); }
+
+// ---- a0 accept -----------------------------------------------------------------------------------
+static int accept_run(rc_ctx* c, u32 n, const u64* id, const u32* P, const u32* N, const u32* bt_off, const u32* bt_ids,
+                      int32_t* st) {
+  Desc* hd = c->h_desc[2];
+  std::vector<u32> cand;
+  u64 up = 0;
+  auto rollback = [&]() { for (u32 k : cand) c->bt_alloc.release(hd[k].bt_off, hd[k].bt_len); };
+  for (u32 k = 0; k < n; ++k) {
+    memset(&hd[k], 0, sizeof(Desc));
+    hd[k].id = id[k];
+    if (id[k] == 0) { st[k] = RC_ST_UNKNOWN_CLAIM; continue; }          // 0 is "no claim"
+    if (c->claims.count(id[k])) { st[k] = RC_ST_DUPLICATE_ID; continue; } // duplicate ownership
+    if (P[k] == 0 || N[k] == 0 || N[k] > P[k] || bt_off[k + 1] < bt_off[k] ||
+        bt_off[k + 1] - bt_off[k] != ceil_div(P[k], c->cfg.block_size)) { st[k] = RC_ST_BAD_TABLE; continue; }
+    const u32 nt = bt_off[k + 1] - bt_off[k];
+    u64 o;
+    if (up + nt > c->cap_entries || !c->bt_alloc.alloc(nt, o)) { rollback(); return RC_ERR_CAPACITY; }
+    hd[k].P = P[k]; hd[k].N = N[k]; hd[k].bt_off = (u32)o; hd[k].bt_len = nt; hd[k].flags = D_ELIG;
+    hd[k].src_off = (u32)up;
+    memcpy(c->h_up + up, bt_ids + bt_off[k], (u64)nt * 4);
+    up += nt;
+    cand.push_back(k);
+    st[k] = -1;
+  }
+  if (cand.empty()) return RC_OK;
+  int rc;
+  if ((rc = upload_desc(c, 2, n))) return rc;
+  CK(cudaMemcpyAsync(c->d_up, c->h_up, up * 4, cudaMemcpyHostToDevice, c->meta));
+  k_accept<<<std::min<u32>(n, c->accept_ctas), 256, 0, c->meta>>>(c->d_desc[2], c->d_res[2], n, c->d_up, c->d_bt, c->d_used,
+                                                                 c->d_ref, c->NB, c->d_bitmaps);
+  CKL();
+  c->st.kernel_launches++;
+  if ((rc = emit(c, 2, n, EM_ACCEPT))) return rc;
+  if ((rc = fetch_res(c, 2, n))) return rc;
+  CK(cudaStreamSynchronize(c->meta));
+  for (u32 k : cand) {
+    if (c->h_res[2][k].flag & R_OK) {
+      Claim cl;
+      cl.id = id[k]; cl.state = RC_CS_ACCEPTED; cl.P = P[k]; cl.N = N[k];
+      cl.bt_off = hd[k].bt_off; cl.bt_len = hd[k].bt_len;
+      c->claims.emplace(id[k], std::move(cl));
+      c->ev_emitted++;
+      st[k] = RC_ST_OK;
+    } else {
+      c->bt_alloc.release(hd[k].bt_off, hd[k].bt_len);
+      st[k] = RC_ST_BAD_TABLE;
+    }
+  }
+  return RC_OK;
+}
+
+extern "C" int rc_accept(rc_ctx* c, uint32_t n, const uint64_t* id, const uint32_t* P, const uint32_t* N,
+                         const uint32_t* bt_off, const uint32_t* bt_ids, int32_t* st) {
+  GUARD();
+  if (n == 0) return RC_OK;
+  if (!id || !P || !N || !bt_off || !st || (bt_off[n] && !bt_ids)) return RC_ERR_INVALID;
+  if (c->claims.size() + n > c->cfg.max_claims || !ev_room(c, n)) return RC_ERR_CAPACITY;
+  // a run never holds the same id twice, so the runs reproduce one-by-one acceptance
+  u32 s = 0;
+  while (s < n) {
+    std::unordered_set<u64> seen;
+    u32 e = s;
+    while (e < n && e - s < c->desc_cap && (id[e] == 0 || seen.insert(id[e]).second)) ++e;
+    const int rc = accept_run(c, e - s, id + s, P + s, N + s, bt_off + s, bt_ids, st + s);
+    if (rc) return rc;
+    s = e;
+  }
+  return RC_OK;
+}
+
+// ---- a1 materialize --------------------------------------------------------------------------------
+extern "C" int rc_materialize(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
+  GUARD();
+  if (n == 0) return RC_OK;
+  if (!id || !st || n > c->desc_cap) return RC_ERR_INVALID;
+  if (!ev_room(c, n)) return RC_ERR_CAPACITY;
+  Desc* hd = c->h_desc[2];
+  std::unordered_map<u64, u32> first;
+  std::vector<std::pair<u32, u32>> dups;
+  std::vector<u32> cand;
+  for (u32 k = 0; k < n; ++k) {
+    memset(&hd[k], 0, sizeof(Desc));
+    hd[k].id = id[k];
+    auto it = c->claims.find(id[k]);
+    if (it == c->claims.end()) { st[k] = RC_ST_UNKNOWN_CLAIM; continue; }   // post-hoc naming
+    Claim& cl = it->second;
+    if (cl.busy || cl.state != RC_CS_ACCEPTED) { st[k] = RC_ST_BAD_STATE; continue; }
+    auto f = first.find(id[k]);
+    if (f != first.end()) { dups.push_back({k, f->second}); continue; }
+    first[id[k]] = k;
+    hd[k].P = cl.P; hd[k].N = cl.N; hd[k].bt_off = cl.bt_off; hd[k].bt_len = cl.bt_len; hd[k].flags = D_ELIG;
+    cand.push_back(k);
+  }
+  if (!cand.empty()) {
+    int rc;
+    if ((rc = upload_desc(c, 2, n))) return rc;
+    k_pred<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[2], c->d_res[2], n, c->d_bt, c->fill, c->cfg.block_size);
+    CKL();
+    c->st.kernel_launches++;
+    if ((rc = emit(c, 2, n, EM_MATERIALIZE))) return rc;
+    if ((rc = fetch_res(c, 2, n))) return rc;
+    CK(cudaStreamSynchronize(c->meta));
+    for (u32 k : cand) {
+      const Res r = c->h_res[2][k];
+      if (r.flag & R_OK) {
+        Claim& cl = c->claims[id[k]];
+        cl.M = r.val; cl.nb = ceil_div(r.val, c->cfg.block_size); cl.state = RC_CS_MATERIALIZED;
+        c->ev_emitted++;
+        st[k] = RC_ST_OK;
+      } else st[k] = RC_ST_PRED_FALSE;
+    }
+  }
+  for (auto& d : dups) st[d.first] = st[d.second] == RC_ST_OK ? RC_ST_BAD_STATE : RC_ST_PRED_FALSE;
+  return RC_OK;
+}
+
+// ---- transfer engine helpers --------------------------------------------------------------------
+// copies the host-store segments that intersect work positions [w0, w1) of a chunk
+static int copy_chunk(rc_ctx* c, int dir, cudaStream_t s, u8* stg, u64 w0, u64 w1, const std::vector<Seg>& segs, size_t& si,
+                      u64& bytes) {
+  u8 *ha = nullptr, *da = nullptr; u64 len = 0;
+  auto flush = [&]() -> cudaError_t {
+    if (!len) return cudaSuccess;
+    cudaError_t e = dir == 0 ? cudaMemcpyAsync(ha, da, len, cudaMemcpyDeviceToHost, s)
+                             : cudaMemcpyAsync(da, ha, len, cudaMemcpyHostToDevice, s);
+    bytes += len; len = 0;
+    return e;
+  };
+  while (si < segs.size() && segs[si].w0 < w1) {
+    const Seg& g = segs[si];
+    const u64 a = std::max(g.w0, w0), b = std::min(g.w0 + g.n, w1);
+    if (a < b) {
+      u8* h = c->h_store + (g.hoff + (a - g.w0)) * c->blk;
+      u8* d = stg + (a - w0) * c->blk;
+      const u64 l = (b - a) * c->blk;
+      if (len && h == ha + len && d == da + len) len += l;
+      else { CK(flush()); ha = h; da = d; len = l; }
+    }
+    if (g.w0 + g.n <= w1) ++si; else break;
+  }
+  CK(flush());
+  return RC_OK;
+}
+
+extern "C" int rc_wait(rc_ctx* c, int which);
+// ---- a1-a4 offload ------------------------------------------------------------------------------------
+extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
+  GUARD();
+  Op& op = c->ops[0];
+  if (op.active) return RC_ERR_BUSY;
+  if (n == 0) return RC_OK;
+  if (!id || !st || n > c->desc_cap) return RC_ERR_INVALID;
+  if (!ev_room(c, n)) return RC_ERR_CAPACITY;
+  Desc* hd = c->h_desc[0];
+  op.cl.assign(n, nullptr);
+  std::vector<Seg> segs;
+  std::vector<u32> served;
+  bool full = false;
+  u64 T = 0;
+  auto rollback = [&]() {
+    for (u32 k : served) {
+      Claim& cl = *op.cl[k];
+      for (auto& e : cl.host) c->host_alloc.release(e.first, e.second);
+      cl.host.clear();
+      c->host_used -= (u64)cl.nb * c->blk;
+      if (cl.dg_len) { c->dg_alloc.release(cl.dg_off, cl.dg_len); cl.dg_len = 0; }
+      cl.busy = false;
+    }
+  };
+  for (u32 k = 0; k < n; ++k) {
+    memset(&hd[k], 0, sizeof(Desc));
+    hd[k].id = id[k];
+    auto it = c->claims.find(id[k]);
+    if (it == c->claims.end()) { st[k] = RC_ST_UNKNOWN_CLAIM; continue; }
+    Claim& cl = it->second;
+    // no claim-less entry point exists: "ordinary offload without claim" cannot produce an outcome
+    if (cl.busy || (cl.state != RC_CS_MATERIALIZED && cl.state != RC_CS_RESIDENT_AGAIN)) { st[k] = RC_ST_BAD_STATE; continue; }
+    if (full || c->host_used + (u64)cl.nb * c->blk > c->cfg.host_store_bytes) { full = true; st[k] = RC_ST_NO_HOST_SPACE; continue; }
+    if (cl.dg_len) { c->dg_alloc.release(cl.dg_off, cl.dg_len); cl.dg_len = 0; }
+    u64 dgo;
+    if (T + cl.nb > c->cap_entries || !c->dg_alloc.alloc(cl.nb, dgo)) { rollback(); return RC_ERR_CAPACITY; }
+    cl.dg_off = (u32)dgo; cl.dg_len = cl.nb;
+    cl.host.clear();
+    // host space is granted by count in _begin order; the extents of a restore still in flight are
+    // physically released when it completes
+    if (c->host_alloc.free_total < cl.nb && c->ops[1].active) { const int wr = rc_wait(c, 1); if (wr) return wr; }
+    c->host_alloc.alloc_split(cl.nb, cl.host);
+    c->host_used += (u64)cl.nb * c->blk;
+    cl.busy = true;
+    op.cl[k] = &cl;
+    served.push_back(k);
+    hd[k].P = cl.P; hd[k].N = cl.N; hd[k].M = cl.M; hd[k].nb = cl.nb; hd[k].bt_off = cl.bt_off; hd[k].bt_len = cl.bt_len;
+    hd[k].dg_off = cl.dg_off; hd[k].flags = D_ELIG;
+    u64 w = T;
+    for (auto& e : cl.host) { segs.push_back({w, e.second, e.first}); w += e.second; }
+    T += cl.nb;
+    st[k] = -1;
+  }
+  if (served.empty()) return RC_OK;
+  op.n = n; op.status = st; op.blocks = T; op.copy_bytes = 0; op.launches = 0;
+  int rc;
+  if ((rc = upload_desc(c, 0, n))) return rc;
+  k_offsets<<<1, 1024, 0, c->meta>>>(c->d_desc[0], n, c->d_off[0]);
+  CKL();
+  k_worklist<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_bt, nullptr, c->d_phys[0], 0);
+  CKL();
+  c->st.kernel_launches += 2;
+  CK(cudaEventRecord(c->ev_plan[0], c->meta));
+  CK(cudaStreamWaitEvent(c->gather, c->ev_plan[0], 0));
+  size_t si = 0;
+  u32 ci = 0;
+  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks, ++ci) {
+    const u64 w1 = std::min(T, w0 + c->chunk_blocks);
+    const u32 slot = ci % c->R, m = (u32)(w1 - w0);
+    if (c->slot_used[0][slot]) CK(cudaStreamWaitEvent(c->gather, c->ev_free[0][slot], 0));
+    cudaEvent_t t0 = get_event(c), t1 = get_event(c);
+    CK(cudaEventRecord(t0, c->gather));
+    launch_move<MV_GATHER>(c, c->gather, c->staging[0][slot], c->d_phys[0] + w0, c->part[0][slot], m);
+    CKL();
+    CK(cudaEventRecord(t1, c->gather));
+    op.t_kernel.push_back({t0, t1});
+    op.launches++;
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, m, c->G);
+    CKL();
+    c->st.kernel_launches++;
+    CK(cudaEventRecord(c->ev_ready[0][slot], c->gather));
+    CK(cudaStreamWaitEvent(c->d2h, c->ev_ready[0][slot], 0));
+    cudaEvent_t c0 = get_event(c), c1 = get_event(c);
+    CK(cudaEventRecord(c0, c->d2h));
+    if ((rc = copy_chunk(c, 0, c->d2h, c->staging[0][slot], w0, w1, segs, si, op.copy_bytes))) return rc;
+    CK(cudaEventRecord(c1, c->d2h));
+    op.t_copy.push_back({c0, c1});
+    CK(cudaEventRecord(c->ev_free[0][slot], c->d2h));
+    c->slot_used[0][slot] = true;
+  }
+  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_dtmp[0], c->d_dg);
+  CKL();
+  c->st.kernel_launches++;
+  CK(cudaEventRecord(c->ev_body_a[0], c->gather));
+  CK(cudaEventRecord(c->ev_body_b[0], c->d2h));
+  CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[0], 0));
+  CK(cudaStreamWaitEvent(c->meta, c->ev_body_b[0], 0));          // "offloaded" follows the finished transfer
+  k_unref<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[0], n, c->d_bt, c->d_used, c->d_ref);
+  CKL();
+  c->st.kernel_launches++;
+  if ((rc = emit(c, 0, n, EM_OFFLOAD))) return rc;
+  CK(cudaMemcpyAsync(c->h_res[0], c->d_res[0], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
+  CK(cudaEventRecord(op.done, c->meta));
+  c->ev_reserved += served.size();
+  op.active = true;
+  return RC_OK;
+}
+
+static int collect_times(rc_ctx* c, Op& op, float& ms_k, float& ms_c) {
+  for (auto& p : op.t_kernel) { float ms = 0; CK(cudaEventElapsedTime(&ms, p.first, p.second)); ms_k += ms; c->ev_pool.push_back(p.first); c->ev_pool.push_back(p.second); }
+  for (auto& p : op.t_copy) { float ms = 0; CK(cudaEventElapsedTime(&ms, p.first, p.second)); ms_c += ms; c->ev_pool.push_back(p.first); c->ev_pool.push_back(p.second); }
+  op.t_kernel.clear(); op.t_copy.clear();
+  return RC_OK;
+}
+
+static int wait_offload(rc_ctx* c) {
+  Op& op = c->ops[0];
+  if (!op.active) return RC_OK;
+  CK(cudaEventSynchronize(op.done));
+  op.active = false;
+  u64 served = 0;
+  for (u32 k = 0; k < op.n; ++k) {
+    Claim* cl = op.cl[k];
+    if (!cl) continue;
+    cl->chain = c->h_res[0][k].chain;
+    cl->state = RC_CS_OFFLOADED;
+    c->bt_alloc.release(cl->bt_off, cl->bt_len);
+    cl->bt_len = 0;
+    cl->busy = false;
+    op.status[k] = RC_ST_OK;
+    ++served;
+  }
+  c->ev_reserved -= served; c->ev_emitted += served;
+  c->st.claims_offloaded += served; c->st.bytes_d2h += op.copy_bytes;
+  c->st.gather_launches += op.launches; c->st.gather_blocks += op.blocks;
+  return collect_times(c, op, c->st.ms_gather, c->st.ms_d2h);
+}
+
+// ---- a5-a8 restore ---------------------------------------------------------------------------------------
+extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
+  GUARD();
+  Op& op = c->ops[1];
+  if (op.active) return RC_ERR_BUSY;
+  if (n == 0) return RC_OK;
+  if (!id || !st || n > c->desc_cap) return RC_ERR_INVALID;
+  Desc* hd = c->h_desc[1];
+  op.cl.assign(n, nullptr);
+  std::vector<u32> elig;
+  std::unordered_set<u64> seen;
+  u64 Te = 0;
+  auto rollback = [&]() { for (u32 k : elig) c->bt_alloc.release(hd[k].bt_off, hd[k].nb); };
+  for (u32 k = 0; k < n; ++k) {
+    memset(&hd[k], 0, sizeof(Desc));
+    hd[k].id = id[k];
+    auto it = c->claims.find(id[k]);
+    if (it == c->claims.end()) { st[k] = RC_ST_UNKNOWN_CLAIM; continue; }
+    Claim& cl = it->second;
+    // restore-after-use and double restore are not OFFLOADED any more
+    if (cl.busy || cl.state != RC_CS_OFFLOADED || !seen.insert(id[k]).second) { st[k] = RC_ST_BAD_STATE; continue; }
+    u64 o;
+    if (Te + cl.nb > c->cap_entries || !c->bt_alloc.alloc(cl.nb, o)) { rollback(); return RC_ERR_CAPACITY; }
+    hd[k].chain = cl.chain; hd[k].P = cl.P; hd[k].N = cl.N; hd[k].M = cl.M; hd[k].nb = cl.nb;
+    hd[k].bt_off = (u32)o; hd[k].bt_len = cl.nb; hd[k].dg_off = cl.dg_off; hd[k].flags = D_ELIG;
+    op.cl[k] = &cl;
+    elig.push_back(k);
+    Te += cl.nb;
+    st[k] = -1;
+  }
+  if (elig.empty()) return RC_OK;
+  if (!ev_room(c, 4ull * elig.size())) { rollback(); for (u32 k : elig) st[k] = RC_ST_BAD_STATE; return RC_ERR_CAPACITY; }
+  int rc;
+  if ((rc = upload_desc(c, 1, n))) return rc;
+  k_restore_plan<<<1, 1024, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_used, c->d_ref, c->NB, c->d_alloc,
+                                          c->d_counters);
+  CKL();
+  c->st.kernel_launches++;
+  CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
+  CK(cudaStreamSynchronize(c->meta));                    // the grant (which claims are served) is needed to plan the copies
+  std::vector<Seg> segs;
+  std::vector<std::pair<u64, u64>> flips;                // (work position, byte in block)
+  u64 T = 0;
+  u32 n_served = 0;
+  bool reupload = false;
+  for (u32 k : elig) {
+    Claim& cl = *op.cl[k];
+    if (!(c->h_res[1][k].flag & R_SERVED)) {
+      c->bt_alloc.release(hd[k].bt_off, hd[k].nb);
+      op.cl[k] = nullptr;
+      st[k] = RC_ST_NO_FREE_BLOCKS;
+      continue;
+    }
+    ++n_served;
+    cl.busy = true;
+    c->host_used -= (u64)cl.nb * c->blk;                 // granted back at once (count); extents at completion
+    // fault decision: the first armed entry naming exactly this claim, one-shot.  Entries naming any
+    // other id never fire for it (wrong-claim / unclaimed failures are not claim outcomes: P:L25)
+    rc_fault flt{0, 0, 0};
+    for (size_t f = 0; f < c->faults.size(); ++f)
+      if (c->faults[f].claim_id == id[k]) { flt = c->faults[f]; c->faults.erase(c->faults.begin() + f); break; }
+    if (flt.kind == RC_FAULT_XFER_ERROR) { hd[k].flags |= D_XFER; reupload = true; }
+    else {
+      if (flt.kind == RC_FAULT_BITFLIP) {
+        const u64 pos = flt.param % ((u64)cl.nb * c->blk);
+        flips.push_back({T + pos / c->blk, pos % c->blk});
+      }
+      u64 w = T;
+      for (auto& e : cl.host) { segs.push_back({w, e.second, e.first}); w += e.second; }
+    }
+    T += cl.nb;
+  }
+  if (n_served == 0) return RC_OK;
+  if (c->fault_flags & RC_FAULT_ALLOW_UNCLAIMED)          // a counter, never an outcome
+    for (size_t f = 0; f < c->faults.size();)
+      if (c->faults[f].claim_id == 0) { c->st.generic_failures++; c->faults.erase(c->faults.begin() + f); } else ++f;
+  op.n = n; op.status = st; op.blocks = T; op.copy_bytes = 0; op.launches = 0;
+  if (reupload && (rc = upload_desc(c, 1, n))) return rc;
+  k_worklist<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_bt, c->d_alloc, c->d_phys[1], 1);
+  CKL();
+  c->st.kernel_launches++;
+  CK(cudaEventRecord(c->ev_plan[1], c->meta));
+  CK(cudaStreamWaitEvent(c->scatter, c->ev_plan[1], 0));
+  std::sort(flips.begin(), flips.end());
+  size_t si = 0, fi = 0;
+  u64 flip_base = 0;
+  u32 ci = 0;
+  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks, ++ci) {
+    const u64 w1 = std::min(T, w0 + c->chunk_blocks);
+    const u32 slot = ci % c->R, m = (u32)(w1 - w0);
+    if (c->slot_used[1][slot]) CK(cudaStreamWaitEvent(c->h2d, c->ev_free[1][slot], 0));
+    cudaEvent_t c0 = get_event(c), c1 = get_event(c);
+    CK(cudaEventRecord(c0, c->h2d));
+    if ((rc = copy_chunk(c, 1, c->h2d, c->staging[1][slot], w0, w1, segs, si, op.copy_bytes))) return rc;
+    CK(cudaEventRecord(c1, c->h2d));
+    op.t_copy.push_back({c0, c1});
+    CK(cudaEventRecord(c->ev_ready[1][slot], c->h2d));
+    CK(cudaStreamWaitEvent(c->scatter, c->ev_ready[1][slot], 0));
+    u32 nf = 0;
+    while (fi < flips.size() && flips[fi].first < w1) {  // injected corruption of the staged copy (host bytes stay intact)
+      c->h_flip[flip_base + nf++] = (flips[fi].first - w0) * c->blk + flips[fi].second;
+      ++fi;
+    }
+    if (nf) {
+      CK(cudaMemcpyAsync(c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8, cudaMemcpyHostToDevice, c->scatter));
+      k_bitflip<<<(nf + 63) / 64, 64, 0, c->scatter>>>(c->staging[1][slot], c->d_flip + flip_base, nf);
+      CKL();
+      c->st.kernel_launches++;
+      flip_base += nf;
+    }
+    cudaEvent_t t0 = get_event(c), t1 = get_event(c);
+    CK(cudaEventRecord(t0, c->scatter));
+    launch_move<MV_SCATTER>(c, c->scatter, c->staging[1][slot], c->d_phys[1] + w0, c->part[1][slot], m);
+    CKL();
+    CK(cudaEventRecord(t1, c->scatter));
+    op.t_kernel.push_back({t0, t1});
+    op.launches++;
+    k_block_digest<<<warps_grid(m), 256, 0, c->scatter>>>(c->part[1][slot], c->d_phys[1] + w0, c->d_dtmp[1] + w0, m, c->G);
+    CKL();
+    c->st.kernel_launches++;
+    CK(cudaEventRecord(c->ev_free[1][slot], c->scatter));
+    c->slot_used[1][slot] = true;
+  }
+  CK(cudaEventRecord(c->ev_body_a[1], c->scatter));
+  CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[1], 0));
+  k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_dg, c->d_bt,
+                                               c->d_used, c->d_ref, c->fill, c->cfg.block_size);
+  CKL();
+  c->st.kernel_launches++;
+  if ((rc = emit(c, 1, n, EM_RESTORE))) return rc;
+  CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
+  CK(cudaEventRecord(op.done, c->meta));
+  c->ev_reserved += 4ull * n_served;
+  op.active = true;
+  return RC_OK;
+}
+
+static int wait_restore(rc_ctx* c) {
+  Op& op = c->ops[1];
+  if (!op.active) return RC_OK;
+  CK(cudaEventSynchronize(op.done));
+  op.active = false;
+  const Desc* hd = c->h_desc[1];
+  for (u32 k = 0; k < op.n; ++k) {
+    Claim* cl = op.cl[k];
+    if (!cl) continue;
+    const Res r = c->h_res[1][k];
+    for (auto& e : cl->host) c->host_alloc.release(e.first, e.second);
+    cl->host.clear();
+    cl->busy = false;
+    c->ev_reserved -= 4;
+    if (r.flag & R_OK) {
+      cl->state = RC_CS_RESIDENT_AGAIN; cl->bt_off = hd[k].bt_off; cl->bt_len = cl->nb;
+      c->ev_emitted += 2; c->st.claims_restored++;
+      op.status[k] = RC_ST_OK;
+    } else {
+      c->bt_alloc.release(hd[k].bt_off, cl->nb);
+      if (cl->dg_len) { c->dg_alloc.release(cl->dg_off, cl->dg_len); cl->dg_len = 0; }
+      cl->bt_len = 0;
+      cl->state = RC_CS_REFUSED;                             // terminal (fail-closed active outcome)
+      c->ev_emitted += 4; c->st.claims_refused++;
+      op.status[k] = RC_ST_RESTORE_FAILED;
+    }
+  }
+  c->st.bytes_h2d += op.copy_bytes;
+  c->st.scatter_launches += op.launches; c->st.scatter_blocks += op.blocks;
+  return collect_times(c, op, c->st.ms_scatter, c->st.ms_h2d);
+}
+
+extern "C" int rc_wait(rc_ctx* c, int which) {
+  GUARD();
+  if (which == 0) return wait_offload(c);
+  if (which == 1) return wait_restore(c);
+  return RC_ERR_INVALID;
+}
+extern "C" int rc_offload(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
+  const int rc = rc_offload_begin(c, n, id, st);
+  return rc ? rc : wait_offload(c);
+}
+extern "C" int rc_restore(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
+  const int rc = rc_restore_begin(c, n, id, st);
+  return rc ? rc : wait_restore(c);
+}
+
+// ---- outcomes, faults, release -----------------------------------------------------------------------------
+extern "C" int rc_outcomes(rc_ctx* c, rc_event* buf, uint64_t cap, uint64_t* n_out) {
+  GUARD();
+  if (!n_out || (cap && !buf)) return RC_ERR_INVALID;
+  const u64 m = std::min<u64>(cap, c->ev_emitted - c->ev_drained), E = c->cfg.max_events;
+  u64 done = 0;
+  while (done < m) {
+    const u64 at = (c->ev_drained + done) % E, l = std::min(m - done, E - at);
+    CK(cudaMemcpyAsync(buf + done, c->d_ring + at, l * sizeof(Event), cudaMemcpyDeviceToHost, c->util));
+    done += l;
+  }
+  CK(cudaStreamSynchronize(c->util));
+  c->ev_drained += m;
+  *n_out = m;
+  return RC_OK;
+}
+
+extern "C" int rc_set_faults(rc_ctx* c, uint32_t n, const rc_fault* f, uint32_t flags) {
+  GUARD();
+  if (n && !f) return RC_ERR_INVALID;
+  for (u32 i = 0; i < n; ++i) {
+    if (f[i].kind != RC_FAULT_XFER_ERROR && f[i].kind != RC_FAULT_BITFLIP) return RC_ERR_INVALID;
+    if (f[i].claim_id == 0 && !(flags & RC_FAULT_ALLOW_UNCLAIMED)) return RC_ERR_INVALID;   // separate flag
+  }
+  c->faults.assign(f, f + n);
+  c->fault_flags = flags;
+  return RC_OK;
+}
+
+extern "C" int rc_release(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
+  GUARD();
+  if (n == 0) return RC_OK;
+  if (!id || !st || n > c->desc_cap) return RC_ERR_INVALID;
+  Desc* hd = c->h_desc[2];
+  bool any = false;
+  for (u32 k = 0; k < n; ++k) {
+    memset(&hd[k], 0, sizeof(Desc));
+    auto it = c->claims.find(id[k]);
+    if (it == c->claims.end()) { st[k] = RC_ST_UNKNOWN_CLAIM; continue; }
+    Claim& cl = it->second;
+    if (cl.busy) { st[k] = RC_ST_BAD_STATE; continue; }
+    if (cl.bt_len) {
+      hd[k].bt_off = cl.bt_off; hd[k].bt_len = cl.bt_len; hd[k].flags = D_ELIG; any = true;
+      c->bt_alloc.release(cl.bt_off, cl.bt_len);
+    }
+    if (cl.dg_len) c->dg_alloc.release(cl.dg_off, cl.dg_len);
+    for (auto& e : cl.host) c->host_alloc.release(e.first, e.second);
+    if (!cl.host.empty()) c->host_used -= (u64)cl.nb * c->blk;
+    c->claims.erase(it);
+    st[k] = RC_ST_OK;
+  }
+  if (any) {
+    int rc;
+    if ((rc = upload_desc(c, 2, n))) return rc;
+    k_unref<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[2], n, c->d_bt, c->d_used, c->d_ref);
+    CKL();
+    c->st.kernel_launches++;
+    CK(cudaStreamSynchronize(c->meta));
+  }
+  return RC_OK;
+}
+
+// ---- introspection -------------------------------------------------------------------------------------------
+extern "C" int rc_claim_info(rc_ctx* c, uint64_t id, rc_claim_info_t* o) {
+  GUARD();
+  auto it = c->claims.find(id);
+  if (it == c->claims.end() || !o) return RC_ERR_INVALID;
+  const Claim& cl = it->second;
+  o->claim_id = id; o->chain = cl.chain; o->host_bytes = cl.host.empty() ? 0 : (u64)cl.nb * c->blk;
+  o->state = cl.state; o->P = cl.P; o->N = cl.N; o->M = cl.M; o->nb = cl.nb; o->n_table = cl.bt_len;
+  return RC_OK;
+}
+extern "C" int rc_claim_blocks(rc_ctx* c, uint64_t id, uint32_t* ids, uint32_t cap, uint32_t* n) {
+  GUARD();
+  auto it = c->claims.find(id);
+  if (it == c->claims.end() || !n) return RC_ERR_INVALID;
+  const Claim& cl = it->second;
+  *n = cl.bt_len;
+  const u32 m = std::min(cap, cl.bt_len);
+  if (m && ids) {
+    CK(cudaMemcpyAsync(ids, c->d_bt + cl.bt_off, (u64)m * 4, cudaMemcpyDeviceToHost, c->util));
+    CK(cudaStreamSynchronize(c->util));
+  }
+  return RC_OK;
+}
+extern "C" int rc_claim_digests(rc_ctx* c, uint64_t id, uint64_t* d, uint32_t cap, uint32_t* n) {
+  GUARD();
+  auto it = c->claims.find(id);
+  if (it == c->claims.end() || !n) return RC_ERR_INVALID;
+  const Claim& cl = it->second;
+  *n = cl.dg_len;
+  const u32 m = std::min(cap, cl.dg_len);
+  if (m && d) {
+    CK(cudaMemcpyAsync(d, c->d_dg + cl.dg_off, (u64)m * 8, cudaMemcpyDeviceToHost, c->util));
+    CK(cudaStreamSynchronize(c->util));
+  }
+  return RC_OK;
+}
+extern "C" int rc_host_read(rc_ctx* c, uint64_t id, void* dst, uint64_t cap, uint64_t* bytes) {
+  GUARD();
+  auto it = c->claims.find(id);
+  if (it == c->claims.end() || !bytes) return RC_ERR_INVALID;
+  const Claim& cl = it->second;
+  *bytes = cl.host.empty() ? 0 : (u64)cl.nb * c->blk;
+  if (dst && cap >= *bytes && *bytes) {
+    u8* o = (u8*)dst;
+    for (auto& e : cl.host) { memcpy(o, c->h_store + e.first * c->blk, e.second * c->blk); o += e.second * c->blk; }
+  }
+  return RC_OK;
+}
+extern "C" int rc_pool_state(rc_ctx* c, uint8_t* used, uint32_t* ref) {
+  GUARD();
+  if (used) CK(cudaMemcpyAsync(used, c->d_used, c->NB, cudaMemcpyDeviceToHost, c->util));
+  if (ref) CK(cudaMemcpyAsync(ref, c->d_ref, (u64)c->NB * 4, cudaMemcpyDeviceToHost, c->util));
+  CK(cudaStreamSynchronize(c->util));
+  return RC_OK;
+}
+extern "C" int rc_stats_get(rc_ctx* c, rc_stats* o) {
+  GUARD();
+  if (!o) return RC_ERR_INVALID;
+  std::vector<u8> used(c->NB);
+  CK(cudaMemcpyAsync(used.data(), c->d_used, c->NB, cudaMemcpyDeviceToHost, c->util));
+  CK(cudaStreamSynchronize(c->util));
+  u64 fr = 0;
+  for (u8 u : used) fr += !u;
+  c->st.host_used_bytes = c->host_used; c->st.free_blocks = fr; c->st.events_emitted = c->ev_emitted;
+  *o = c->st;
+  return RC_OK;
+}
+extern "C" int rc_stats_reset(rc_ctx* c) {
+  GUARD();
+  const u64 g = c->st.generic_failures;
+  memset(&c->st, 0, sizeof(c->st));
+  c->st.generic_failures = g;
+  return RC_OK;
+}
+
+// ---- measurement helpers -----------------------------------------------------------------------------------------
+extern "C" int rc_measure_link(rc_ctx* c, uint64_t bytes, int direction, int reps, double* gbs) {
+  GUARD();
+  if (!gbs || direction < 0 || direction > 2 || reps < 1) return RC_ERR_INVALID;
+  if (c->ops[0].active || c->ops[1].active) return RC_ERR_BUSY;
+  const u64 hs = c->host_blocks * c->blk, cs = c->chunk_blocks * c->blk;
+  const u64 hmax = direction == 2 ? hs / 2 : hs;
+  bytes = std::min(bytes, std::min(hmax, cs));
+  if (bytes == 0) return RC_ERR_INVALID;
+  cudaEvent_t a0 = get_event(c), a1 = get_event(c), b0 = get_event(c), b1 = get_event(c);
+  double best = 0;
+  for (int r = 0; r < reps; ++r) {
+    CK(cudaDeviceSynchronize());
+    float ma = 0, mb = 0;
+    if (direction == 0 || direction == 2) {
+      CK(cudaEventRecord(a0, c->d2h));
+      CK(cudaMemcpyAsync(c->h_store, c->staging[0][0], bytes, cudaMemcpyDeviceToHost, c->d2h));
+      CK(cudaEventRecord(a1, c->d2h));
+    }
+    if (direction == 1 || direction == 2) {
+      CK(cudaEventRecord(b0, c->h2d));
+      CK(cudaMemcpyAsync(c->staging[1][0], c->h_store + (direction == 2 ? hs / 2 : 0), bytes, cudaMemcpyHostToDevice, c->h2d));
+      CK(cudaEventRecord(b1, c->h2d));
+    }
+    CK(cudaDeviceSynchronize());
+    if (direction != 1) CK(cudaEventElapsedTime(&ma, a0, a1));
+    if (direction != 0) CK(cudaEventElapsedTime(&mb, b0, b1));
+    const double ms = std::max(ma, mb), g = (direction == 2 ? 2.0 : 1.0) * bytes / (ms * 1e6);
+    best = std::max(best, g);
+  }
+  c->ev_pool.insert(c->ev_pool.end(), {a0, a1, b0, b1});
+  *gbs = best;
+  return RC_OK;
+}
+
+extern "C" int rc_digest_blocks(rc_ctx* c, const void* src, uint32_t n_blocks, uint64_t* digests, float* ms_out) {
+  GUARD();
+  if (!src || ((uintptr_t)src & 15) || n_blocks > c->cap_entries) return RC_ERR_INVALID;
+  if (c->ops[0].active) return RC_ERR_BUSY;
+  cudaEvent_t t0 = get_event(c), t1 = get_event(c);
+  float total = 0;
+  for (u64 w0 = 0; w0 < n_blocks; w0 += c->chunk_blocks) {
+    const u32 m = (u32)std::min<u64>(c->chunk_blocks, n_blocks - w0);
+    CK(cudaEventRecord(t0, c->gather));
+    launch_move<MV_DIGEST>(c, c->gather, (u8*)src + w0 * c->blk, nullptr, c->part[0][0], m);
+    CKL();
+    CK(cudaEventRecord(t1, c->gather));
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][0], nullptr, c->d_dtmp[0] + w0, m, c->G);
+    CKL();
+    CK(cudaStreamSynchronize(c->gather));
+    float ms = 0;
+    CK(cudaEventElapsedTime(&ms, t0, t1));
+    total += ms;
+  }
+  if (digests && n_blocks) {
+    CK(cudaMemcpyAsync(digests, c->d_dtmp[0], (u64)n_blocks * 8, cudaMemcpyDeviceToHost, c->gather));
+    CK(cudaStreamSynchronize(c->gather));
+  }
+  c->ev_pool.push_back(t0); c->ev_pool.push_back(t1);
+  if (ms_out) *ms_out = total;
+  return RC_OK;
+}
+
+extern "C" const char* rc_strerror(int err) {
+  switch (err) {
+    case RC_OK: return "ok";
+    case RC_ERR_INVALID: return "invalid argument";
+    case RC_ERR_CUDA: return "CUDA error (context poisoned) or no CUDA device";
+    case RC_ERR_NOMEM: return "out of memory";
+    case RC_ERR_CAPACITY: return "capacity exceeded (claims, table entries, events or batch size)";
+    case RC_ERR_BUSY: return "an operation of this kind is still in flight";
+    default: return "unknown error";
+  }
+}
+extern "C" const char* rc_last_cuda_error(rc_ctx* c) { return c ? c->cuda_err.c_str() : ""; }

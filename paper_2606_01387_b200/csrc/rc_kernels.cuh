@@ -1,0 +1,556 @@
+// rc_kernels.cuh -- device code of librc (sm_100a only).
+//
+// Kernels of the claim-scoped KV offload / restore path:
+//   k_pred          K1  leading-prefix-at-least-N from fill[] (warp ballot + ffs)
+//   k_offsets       K1  exclusive scan of per-claim block counts (block scan)
+//   k_worklist      K1  compacted physical-block list (warp per claim)
+//   k_move_hash     K2/K4 page gather / scatter with the lane-fold checksum fused in   BJ (b),(c),(d)
+//   k_move_hash_tma K2/K4 same, staged through cp.async.bulk (TMA) + mbarrier ring
+//   k_block_digest  K2/K4 tail: page terms -> per-block digest
+//   k_chain         K3  per-claim affine warp scan of block digests                     BJ (d)
+//   k_restore_plan  K5  free count, prefix grant, lowest-free-id allocation             DESIGN R6/R7
+//   k_verify        K4/K3 digest compare, chain compare, verdict, fill / free
+//   k_unref         K5  reference drop at offload
+//   k_accept        a0  table validation + reference take
+//   k_emit          K6  ordered claim-scoped event records (scan-assigned offsets)
+// The checksum constants are restated here from DESIGN.md "Checksum"; nothing is
+// shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+typedef uint64_t u64;
+typedef uint32_t u32;
+typedef uint8_t u8;
+
+namespace rck {
+
+constexpr u64 C1 = 0x9E3779B97F4A7C15ull;
+constexpr u64 C2 = 0x6A09E667F3BCC909ull;
+constexpr u64 CA = 0xBB67AE8584CAA73Bull;
+constexpr u64 C3 = 0x3C6EF372FE94F82Bull;
+constexpr u32 SKIP = 0xFFFFFFFFu;       // work item whose transfer was suppressed (XFER_ERROR)
+constexpr int LANES = 256;              // checksum lanes per page == threads per CTA of k_move_hash
+constexpr int WPC = LANES / 32;         // warps per CTA
+
+// batch descriptor, one per claim of a call (host fills, device reads)
+struct Desc {
+  u64 id, chain;
+  u32 P, N, M, nb;
+  u32 bt_off, bt_len;     // table extent in the arena (bt_len entries)
+  u32 dg_off;             // digest extent in the digest arena (nb entries)
+  u32 flags;              // D_* below
+  u32 src_off;            // accept: offset of the candidate table in the upload buffer
+  u32 pad;
+};
+enum { D_ELIG = 1, D_XFER = 2 };
+
+// per-claim result of a call (device fills, host reads)
+struct Res {
+  u32 flag;               // R_* below
+  u32 val;                // M (materialize) or first bad block (restore)
+  u64 chain;
+};
+enum { R_OK = 1, R_SERVED = 2 };
+
+struct Event { u64 seq, claim_id; u32 code, aux; u64 arg; };
+enum { EV_ACCEPTED = 1, EV_MATERIALIZED = 2, EV_OFFLOADED = 3, EV_RESTORE_REQUIRED = 4, EV_LOAD_FAILED = 5,
+       EV_RESTORED = 6, EV_RESTORATION_FAILED = 7, EV_ACTIVE_REQUEST_REFUSED = 8 };
+enum { EM_ACCEPT = 0, EM_MATERIALIZE = 1, EM_OFFLOAD = 2, EM_RESTORE = 3 };
+
+__device__ __forceinline__ u64 mixL(u64 x) { u64 y = x ^ (x >> 32); y *= C2; return y ^ (y >> 29); }
+__device__ __forceinline__ u64 mixF(u64 x) { u64 y = mixL(x); y *= C1; return y ^ (y >> 32); }
+
+__device__ __forceinline__ u64 shfl_xor64(u64 v, int m) { return __shfl_xor_sync(0xFFFFFFFFu, v, m); }
+__device__ __forceinline__ u64 shfl_up64(u64 v, int d) { return __shfl_up_sync(0xFFFFFFFFu, v, d); }
+__device__ __forceinline__ u64 warp_sum64(u64 v) {
+#pragma unroll
+  for (int m = 16; m > 0; m >>= 1) v += shfl_xor64(v, m);
+  return v;
+}
+__device__ __forceinline__ u32 warp_sum32(u32 v) {
+#pragma unroll
+  for (int m = 16; m > 0; m >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, m);
+  return v;
+}
+
+// streaming 16-byte accesses: the data is touched once, keep it out of L1 and first out of L2
+__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
+               :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ u64 fold(u64 h, const uint4& v) {
+  h = (h ^ ((u64)v.x | ((u64)v.y << 32))) * C2;
+  h = (h ^ ((u64)v.z | ((u64)v.w << 32))) * C2;
+  return h;
+}
+
+// ---------------------------------------------------------------------------------------------
+// K2 / K4: page mover with fused checksum.  One CTA (256 threads = the 256 checksum lanes) per
+// page at a time, grid-stride over the n_items*G pages of a staging chunk.  Thread t moves
+// vectors t, t+256, ... of the page (each warp access = 512 contiguous bytes) and folds them in
+// that order; each warp writes the sum of its 32 lane terms to part[page*8 + warp] -- no block
+// barrier and no atomics in the streaming loop.  MODE 0 gather (pool -> staging), 1 scatter
+// (staging -> pool), 2 digest only (read staging).
+// ---------------------------------------------------------------------------------------------
+enum { MV_GATHER = 0, MV_SCATTER = 1, MV_DIGEST = 2 };
+
+template <int MODE, int UNR>
+__global__ void __launch_bounds__(LANES)
+k_move_hash(uint4* __restrict__ pool, uint4* __restrict__ staging, const u32* __restrict__ phys,
+            u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 vpp) {
+  const u32 t = threadIdx.x;
+  const u32 n_pages = n_items * G;
+  const u32 vpt = vpp / LANES;
+  for (u32 u = blockIdx.x; u < n_pages; u += gridDim.x) {
+    const u32 w = u / G, g = u - w * G;
+    u32 b = 0;
+    if (MODE != MV_DIGEST) { b = __ldg(phys + w); if (b == SKIP) continue; }
+    uint4* pp = pool + ((u64)g * NB + b) * vpp + t;
+    uint4* sp = staging + (u64)u * vpp + t;
+    const uint4* src = (MODE == MV_GATHER) ? pp : sp;
+    uint4* dst = (MODE == MV_GATHER) ? sp : pp;
+    u64 h = (u64)(t + 1) * C1;
+    for (u32 j0 = 0; j0 < vpt; j0 += UNR) {
+      uint4 v[UNR];
+#pragma unroll
+      for (int jj = 0; jj < UNR; ++jj)
+        if (j0 + jj < vpt) v[jj] = ld_stream(src + (u64)(j0 + jj) * LANES);
+#pragma unroll
+      for (int jj = 0; jj < UNR; ++jj)
+        if (j0 + jj < vpt) {
+          if (MODE != MV_DIGEST) st_stream(dst + (u64)(j0 + jj) * LANES, v[jj]);
+          h = fold(h, v[jj]);
+        }
+    }
+    const u64 s = warp_sum64(mixL(h));
+    if ((t & 31) == 0) part[(u64)u * WPC + (t >> 5)] = s;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K2 / K4, TMA variant: the page is staged through shared memory with 1-D bulk copies
+// (cp.async.bulk global->shared completing on an mbarrier; shared->global bulk store), so the
+// LSU only sees conflict-free 16-byte shared loads for the checksum.  One elected thread issues
+// the copies; a ring of STAGES tiles of TILE bytes keeps STAGES-1 loads in flight per CTA.
+// Tiles are consumed in page order, so thread t still folds vectors t, t+256, ... in increasing
+// order.  Persistent grid: CTA c handles pages c, c+grid, ...
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(u64* bar, u32 count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, u32 bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u64* bar, u32 parity) {
+  asm volatile(
+      "{\n .reg .pred p;\n WAIT_%=:\n"
+      " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      " @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" :: "r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, u32 bytes, u64* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, u32 bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               :: "l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+template <int MODE, int STAGES, int TILE>
+__global__ void __launch_bounds__(LANES)
+k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __restrict__ phys,
+                u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 page_bytes) {
+  extern __shared__ __align__(128) u8 smem[];
+  __shared__ __align__(8) u64 full[STAGES];
+  const u32 t = threadIdx.x;
+  const u32 n_pages = n_items * G;
+  const u32 tpp = page_bytes / TILE;                     // tiles per page (page % TILE == 0)
+  constexpr u32 VT = TILE / (16 * LANES);                // vectors per thread per tile
+  if (t == 0) {
+    for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  // this CTA's tile sequence: for page u = blockIdx.x + k*grid, tiles 0..tpp-1
+  const u32 my_pages = (n_pages > blockIdx.x) ? (n_pages - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  const u64 n_tiles = (u64)my_pages * tpp;
+  auto addr = [&](u64 q, u8*& gsrc, u8*& gdst, bool& skip) {
+    const u32 k = (u32)(q / tpp), tile = (u32)(q - (u64)k * tpp);
+    const u32 u = blockIdx.x + k * gridDim.x;
+    const u32 w = u / G, g = u - w * G;
+    u32 b = 0;
+    skip = false;
+    if (MODE != MV_DIGEST) { b = __ldg(phys + w); skip = (b == SKIP); if (skip) b = 0; }
+    u8* pp = pool + ((u64)g * NB + b) * page_bytes + (u64)tile * TILE;
+    u8* sp = staging + (u64)u * page_bytes + (u64)tile * TILE;
+    gsrc = (MODE == MV_GATHER) ? pp : sp;
+    gdst = (MODE == MV_GATHER) ? sp : pp;
+  };
+  if (t == 0) {                                            // prologue: fill the ring
+    for (u64 q = 0; q < n_tiles && q < STAGES; ++q) {
+      u8 *gs, *gd; bool skip; addr(q, gs, gd, skip);
+      mbar_expect_tx(&full[q], TILE);
+      bulk_g2s(smem + (u32)q * TILE, gs, TILE, &full[q]);
+    }
+  }
+  u64 h = 0;
+  for (u64 q = 0; q < n_tiles; ++q) {
+    const u32 s = (u32)(q % STAGES), ph = (u32)((q / STAGES) & 1);
+    const u32 tile = (u32)(q % tpp);
+    if (tile == 0) h = (u64)(t + 1) * C1;
+    mbar_wait(&full[s], ph);
+    u8 *gs, *gd; bool skip; addr(q, gs, gd, skip);
+    if (MODE != MV_DIGEST && t == 0 && !skip) { bulk_s2g(gd, smem + s * TILE, TILE); bulk_commit(); }
+    const uint4* sv = reinterpret_cast<const uint4*>(smem + s * TILE) + t;
+#pragma unroll
+    for (u32 j = 0; j < VT; ++j) h = fold(h, sv[j * LANES]);
+    if (tile == tpp - 1 && !skip) {
+      const u64 sum = warp_sum64(mixL(h));
+      const u32 k = (u32)(q / tpp), u = blockIdx.x + k * gridDim.x;
+      if ((t & 31) == 0) part[(u64)u * WPC + (t >> 5)] = sum;
+    }
+    __syncthreads();                                       // every thread is done reading stage s
+    if (t == 0 && q + STAGES < n_tiles) {
+      if (MODE != MV_DIGEST) bulk_wait_read<0>();          // the store that reads stage s has drained it
+      u8 *ngs, *ngd; bool nskip; addr(q + STAGES, ngs, ngd, nskip);
+      mbar_expect_tx(&full[s], TILE);
+      bulk_g2s(smem + s * TILE, ngs, TILE, &full[s]);
+    }
+  }
+  if (MODE != MV_DIGEST && t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+// Per-block digest from the warp partial sums: page_digest(g) = sum of its 8 partials,
+// d = mixF( sum_g mixL(page_digest(g) ^ (g+1)*C3) ).  One warp per work item.
+__global__ void k_block_digest(const u64* __restrict__ part, const u32* __restrict__ phys, u64* __restrict__ d_out,
+                               u32 n_items, u32 G) {
+  const u32 w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (w >= n_items) return;
+  if (phys && __ldg(phys + w) == SKIP) { if (lane == 0) d_out[w] = 0; return; }
+  u64 s = 0;
+  for (u32 g = lane; g < G; g += 32) {
+    const u64* p = part + ((u64)w * G + g) * WPC;
+    u64 pd = 0;
+#pragma unroll
+    for (int i = 0; i < WPC; ++i) pd += p[i];
+    s += mixL(pd ^ ((u64)(g + 1) * C3));
+  }
+  s = warp_sum64(s);
+  if (lane == 0) d_out[w] = mixF(s);
+}
+
+// ---------------------------------------------------------------------------------------------
+// K1: predicate.  One warp per claim; lane l looks at table entries l, l+32, ...  Block i holds
+// tokens [i*BS, min(P,(i+1)*BS)); it is complete iff fill[bt[i]] >= that count.  The leading run
+// ends inside the first incomplete block: M = i0*BS + fill[bt[i0]], or P when all are complete.
+// ---------------------------------------------------------------------------------------------
+__global__ void k_pred(const Desc* __restrict__ desc, Res* __restrict__ res, u32 n, const u32* __restrict__ bt,
+                       const u8* __restrict__ fill, u32 BS) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= n) return;
+  const Desc d = desc[k];
+  if (!(d.flags & D_ELIG)) { if (lane == 0) res[k] = Res{0, 0, 0}; return; }
+  u32 M = d.P;
+  for (u32 base = 0; base < d.bt_len; base += 32) {
+    const u32 i = base + lane;
+    u32 f = 0; bool inc = false;
+    if (i < d.bt_len) {
+      f = fill[bt[d.bt_off + i]];
+      const u32 rem = d.P - i * BS, cap = rem < BS ? rem : BS;
+      inc = f < cap;
+    }
+    const u32 mask = __ballot_sync(0xFFFFFFFFu, inc);
+    if (mask) {
+      const int j = __ffs(mask) - 1;
+      M = (base + j) * BS + __shfl_sync(0xFFFFFFFFu, f, j);
+      break;
+    }
+  }
+  if (lane == 0) res[k] = Res{M >= d.N ? (u32)R_OK : 0u, M, 0};
+}
+
+// block-wide inclusive scan of one u32 per thread (blockDim.x <= 1024)
+__device__ __forceinline__ u32 block_scan_incl(u32 v, u32* warp_tot /*[32]*/, u32& total) {
+  const u32 lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, v, d); if (lane >= (u32)d) v += o; }
+  __syncthreads();
+  if (lane == 31) warp_tot[wid] = v;
+  __syncthreads();
+  if (wid == 0) {
+    u32 x = lane < nw ? warp_tot[lane] : 0;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, x, d); if (lane >= (u32)d) x += o; }
+    warp_tot[lane] = x;
+  }
+  __syncthreads();
+  total = warp_tot[nw - 1];
+  return v + (wid ? warp_tot[wid - 1] : 0);
+}
+
+// K1: exclusive scan of nb over the eligible claims of a batch -> off[0..n].  One CTA.
+__global__ void k_offsets(const Desc* __restrict__ desc, u32 n, u32* __restrict__ off) {
+  __shared__ u32 wt[32];
+  u32 carry = 0;
+  for (u32 base = 0; base < n; base += blockDim.x) {
+    const u32 k = base + threadIdx.x;
+    const u32 c = (k < n && (desc[k].flags & D_ELIG)) ? desc[k].nb : 0;
+    u32 tot;
+    const u32 inc = block_scan_incl(c, wt, tot);
+    if (k < n) off[k] = carry + inc - c;
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) off[n] = carry;
+}
+
+// K1: compaction.  Offload: phys[off_k+i] = bt[bt_off_k+i].  Restore: the allocation list is the
+// work list; write it into the claim's new table and mark suppressed transfers.
+__global__ void k_worklist(const Desc* __restrict__ desc, const Res* __restrict__ res, u32 n,
+                           const u32* __restrict__ off, u32* __restrict__ bt, const u32* __restrict__ alloc,
+                           u32* __restrict__ phys, int restore) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= n) return;
+  const Desc d = desc[k];
+  if (!restore) {
+    if (!(d.flags & D_ELIG)) return;
+    for (u32 i = lane; i < d.nb; i += 32) phys[off[k] + i] = bt[d.bt_off + i];
+  } else {
+    if (!(res[k].flag & R_SERVED)) return;
+    for (u32 i = lane; i < d.nb; i += 32) {
+      const u32 b = alloc[off[k] + i];
+      bt[d.bt_off + i] = b;
+      phys[off[k] + i] = (d.flags & D_XFER) ? SKIP : b;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K3: chain.  H = seed(C); H = H*A + d_i.  The step is the affine map x -> x*A + d_i; maps
+// compose associatively as (a1,b1)*(a2,b2) = (a1*a2, b1*a2 + b2), so an inclusive warp scan of 32
+// blocks gives the tile's map and H advances one tile per iteration.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ u64 chain_tile(u64 h, u64 d, bool valid) {
+  const u32 lane = threadIdx.x & 31;
+  u64 a = valid ? CA : 1ull, b = valid ? d : 0ull;
+#pragma unroll
+  for (int s = 1; s < 32; s <<= 1) {
+    const u64 pa = shfl_up64(a, s), pb = shfl_up64(b, s);
+    if (lane >= (u32)s) { b = pb * a + b; a = pa * a; }
+  }
+  a = __shfl_sync(0xFFFFFFFFu, a, 31);
+  b = __shfl_sync(0xFFFFFFFFu, b, 31);
+  return h * a + b;
+}
+
+__global__ void k_chain(const Desc* __restrict__ desc, Res* __restrict__ res, u32 n, const u32* __restrict__ off,
+                        const u64* __restrict__ d_tmp, u64* __restrict__ dg) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= n) return;
+  const Desc d = desc[k];
+  if (!(d.flags & D_ELIG)) { if (lane == 0) res[k] = Res{0, 0, 0}; return; }
+  u64 h = mixF(d.id ^ C3);
+  for (u32 base = 0; base < d.nb; base += 32) {
+    const u32 i = base + lane;
+    const bool valid = i < d.nb;
+    const u64 x = valid ? d_tmp[off[k] + i] : 0;
+    if (valid) dg[d.dg_off + i] = x;
+    h = chain_tile(h, x, valid);
+  }
+  if (lane == 0) res[k] = Res{R_OK | R_SERVED, d.nb, h};
+}
+
+// ---------------------------------------------------------------------------------------------
+// K5: restore plan.  One CTA.  (1) free count at entry; (2) inclusive scan of nb over eligible
+// claims in batch order: claim k is served iff the running sum <= free count (nb >= 1, so the
+// served set is a prefix of the eligible claims); (3) the r-th free block in ascending id order,
+// r < total, goes to alloc[r].  Work-list offsets off[] are the same scan.
+// ---------------------------------------------------------------------------------------------
+__global__ void k_restore_plan(const Desc* __restrict__ desc, Res* __restrict__ res, u32 n, u32* __restrict__ off,
+                               u8* __restrict__ used, u32* __restrict__ ref, u32 NB, u32* __restrict__ alloc,
+                               u32* __restrict__ counters /*[2]: nfree, total*/) {
+  __shared__ u32 wt[32];
+  __shared__ u32 s_nfree, s_total;
+  u32 cnt = 0;
+  for (u32 b = threadIdx.x; b < NB; b += blockDim.x) cnt += used[b] == 0;
+  { u32 tot; block_scan_incl(cnt, wt, tot); if (threadIdx.x == 0) { s_nfree = tot; s_total = 0; } }
+  __syncthreads();
+  const u32 nfree = s_nfree;
+  u32 carry = 0;
+  for (u32 base = 0; base < n; base += blockDim.x) {
+    const u32 k = base + threadIdx.x;
+    const bool el = k < n && (desc[k].flags & D_ELIG);
+    const u32 c = el ? desc[k].nb : 0;
+    u32 tot;
+    const u32 inc = carry + block_scan_incl(c, wt, tot);
+    if (k < n) {
+      const bool served = el && inc <= nfree;
+      res[k] = Res{served ? (u32)R_SERVED : 0u, 0, 0};
+      off[k] = served ? inc - c : 0xFFFFFFFFu;
+      if (served) atomicMax(&s_total, inc);
+    }
+    carry += tot;
+    __syncthreads();
+  }
+  __syncthreads();
+  const u32 total = s_total;
+  if (threadIdx.x == 0) { off[n] = total; counters[0] = nfree; counters[1] = total; }
+  for (u32 k = threadIdx.x; k < n; k += blockDim.x) if (off[k] == 0xFFFFFFFFu) off[k] = total;
+  carry = 0;
+  for (u32 base = 0; base < NB && carry < total; base += blockDim.x) {
+    const u32 b = base + threadIdx.x;
+    const u32 f = (b < NB && used[b] == 0) ? 1u : 0u;
+    u32 tot;
+    const u32 r = carry + block_scan_incl(f, wt, tot) - f;
+    if (f && r < total) { alloc[r] = b; used[b] = 1; ref[b] = 1; }
+    carry += tot;
+    __syncthreads();
+  }
+}
+
+// K4 tail: verdict per served claim.  bad = first block whose recomputed digest differs; ok iff the
+// transfer was not suppressed, no block differs and the recomputed chain equals the recorded one.
+// ok: fill of the new blocks := leading tokens they hold.  not ok: the new blocks are freed.
+__global__ void k_verify(const Desc* __restrict__ desc, Res* __restrict__ res, u32 n, const u32* __restrict__ off,
+                         const u64* __restrict__ d_tmp, const u64* __restrict__ dg, const u32* __restrict__ bt,
+                         u8* __restrict__ used, u32* __restrict__ ref, u8* __restrict__ fill, u32 BS) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= n) return;
+  if (!(res[k].flag & R_SERVED)) return;
+  const Desc d = desc[k];
+  u32 bad = 0xFFFFFFFFu;
+  bool ok = !(d.flags & D_XFER);
+  if (ok) {
+    u64 h = mixF(d.id ^ C3);
+    for (u32 base = 0; base < d.nb; base += 32) {
+      const u32 i = base + lane;
+      const bool valid = i < d.nb;
+      const u64 x = valid ? d_tmp[off[k] + i] : 0;
+      const u32 mm = __ballot_sync(0xFFFFFFFFu, valid && x != dg[d.dg_off + i]);
+      if (mm && bad == 0xFFFFFFFFu) bad = base + __ffs(mm) - 1;
+      h = chain_tile(h, x, valid);
+    }
+    ok = bad == 0xFFFFFFFFu && h == d.chain;
+  }
+  for (u32 i = lane; i < d.nb; i += 32) {
+    const u32 b = bt[d.bt_off + i];
+    if (ok) { const u32 rem = d.M - i * BS; fill[b] = (u8)(rem < BS ? rem : BS); }
+    else { used[b] = 0; ref[b] = 0; fill[b] = 0; }
+  }
+  if (lane == 0) res[k] = Res{R_SERVED | (ok ? (u32)R_OK : 0u), bad, d.chain};
+}
+
+// K5: drop the claim's references to all its table blocks; a block whose count reaches 0 is free.
+__global__ void k_unref(const Desc* __restrict__ desc, u32 n, const u32* __restrict__ bt, u8* __restrict__ used,
+                        u32* __restrict__ ref) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= n) return;
+  const Desc d = desc[k];
+  if (!(d.flags & D_ELIG)) return;
+  for (u32 i = lane; i < d.bt_len; i += 32) {
+    const u32 b = bt[d.bt_off + i];
+    const u32 old = atomicSub(&ref[b], 1u);
+    if (old == 1u) used[b] = 0;
+  }
+}
+
+__global__ void k_mark(const u32* __restrict__ ids, u32 n, u8* __restrict__ used, const u32* __restrict__ ref, int val) {
+  const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const u32 b = ids[i];
+  if (val) used[b] = 1; else if (ref[b] == 0) used[b] = 0;
+}
+
+// a0: table validation.  One CTA per candidate at a time; `bm` is this CTA's private NB-bit map
+// (all zero between candidates).  Valid iff every id is in range, used, and distinct.
+__global__ void k_accept(const Desc* __restrict__ desc, Res* __restrict__ res, u32 n, const u32* __restrict__ up,
+                         u32* __restrict__ bt, const u8* __restrict__ used, u32* __restrict__ ref, u32 NB,
+                         u32* __restrict__ bitmaps) {
+  u32* bm = bitmaps + (size_t)blockIdx.x * ((NB + 31) / 32);
+  for (u32 k = blockIdx.x; k < n; k += gridDim.x) {
+    const Desc d = desc[k];
+    if (!(d.flags & D_ELIG)) { if (threadIdx.x == 0) res[k] = Res{0, 0, 0}; continue; }
+    int bad = 0;
+    for (u32 i = threadIdx.x; i < d.bt_len; i += blockDim.x) {
+      const u32 b = up[d.src_off + i];
+      if (b >= NB || !used[b]) { bad = 1; continue; }
+      const u32 bit = 1u << (b & 31);
+      if (atomicOr(&bm[b >> 5], bit) & bit) bad = 1;
+    }
+    bad = __syncthreads_or(bad);
+    for (u32 i = threadIdx.x; i < d.bt_len; i += blockDim.x) {
+      const u32 b = up[d.src_off + i];
+      if (b < NB) bm[b >> 5] = 0;
+      if (!bad) { bt[d.bt_off + i] = b; atomicAdd(&ref[b], 1u); }
+    }
+    if (threadIdx.x == 0) res[k] = Res{bad ? 0u : (u32)R_OK, 0, 0};
+    __syncthreads();
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K6: outcome emission.  One CTA.  Per claim of the batch, in batch order, the number of records
+// follows from the call and the claim's result; an exclusive scan assigns record offsets, so all
+// records of claim k precede those of claim k+1 and seq is gap-free (P:L27 order per claim).
+// ---------------------------------------------------------------------------------------------
+__global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ res, u32 n, int mode,
+                       Event* __restrict__ ring, u32 ring_cap, u64* __restrict__ ev_count) {
+  __shared__ u32 wt[32];
+  const u64 seq0 = *ev_count;
+  u32 carry = 0;
+  for (u32 base = 0; base < n; base += blockDim.x) {
+    const u32 k = base + threadIdx.x;
+    Desc d; Res r; u32 c = 0;
+    if (k < n) {
+      d = desc[k]; r = res[k];
+      if (mode == EM_RESTORE) c = (r.flag & R_SERVED) ? ((r.flag & R_OK) ? 2u : 4u) : 0u;
+      else c = (r.flag & R_OK) ? 1u : 0u;
+    }
+    u32 tot;
+    const u32 o = carry + block_scan_incl(c, wt, tot) - c;
+    if (c) {
+      u64 s = seq0 + o;
+      auto put = [&](u32 code, u32 aux, u64 arg) {
+        ring[s % ring_cap] = Event{s, d.id, code, aux, arg};
+        ++s;
+      };
+      if (mode == EM_ACCEPT) put(EV_ACCEPTED, d.N, d.P);
+      else if (mode == EM_MATERIALIZE) put(EV_MATERIALIZED, r.val, 0);
+      else if (mode == EM_OFFLOAD) put(EV_OFFLOADED, d.nb, r.chain);
+      else {
+        put(EV_RESTORE_REQUIRED, d.M, 0);
+        if (r.flag & R_OK) put(EV_RESTORED, d.nb, d.chain);
+        else {
+          put(EV_LOAD_FAILED, r.val, 0);
+          put(EV_RESTORATION_FAILED, 0, 0);
+          put(EV_ACTIVE_REQUEST_REFUSED, 1, d.id);
+        }
+      }
+    }
+    carry += tot;
+    __syncthreads();
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) *ev_count = seq0 + carry;
+}
+
+// fault injection (CPU->GPU transfers only): flip bit 0 of the listed staged bytes
+__global__ void k_bitflip(u8* staging, const u64* __restrict__ offs, u32 n) {
+  const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) staging[offs[i]] ^= 0x01;
+}
+
+}  // namespace rck

@@ -79,8 +79,9 @@ def _ids(rng, n):
     return sorted(ids, key=lambda x: (x * 0x9E3779B1) & 0xFFFFFFFF)   # fixed shuffle, not sorted by value
 
 
-def make_workload(index, n_claims=None, pool_blocks=None):
-    """configs[index]; n_claims / pool_blocks shrink it for parity tests (same recipe, fewer units)."""
+def make_workload(index, n_claims=None, pool_blocks=None, scale=1):
+    """configs[index]; n_claims / pool_blocks shrink it for parity tests (same recipe, fewer units);
+    scale divides the prefix lengths of config 4 (long context) for the same purpose."""
     g0 = GEOMS[index]
     g = Geometry(**{**g0.__dict__, "pool_blocks": pool_blocks or g0.pool_blocks})
     rng = np.random.default_rng(SEED0 + index)
@@ -151,7 +152,7 @@ def make_workload(index, n_claims=None, pool_blocks=None):
         ids = _ids(rng, n)
         claims = []
         for k in range(n):
-            P = int(rng.integers(32768, 131073))
+            P = int(rng.integers(32768 // scale, 131072 // scale + 1))
             u = float(rng.uniform(0.25, 1.0))
             claims.append(ClaimSpec(ids[k], P, N_PRED, max(N_PRED, int(u * P))))
         return Workload(4, g, claims, batch=8)

@@ -1,0 +1,221 @@
+"""GPU parity: librc (CUDA, through the C ABI) against the oracle, bit-exact, on BASELINE.json
+configs[0..4] (configs 1-4 at reduced unit counts so the oracle finishes in seconds; same recipe).
+Compared after every call: statuses, claim info, block tables, digests, chains, host-store
+bytes, allocator state, fill, raw pool bytes of live blocks, the claim-logical round trip and the
+event stream (P:L27 order per claim, batch-major across claims)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import rco, validator as V
+from paper_2606_01387_b200 import rc, workloads as W
+from parity_harness import Pair
+
+GOLD = [l.split("#")[0].strip() for l in open(__file__.rsplit("/", 1)[0] + "/golden/event_orders.txt")]
+GOLD = {l.split(":")[0].strip(): [x.strip() for x in l.split(":")[1].split(",")] for l in GOLD if l}
+
+
+def names(ev, cid):
+    return [rco.EV_NAMES[int(e["code"])] for e in ev if int(e["claim_id"]) == cid]
+
+
+@pytest.mark.parametrize("mover", [rc.MOVER_LDG, rc.MOVER_TMA])
+@pytest.mark.parametrize("kind", [W.FK_BITFLIP, W.FK_XFER_ERROR])
+@pytest.mark.parametrize("chunk_blocks", [5, 64])
+def test_tiny_full_parity(mover, kind, chunk_blocks):
+    wl = W.make_workload(0)
+    p = Pair(wl, 1 << 30, chunk_blocks=chunk_blocks, mover=mover)
+    wave = W.plan_waves(wl, 1 << 30)[0]
+    faults = [(cid, kind, prm) for cid, _, prm in wave.faults]
+    ev, st_r = p.run_wave(wave, faults=faults)
+    ok, why = V.validate(ev)
+    assert ok, why
+    for k, c in enumerate(wl.claims):
+        got = names(ev, c.claim_id)
+        if k == 6:
+            assert got == ["ACCEPTED"] and st_r[k] == rc.ST_BAD_STATE
+        elif k == 3:
+            assert got == GOLD["failure_path"] and st_r[k] == rc.ST_RESTORE_FAILED     # P:L27, exact
+        else:
+            assert got == GOLD["success_path"] and st_r[k] == rc.ST_OK
+    p.close()
+
+
+def _run_config(index, n_claims, pool_blocks, host_bytes, chunk_blocks, mover=rc.MOVER_AUTO, flags=0, scale=None,
+                sub=None):
+    kw = {} if scale is None else {"scale": scale}
+    wl = W.make_workload(index, n_claims=n_claims, pool_blocks=pool_blocks, **kw)
+    p = Pair(wl, host_bytes, chunk_blocks=chunk_blocks, mover=mover)
+    evs = []
+    for wave in W.plan_waves(wl, host_bytes):
+        ids = [wl.claims[k].claim_id for k in wave.claim_idx]
+        faults = wave.faults + (wl.decoys if flags else [])
+        batches = [ids[i:i + sub] for i in range(0, len(ids), sub)] if sub else None
+        ev, _ = p.run_wave(wave, restore_batches=batches, faults=faults, fault_flags=flags)
+        ok, why = V.validate(ev)
+        assert ok, why
+        evs.append(ev)
+    p.close()
+    return wl, evs
+
+
+@pytest.mark.parametrize("mover", [rc.MOVER_LDG, rc.MOVER_TMA])
+def test_config1_llama8b_reduced(mover):
+    wl, evs = _run_config(1, 6, 768, 2 << 30, chunk_blocks=37, mover=mover)
+    assert sum(len(e) for e in evs) > 0
+
+
+def test_config2_llama70b_shared_prefixes_reduced():
+    # Zipf-shared prefix groups: shared physical blocks (ref > 1), duplicated in the host store,
+    # restored in sub-batches that fit the free pool
+    _run_config(2, 4, 1300, 6 << 30, chunk_blocks=50, sub=2)
+
+
+def test_config3_fp8_decoys_reduced():
+    wl, evs = _run_config(3, 80, 2048, 4 << 30, chunk_blocks=100, flags=rc.FAULT_ALLOW_UNCLAIMED)
+    ev = np.concatenate(evs)
+    failed = {int(e["claim_id"]) for e in ev if int(e["code"]) == 8}
+    real = {c.claim_id for c in wl.claims if c.fault}
+    assert failed == real                   # decoys (never-accepted ids, id 0, not-restored claims) changed nothing
+
+
+def test_config4_long_context_interleaved_reduced():
+    # batches of 8 claims; restore of batch k overlapped with the offload of batch k+1 (begin/wait),
+    # compared with the oracle making the same calls synchronously in begin order
+    wl = W.make_workload(4, n_claims=24, pool_blocks=2048, scale=64)
+    host = 3 << 30
+    p = Pair(wl, host, chunk_blocks=64)
+    o, r = p.o, p.r
+    B = wl.batch
+    batches = [list(range(i, min(i + B, len(wl.claims)))) for i in range(0, len(wl.claims), B)]
+    waves = W.plan_waves(wl, host, max_claims_per_wave=B)
+    assert [w.claim_idx for w in waves] == batches
+
+    def admit(wave):
+        cl = [wl.claims[k] for k in wave.claim_idx]
+        ids = [c.claim_id for c in cl]
+        used, _ = o.pool_state()
+        free = np.nonzero(used == 0)[0].astype(np.uint32)
+        assert free.size >= wave.used_ids.size
+        remap = np.zeros(wl.geom.pool_blocks, np.uint32)       # place the wave's tables on currently free blocks
+        remap[wave.used_ids] = free[: wave.used_ids.size]
+        bt = remap[wave.bt_ids]
+        p.set_fill(remap[wave.fill_ids], wave.fill_val)
+        assert o.mark_used(remap[wave.used_ids]) == 0 and r.mark_used(remap[wave.used_ids]) == 0
+        args = (ids, [c.P for c in cl], [c.N for c in cl], wave.bt_off, bt)
+        assert np.array_equal(o.accept(*args), r.accept(*args))
+        assert np.array_equal(o.materialize(ids), r.materialize(ids))
+        return ids
+
+    prev = None
+    for wave in waves:
+        ids = admit(wave)
+        if prev is None:
+            assert np.array_equal(o.offload(ids), r.offload(ids))
+        else:
+            # oracle: restore(prev) then offload(ids); cuda: both in flight at once, begun in that order
+            sa_r, sa_o = o.restore(prev), o.offload(ids)
+            r.restore_begin(prev)
+            r.offload_begin(ids)
+            sb_o, sb_r = r.wait(0), r.wait(1)
+            assert np.array_equal(sa_r, sb_r) and np.array_equal(sa_o, sb_o)
+            p.check_claims(prev, "restore(k)")
+            assert np.array_equal(o.release(prev), r.release(prev))
+        p.check_claims(ids, "offload(k+1)", host=True)
+        p.check_pool_state("interleaved", bytes_too=True)
+        p.poison_free()
+        prev = ids
+    assert np.array_equal(o.restore(prev), r.restore(prev))
+    p.check_pool_state("last restore")
+    ev = p.check_events("interleaved")
+    ok, why = V.validate(ev)
+    assert ok, why
+    p.close()
+
+
+def test_edge_cases_fail_closed():
+    """Empty batches, unknown / duplicate ids, bad tables, restore-after-use, host-store and
+    free-block exhaustion: statuses and (absence of) events equal the oracle's."""
+    wl = W.make_workload(0)
+    g = wl.geom
+    host = 70 * g.blk_bytes                                    # room for two claims only (28-32 blocks each)
+    p = Pair(wl, host, chunk_blocks=7)
+    o, r = p.o, p.r
+    wave = W.plan_waves(wl, 1 << 30)[0]
+    cl = wl.claims
+    ids = [c.claim_id for c in cl]
+    p.set_fill(wave.fill_ids, wave.fill_val)
+    for x in (o, r):
+        assert x.mark_used(wave.used_ids) == 0
+        assert len(x.accept([], [], [], [0], [])) == 0 and len(x.offload([])) == 0 and len(x.restore([])) == 0
+    # bad tables: out of range id, repeated id, unused block, wrong length, N > P, id 0, in-batch duplicate id
+    t0 = wave.bt_ids[wave.bt_off[0]:wave.bt_off[1]].copy()
+    free_blk = int(np.setdiff1d(np.arange(g.pool_blocks), wave.used_ids)[0]) if wave.used_ids.size < g.pool_blocks else None
+    cases = []
+    bad = t0.copy(); bad[3] = g.pool_blocks + 5; cases.append((ids[0], cl[0].P, 448, bad))
+    bad = t0.copy(); bad[5] = bad[1]; cases.append((ids[0], cl[0].P, 448, bad))
+    if free_blk is not None:
+        bad = t0.copy(); bad[2] = free_blk; cases.append((ids[0], cl[0].P, 448, bad))
+    cases.append((ids[0], cl[0].P, 448, t0[:-1]))
+    cases.append((ids[0], cl[0].P, cl[0].P + 1, t0))
+    cases.append((0, cl[0].P, 448, t0))
+    cases.append((ids[0], cl[0].P, 448, t0))                   # valid
+    cases.append((ids[0], cl[0].P, 448, t0))                   # duplicate of the previous, same batch
+    off = np.cumsum([0] + [len(c[3]) for c in cases]).astype(np.uint32)
+    args = ([c[0] for c in cases], [c[1] for c in cases], [c[2] for c in cases], off, np.concatenate([c[3] for c in cases]))
+    sa, sb = o.accept(*args), r.accept(*args)
+    assert np.array_equal(sa, sb) and list(sa[-2:]) == [0, 4]
+    rest = list(range(1, len(cl)))
+    args = ([ids[k] for k in rest], [cl[k].P for k in rest], [cl[k].N for k in rest],
+            wave.bt_off[1:] - wave.bt_off[1], wave.bt_ids[wave.bt_off[1]:])
+    assert np.array_equal(o.accept(*args), r.accept(*args))
+    unknown = 0xDEADBEEF
+    q = ids + [unknown, ids[0]]
+    for fn in ("materialize", "offload", "restore"):           # offload: only the first two claims fit the host store
+        sa, sb = getattr(o, fn)(q), getattr(r, fn)(q)
+        assert np.array_equal(sa, sb), (fn, sa, sb)
+        p.check_claims(ids, fn)
+        p.check_pool_state(fn)
+    assert np.array_equal(o.restore(q), r.restore(q))          # restore-after-use: BAD_STATE everywhere
+    # free-block exhaustion at restore: offload two more, occupy the pool, restore both
+    sa, sb = o.offload(ids[2:4]), r.offload(ids[2:4])
+    assert np.array_equal(sa, sb) and list(sa) == [0, 0]
+    used, _ = o.pool_state()
+    free = np.nonzero(used == 0)[0].astype(np.uint32)
+    keep = o.claim_info(ids[2])["nb"] + 3
+    for x in (o, r):
+        x.mark_used(free[keep:])
+    sa, sb = o.restore(ids[2:4]), r.restore(ids[2:4])
+    assert np.array_equal(sa, sb) and list(sa) == [0, 6]
+    p.check_claims(ids, "exhaustion")
+    p.check_pool_state("exhaustion")
+    ev = p.check_events("edge")
+    ok, why = V.validate(ev)
+    assert ok, why
+    p.close()
+
+
+def test_determinism_repeated_runs():
+    """The analogue of 131/131 valid sequences: repeated runs give byte-identical streams."""
+    streams = []
+    for _ in range(3):
+        wl = W.make_workload(0)
+        p = Pair(wl, 1 << 30, chunk_blocks=9)
+        ev, _ = p.run_wave(W.plan_waves(wl, 1 << 30)[0])
+        streams.append(ev.tobytes())
+        p.close()
+    assert streams[0] == streams[1] == streams[2]
+
+
+def test_standalone_digest_matches_oracle():
+    import torch
+    wl = W.make_workload(0)
+    g = wl.geom
+    p = Pair(wl, 1 << 30, chunk_blocks=6)
+    x = torch.randint(0, 256, (20 * g.blk_bytes,), dtype=torch.uint8, device="cuda")
+    d, ms = p.r.digest_blocks(x.data_ptr(), 20)
+    xh = x.cpu().numpy()
+    want = [rco.block_digest(xh[i * g.blk_bytes:(i + 1) * g.blk_bytes], 2 * g.layers) for i in range(20)]
+    assert [int(v) for v in d] == want
+    p.close()
