@@ -1,0 +1,350 @@
+"""bench.py -- claim-scoped KV offload+restore throughput on B200 (BASELINE.json metric).
+
+A step is one pass of the whole hot path (accept, materialize, offload, restore, outcomes,
+release: SURVEY.md 8(a) rows a0-a8) over every wave of the workload.  Default workload:
+BASELINE.json configs[1] (Llama-3-8B KV shape, pool 8192 blocks = 16 GiB, 256 claims of 448-4096
+tokens, 2% injected restore failures), synthetic and seeded.  Prints ONE JSON line.
+
+  python bench.py --gpus 1 --steps 3 --warmup 3
+  python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N ...   (claims are independent:
+        every rank runs the workload on its own GPU, pool and host link; no data-path collective)
+  python bench.py --impl reference      (the oracle, as it stands, on the host cores; bounded sample)
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2606_01387_b200 import workloads as W  # noqa: E402
+
+METRIC = "kv_offload_restore_throughput"
+UNIT = "GB/s"
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i] == "Active"})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def host_ram_bytes():
+    try:
+        return os.sysconf("SC_PAGE_SIZE") * os.sysconf("SC_PHYS_PAGES")
+    except Exception:
+        return 64 << 30
+
+
+class Job:
+    """One rank's workload: context, resident pool, pre-marshalled waves."""
+
+    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None):
+        import torch
+        from paper_2606_01387_b200 import rc
+        self.torch, self.rc = torch, rc
+        self.wl = W.make_workload(index)
+        g = self.g = self.wl.geom
+        dev = torch.device("cuda", torch.cuda.current_device())
+        budget = int(0.5 * host_ram_bytes() / max(1, n_gpus))
+        self.host_store = min(g.pool_bytes, budget, host_cap or (1 << 62)) // g.blk_bytes * g.blk_bytes
+        self.waves = W.plan_waves(self.wl, self.host_store)
+        self.pool = W.pool_torch(g, dev, seed=W.SEED0 + 77 + rank)
+        self.fill = torch.zeros(g.pool_blocks, dtype=torch.uint8, device=dev)
+        n_max = max(len(w.claim_idx) for w in self.waves)
+        self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, self.pool, self.fill,
+                       self.host_store, staging_chunk_bytes=min(chunk_bytes, self.host_store), staging_chunks=2,
+                       max_claims=max(1024, 2 * n_max), max_table_entries=max(4 * g.pool_blocks, 1 << 16),
+                       max_events=max(1 << 16, 16 * n_max), mover=mover, grid_ctas=grid_ctas)
+        self.prep = []
+        for w in self.waves:
+            cl = [self.wl.claims[k] for k in w.claim_idx]
+            ids = np.array([c.claim_id for c in cl], np.uint64)
+            fid_h = torch.from_numpy(w.fill_ids.astype(np.int64)).pin_memory()
+            fval_h = torch.from_numpy(w.fill_val.copy()).pin_memory()
+            self.prep.append(dict(ids=ids, P=np.array([c.P for c in cl], np.uint32), N=np.array([c.N for c in cl], np.uint32),
+                                  bt_off=w.bt_off, bt_ids=w.bt_ids, used=w.used_ids, faults=w.faults,
+                                  fid_h=fid_h, fval_h=fval_h, fid_d=fid_h.to(dev), fval_d=fval_h.to(dev), n=len(cl)))
+        self.meta_h2d = sum(p["ids"].nbytes + p["P"].nbytes + p["N"].nbytes + p["bt_off"].nbytes + p["bt_ids"].nbytes +
+                            p["used"].nbytes + 4 * p["ids"].nbytes for p in self.prep)   # ids re-sent by 4 more calls
+        self.fill_h2d = sum(p["fid_h"].numel() * 8 + p["fval_h"].numel() for p in self.prep)
+        self.events = 0
+
+    def step(self, e2e):
+        r, torch = self.r, self.torch
+        n_ev = 0
+        for p in self.prep:
+            if e2e:     # fill[] arrives from pinned host memory inside the timed region
+                self.fill.index_copy_(0, p["fid_h"].to(self.fill.device, non_blocking=True),
+                                      p["fval_h"].to(self.fill.device, non_blocking=True))
+            else:       # resident inputs: fill values already in HBM
+                self.fill.index_copy_(0, p["fid_d"], p["fval_d"])
+            torch.cuda.current_stream().synchronize()
+            r.mark_used(p["used"])
+            r.accept(p["ids"], p["P"], p["N"], p["bt_off"], p["bt_ids"])
+            r.materialize(p["ids"])
+            r.offload(p["ids"])
+            r.set_faults(p["faults"])
+            r.restore(p["ids"])
+            n_ev += len(r.outcomes(cap=8 * p["n"]))
+            r.release(p["ids"])
+        self.events = n_ev
+        return n_ev
+
+
+def time_steps(job, steps, warmup, e2e, dist):
+    torch = job.torch
+    for _ in range(warmup):
+        job.step(e2e)
+    job.r.stats_reset()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(steps):
+        job.step(e2e)
+    e1.record()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    if dist is not None:
+        dist.barrier()
+    ms = max(e0.elapsed_time(e1), 0.0)
+    st = job.r.stats()
+    return ms, wall * 1e3, st
+
+
+class OracleJob:
+    """The oracle (oracle/, plain single-threaded C++) on a bounded sample of the same workload:
+    the first `n_claims` claims of the config on a reduced pool, same recipe, same calls."""
+
+    def __init__(self, index, n_claims, pool_blocks):
+        from oracle import rco
+        self.wl = W.make_workload(index, n_claims=n_claims, pool_blocks=pool_blocks)
+        g = self.g = self.wl.geom
+        self.pool = W.pool_host(g)
+        self.fill = np.zeros(g.pool_blocks, np.uint8)
+        self.host_store = g.pool_bytes
+        self.waves = W.plan_waves(self.wl, self.host_store)
+        self.o = rco.Oracle(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, self.pool,
+                            self.fill, self.host_store)
+        self.sample = "first %d claims of configs[%d] on a %d-block pool (%d waves), offload+restore+outcomes" % (
+            n_claims, index, pool_blocks, len(self.waves))
+
+    def step(self):
+        o, wl = self.o, self.wl
+        moved = 0
+        for w in self.waves:
+            cl = [wl.claims[k] for k in w.claim_idx]
+            ids = [c.claim_id for c in cl]
+            self.fill[w.fill_ids] = w.fill_val
+            o.mark_used(w.used_ids)
+            o.accept(ids, [c.P for c in cl], [c.N for c in cl], w.bt_off, w.bt_ids)
+            o.materialize(ids)
+            st = o.offload(ids)
+            nb = sum(o.claim_info(c)["nb"] for c, s in zip(ids, st) if s == 0)
+            o.set_faults(w.faults)
+            st = o.restore(ids)
+            o.outcomes(cap=8 * len(ids))
+            moved += nb * self.g.blk_bytes * 2        # once per direction, as the GPU arm counts payload
+            o.release(ids)
+        return moved
+
+
+def oracle_sample_shape(index):
+    # sized for roughly 10 s of single-thread work per pass
+    return {0: (8, 256), 1: (8, 640), 2: (3, 700), 3: (96, 2560), 4: (8, 640)}[index]
+
+
+def run_oracle(index, steps, warmup):
+    n_claims, pool_blocks = oracle_sample_shape(index)
+    job = OracleJob(index, n_claims, pool_blocks)
+    for _ in range(warmup):
+        job.step()
+    t0 = time.perf_counter()
+    moved = 0
+    for _ in range(steps):
+        moved += job.step()
+    dt = time.perf_counter() - t0
+    claims = sum(len(w.claim_idx) for w in job.waves) * steps
+    return {"value": moved / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": job.sample,
+            "claims_per_s": claims / dt, "seconds": dt, "steps": steps}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (1 = the metric's workload)")
+    ap.add_argument("--chunk-mib", type=int, default=1024)
+    ap.add_argument("--mover", default="auto", choices=["auto", "ldg", "tma"])
+    ap.add_argument("--grid", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per gather launch (profiles/), if known")
+    a = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    wname = "configs[%d] %s" % (a.config, W.GEOMS[a.config].name)
+
+    if a.impl == "reference":
+        if rank != 0:
+            return
+        steps, warmup = max(1, min(a.steps, 3)), min(a.warmup, 1)
+        res = run_oracle(a.config, steps, warmup)
+        line = {"impl": "reference", "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": a.gpus,
+                "steps": steps, "warmup": warmup, "ms_per_step": res["seconds"] * 1e3 / steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+                "config": {"workload": wname, "sample": res["sample"]}, "claims_per_s": res["claims_per_s"],
+                "cpu_baseline": {"value": res["value"], "unit": UNIT, "cores": 1, "kind": "oracle", "sample": res["sample"]},
+                "e2e": {"value": res["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line))
+        return
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; librc has no CPU path (use --impl reference for the oracle)")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2606_01387_b200 import rc
+    mover = {"auto": rc.MOVER_AUTO, "ldg": rc.MOVER_LDG, "tma": rc.MOVER_TMA}[a.mover]
+    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid)
+    g = job.g
+    link = {}
+    if world == 1:
+        for name, d in (("d2h", 0), ("h2d", 1), ("both", 2)):
+            link[name] = job.r.measure_link(1 << 30, d, reps=5)
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms, wall_ms, st = time_steps(job, a.steps, a.warmup, False, dist)
+    clocks = sampler.stop() if sampler else None
+    payload = st["bytes_d2h"] + st["bytes_h2d"]
+    claims = sum(p["n"] for p in job.prep) * a.steps
+    e2e = None
+    if not a.no_e2e:
+        ms2, _, st2 = time_steps(job, a.steps, min(a.warmup, 1), True, dist)
+        e2e = (ms2, st2)
+
+    def allred(x, op):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=op)
+        return float(t.item())
+
+    ms_max = allred(ms, dist.ReduceOp.MAX if dist else None)
+    payload_all = allred(float(payload), dist.ReduceOp.SUM if dist else None)
+    claims_all = allred(float(claims), dist.ReduceOp.SUM if dist else None)
+    launches_all = allred(float(st["kernel_launches"]), dist.ReduceOp.SUM if dist else None)
+    if e2e:
+        ms2_max = allred(e2e[0], dist.ReduceOp.MAX if dist else None)
+        pay2_all = allred(float(e2e[1]["bytes_d2h"] + e2e[1]["bytes_h2d"]), dist.ReduceOp.SUM if dist else None)
+    if rank != 0:
+        dist.destroy_process_group()
+        return
+
+    peak, peak_src = peaks()
+    blk = g.blk_bytes
+
+    def roof(ms_k, launches, blocks):
+        if not launches or ms_k <= 0:
+            return None
+        per_launch = 2.0 * blk * blocks / launches                  # algorithmic bytes: read blk + write blk per block
+        ach = per_launch / (ms_k / launches * 1e6)
+        return {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": a.traffic, "peak_source": peak_src, "launches": launches,
+                "avg_launch_ms": ms_k / launches, "algorithmic_bytes_per_launch": per_launch}
+
+    roofline = roof(st["ms_gather"], st["gather_launches"], st["gather_blocks"])
+    if roofline:
+        roofline["kernel"] = "k_move_hash%s<GATHER> (K2 gather+checksum)" % ("_tma" if mover != rc.MOVER_LDG else "")
+    roof_sc = roof(st["ms_scatter"], st["scatter_launches"], st["scatter_blocks"])
+    if roof_sc:
+        roof_sc["kernel"] = "k_move_hash%s<SCATTER> (K4 scatter+checksum)" % ("_tma" if mover != rc.MOVER_LDG else "")
+        roof_sc["traffic"] = None
+    links = None
+    if link:
+        d2h = st["bytes_d2h"] / (st["ms_d2h"] * 1e6) if st["ms_d2h"] > 0 else None
+        h2d = st["bytes_h2d"] / (st["ms_h2d"] * 1e6) if st["ms_h2d"] > 0 else None
+        links = {"ceiling_gbs": link, "d2h_gbs": d2h, "h2d_gbs": h2d,
+                 "d2h_frac": d2h / link["d2h"] if d2h else None, "h2d_frac": h2d / link["h2d"] if h2d else None,
+                 "ceiling_how": "best of 5 cudaMemcpyAsync of 1 GiB, pinned store <-> staging, same process"}
+    line = {"metric": METRIC, "value": payload_all / (ms_max * 1e6), "unit": UNIT, "n_gpus": world, "steps": a.steps,
+            "warmup": a.warmup, "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": wname, "claims": len(job.wl.claims), "pool_blocks": g.pool_blocks, "blk_bytes": blk,
+                       "waves": len(job.waves), "host_store_bytes": job.host_store, "staging_chunk_bytes": a.chunk_mib << 20,
+                       "mover": a.mover, "l2": "inputs larger than L2 (16 GiB pool, 1 GiB staging chunks)",
+                       "parallelism": "claims independent: one replica of the workload per GPU, no collective"},
+            "claims_per_s": claims_all / (ms_max / 1e3), "payload_bytes_per_step": payload_all / a.steps,
+            "wall_ms_per_step": wall_ms / a.steps, "clocks": clocks, "gpu_launches": int(launches_all),
+            "roofline": roofline, "roofline_scatter": roof_sc, "host_link": links}
+    if e2e:
+        n_ev = job.events
+        line["e2e"] = {"value": pay2_all / (ms2_max * 1e6), "unit": UNIT,
+                       "h2d_bytes_per_step": int(e2e[1]["bytes_h2d"] / a.steps + job.meta_h2d + job.fill_h2d),
+                       "d2h_bytes_per_step": int(e2e[1]["bytes_d2h"] / a.steps + 32 * n_ev + 4 * 5 * claims / a.steps),
+                       "ms_per_step": ms2_max / a.steps,
+                       "what": "same step through the C ABI with host arrays; fill[] sent from pinned host memory, "
+                               "statuses and the event stream read back, inside the timed region"}
+    if world == 1 and not a.no_cpu_baseline:
+        line["cpu_baseline"] = {k: v for k, v in run_oracle(a.config, 1, 0).items() if k in
+                                ("value", "unit", "cores", "kind", "sample", "claims_per_s", "seconds")}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
