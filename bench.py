@@ -82,7 +82,7 @@ def host_ram_bytes():
 class Job:
     """One rank's workload: context, resident pool, pre-marshalled waves."""
 
-    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None):
+    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True):
         import torch
         from paper_2606_01387_b200 import rc
         self.torch, self.rc = torch, rc
@@ -91,7 +91,13 @@ class Job:
         dev = torch.device("cuda", torch.cuda.current_device())
         budget = int(0.5 * host_ram_bytes() / max(1, n_gpus))
         self.host_store = min(g.pool_bytes, budget, host_cap or (1 << 62)) // g.blk_bytes * g.blk_bytes
-        self.waves = W.plan_waves(self.wl, self.host_store)
+        # pipelined: restore of wave k overlaps the offload of wave k+1 (full-duplex host link), so two waves
+        # share the pool and the host store; serial: one wave owns both
+        self.pipelined = pipelined
+        if pipelined:
+            self.waves = W.plan_waves(self.wl, self.host_store // 2, pool_blocks=g.pool_blocks // 2)
+        else:
+            self.waves = W.plan_waves(self.wl, self.host_store)
         self.pool = W.pool_torch(g, dev, seed=W.SEED0 + 77 + rank)
         self.fill = torch.zeros(g.pool_blocks, dtype=torch.uint8, device=dev)
         n_max = max(len(w.claim_idx) for w in self.waves)
@@ -113,24 +119,44 @@ class Job:
         self.fill_h2d = sum(p["fid_h"].numel() * 8 + p["fval_h"].numel() for p in self.prep)
         self.events = 0
 
+    def _admit(self, p, e2e):
+        if e2e:     # fill[] arrives from pinned host memory inside the timed region
+            self.fill.index_copy_(0, p["fid_h"].to(self.fill.device, non_blocking=True),
+                                  p["fval_h"].to(self.fill.device, non_blocking=True))
+        else:       # resident inputs: fill values already in HBM
+            self.fill.index_copy_(0, p["fid_d"], p["fval_d"])
+        self.torch.cuda.current_stream().synchronize()
+        self.r.mark_used(p["used"])
+        self.r.accept(p["ids"], p["P"], p["N"], p["bt_off"], p["bt_ids"])
+        self.r.materialize(p["ids"])
+
     def step(self, e2e):
-        r, torch = self.r, self.torch
+        r = self.r
         n_ev = 0
-        for p in self.prep:
-            if e2e:     # fill[] arrives from pinned host memory inside the timed region
-                self.fill.index_copy_(0, p["fid_h"].to(self.fill.device, non_blocking=True),
-                                      p["fval_h"].to(self.fill.device, non_blocking=True))
-            else:       # resident inputs: fill values already in HBM
-                self.fill.index_copy_(0, p["fid_d"], p["fval_d"])
-            torch.cuda.current_stream().synchronize()
-            r.mark_used(p["used"])
-            r.accept(p["ids"], p["P"], p["N"], p["bt_off"], p["bt_ids"])
-            r.materialize(p["ids"])
-            r.offload(p["ids"])
-            r.set_faults(p["faults"])
-            r.restore(p["ids"])
-            n_ev += len(r.outcomes(cap=8 * p["n"]))
-            r.release(p["ids"])
+        if not self.pipelined:
+            for p in self.prep:
+                self._admit(p, e2e)
+                r.offload(p["ids"])
+                r.set_faults(p["faults"])
+                r.restore(p["ids"])
+                n_ev += len(r.outcomes(cap=8 * p["n"]))
+                r.release(p["ids"])
+        else:
+            # wave k is restored while wave k+1 is offloaded; metadata steps run in _begin order
+            self._admit(self.prep[0], e2e)
+            r.offload(self.prep[0]["ids"])
+            for k, p in enumerate(self.prep):
+                nxt = self.prep[k + 1] if k + 1 < len(self.prep) else None
+                if nxt is not None:
+                    self._admit(nxt, e2e)
+                r.set_faults(p["faults"])
+                r.restore_begin(p["ids"])
+                if nxt is not None:
+                    r.offload_begin(nxt["ids"])
+                    r.wait(0)
+                r.wait(1)
+                n_ev += len(r.outcomes(cap=16 * max(p["n"], nxt["n"] if nxt else 0)))
+                r.release(p["ids"])
         self.events = n_ev
         return n_ev
 
@@ -225,6 +251,7 @@ def main():
     ap.add_argument("--chunk-mib", type=int, default=1024)
     ap.add_argument("--mover", default="auto", choices=["auto", "ldg", "tma"])
     ap.add_argument("--grid", type=int, default=0)
+    ap.add_argument("--serial", action="store_true", help="one wave at a time: offload, then restore (no duplex overlap)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per gather launch (profiles/), if known")
@@ -259,7 +286,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2606_01387_b200 import rc
     mover = {"auto": rc.MOVER_AUTO, "ldg": rc.MOVER_LDG, "tma": rc.MOVER_TMA}[a.mover]
-    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid)
+    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial)
     g = job.g
     link = {}
     if world == 1:
@@ -319,17 +346,21 @@ def main():
         h2d = st["bytes_h2d"] / (st["ms_h2d"] * 1e6) if st["ms_h2d"] > 0 else None
         links = {"ceiling_gbs": link, "d2h_gbs": d2h, "h2d_gbs": h2d,
                  "d2h_frac": d2h / link["d2h"] if d2h else None, "h2d_frac": h2d / link["h2d"] if h2d else None,
-                 "ceiling_how": "best of 5 cudaMemcpyAsync of 1 GiB, pinned store <-> staging, same process"}
+                 "ceiling_how": "best of 5 cudaMemcpyAsync of 1 GiB, pinned store <-> staging, same process; "
+                                "'both' = D2H and H2D at once (sum); fractions are per direction over that "
+                                "direction's copy-stream busy time against its one-way ceiling"}
     line = {"metric": METRIC, "value": payload_all / (ms_max * 1e6), "unit": UNIT, "n_gpus": world, "steps": a.steps,
             "warmup": a.warmup, "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": wname, "claims": len(job.wl.claims), "pool_blocks": g.pool_blocks, "blk_bytes": blk,
                        "waves": len(job.waves), "host_store_bytes": job.host_store, "staging_chunk_bytes": a.chunk_mib << 20,
-                       "mover": a.mover, "l2": "inputs larger than L2 (16 GiB pool, 1 GiB staging chunks)",
+                       "mover": a.mover, "schedule": "serial" if a.serial else "restore(k) overlapped with offload(k+1)", "l2": "inputs larger than L2 (16 GiB pool, 1 GiB staging chunks)",
                        "parallelism": "claims independent: one replica of the workload per GPU, no collective"},
             "claims_per_s": claims_all / (ms_max / 1e3), "payload_bytes_per_step": payload_all / a.steps,
             "wall_ms_per_step": wall_ms / a.steps, "clocks": clocks, "gpu_launches": int(launches_all),
             "roofline": roofline, "roofline_scatter": roof_sc, "host_link": links}
+    if links:
+        links["value_over_duplex_ceiling"] = line["value"] / link["both"]
     if e2e:
         n_ev = job.events
         line["e2e"] = {"value": pay2_all / (ms2_max * 1e6), "unit": UNIT,

@@ -578,14 +578,14 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   if (served.empty()) return RC_OK;
   op.n = n; op.status = st; op.blocks = T; op.copy_bytes = 0; op.launches = 0;
   int rc;
-  if ((rc = upload_desc(c, 0, n))) return rc;
-  k_offsets<<<1, 1024, 0, c->meta>>>(c->d_desc[0], n, c->d_off[0]);
+  // The head (offsets, compaction) only reads tables that completed calls wrote, so it runs on the gather
+  // stream: an offload begun after a restore does not queue behind that restore's tail on `meta`.
+  CK(cudaMemcpyAsync(c->d_desc[0], c->h_desc[0], (u64)n * sizeof(Desc), cudaMemcpyHostToDevice, c->gather));
+  k_offsets<<<1, 1024, 0, c->gather>>>(c->d_desc[0], n, c->d_off[0]);
   CKL();
-  k_worklist<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_bt, nullptr, c->d_phys[0], 0);
+  k_worklist<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_bt, nullptr, c->d_phys[0], 0);
   CKL();
   c->st.kernel_launches += 2;
-  CK(cudaEventRecord(c->ev_plan[0], c->meta));
-  CK(cudaStreamWaitEvent(c->gather, c->ev_plan[0], 0));
   size_t si = 0;
   u32 ci = 0;
   for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks, ++ci) {
