@@ -82,7 +82,7 @@ def host_ram_bytes():
 class Job:
     """One rank's workload: context, resident pool, pre-marshalled waves."""
 
-    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True):
+    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=4):
         import torch
         from paper_2606_01387_b200 import rc
         self.torch, self.rc = torch, rc
@@ -91,11 +91,12 @@ class Job:
         dev = torch.device("cuda", torch.cuda.current_device())
         budget = int(0.5 * host_ram_bytes() / max(1, n_gpus))
         self.host_store = min(g.pool_bytes, budget, host_cap or (1 << 62)) // g.blk_bytes * g.blk_bytes
-        # pipelined: restore of wave k overlaps the offload of wave k+1 (full-duplex host link), so two waves
-        # share the pool and the host store; serial: one wave owns both
+        # pipelined: restore of wave k overlaps the offload of wave k+1 (full-duplex host link); waves of 1/wave_frac
+        # of the pool (>= 2 so that two waves fit) keep the un-overlapped first offload and last restore short;
+        # serial: one wave owns the pool and the host store
         self.pipelined = pipelined
         if pipelined:
-            self.waves = W.plan_waves(self.wl, self.host_store // 2, pool_blocks=g.pool_blocks // 2)
+            self.waves = W.plan_waves(self.wl, self.host_store // wave_frac, pool_blocks=g.pool_blocks // wave_frac)
         else:
             self.waves = W.plan_waves(self.wl, self.host_store)
         self.pool = W.pool_torch(g, dev, seed=W.SEED0 + 77 + rank)
@@ -248,10 +249,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (1 = the metric's workload)")
-    ap.add_argument("--chunk-mib", type=int, default=1024)
+    ap.add_argument("--chunk-mib", type=int, default=2048)
     ap.add_argument("--mover", default="auto", choices=["auto", "ldg", "tma"])
     ap.add_argument("--grid", type=int, default=0)
     ap.add_argument("--serial", action="store_true", help="one wave at a time: offload, then restore (no duplex overlap)")
+    ap.add_argument("--wave-frac", type=int, default=4, help="pipelined schedule: a wave uses 1/N of the pool (N >= 2)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per gather launch (profiles/), if known")
@@ -286,7 +288,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2606_01387_b200 import rc
     mover = {"auto": rc.MOVER_AUTO, "ldg": rc.MOVER_LDG, "tma": rc.MOVER_TMA}[a.mover]
-    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial)
+    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac))
     g = job.g
     link = {}
     if world == 1:
@@ -354,7 +356,7 @@ def main():
             "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": wname, "claims": len(job.wl.claims), "pool_blocks": g.pool_blocks, "blk_bytes": blk,
                        "waves": len(job.waves), "host_store_bytes": job.host_store, "staging_chunk_bytes": a.chunk_mib << 20,
-                       "mover": a.mover, "schedule": "serial" if a.serial else "restore(k) overlapped with offload(k+1)", "l2": "inputs larger than L2 (16 GiB pool, 1 GiB staging chunks)",
+                       "mover": a.mover, "schedule": "serial" if a.serial else "restore(k) overlapped with offload(k+1)", "l2": "inputs larger than L2 (pool %d GiB, staging chunks %d MiB, L2 126 MB)" % (g.pool_bytes >> 30, a.chunk_mib),
                        "parallelism": "claims independent: one replica of the workload per GPU, no collective"},
             "claims_per_s": claims_all / (ms_max / 1e3), "payload_bytes_per_step": payload_all / a.steps,
             "wall_ms_per_step": wall_ms / a.steps, "clocks": clocks, "gpu_launches": int(launches_all),

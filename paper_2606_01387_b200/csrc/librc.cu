@@ -15,6 +15,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <string>
@@ -100,7 +101,7 @@ struct Op {
 
 struct rc_ctx {
   rc_config cfg;
-  u32 G = 0, vpp = 0, NB = 0, R = 0, sms = 0, grid = 0, tile = 0, mover = 0;
+  u32 G = 0, vpp = 0, NB = 0, R = 0, sms = 0, grid = 0, tma_variant = 0, mover = 0;
   u64 page = 0, blk = 0, chunk_blocks = 0, host_blocks = 0, cap_entries = 0, desc_cap = 0;
   cudaStream_t meta = 0, gather = 0, d2h = 0, scatter = 0, h2d = 0, util = 0;
   bool own[5] = {false, false, false, false, false};
@@ -165,34 +166,25 @@ static void launch_ldg(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, 
     k_move_hash<MODE, 1><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp);
 }
 
-constexpr int TMA_STAGES = 4;
-template <int MODE, int TILE>
-static void launch_tma_t(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
-  const u32 pages = n_items * c->G;
-  const u32 grid = std::min(pages, c->grid);
-  k_move_hash_tma<MODE, TMA_STAGES, TILE><<<grid, LANES, TMA_STAGES * TILE, s>>>(c->pool, staging, phys, part, n_items,
-                                                                             c->G, c->NB, (u32)c->page);
-}
-template <int MODE>
-static void launch_tma(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
-  if (c->tile == 16384) launch_tma_t<MODE, 16384>(c, s, staging, phys, part, n_items);
-  else if (c->tile == 8192) launch_tma_t<MODE, 8192>(c, s, staging, phys, part, n_items);
-  else launch_tma_t<MODE, 4096>(c, s, staging, phys, part, n_items);
-}
+// (TILE, STAGES) variants of the TMA mover; RC_TMA_VARIANT=<index> overrides the default choice (tuning sweeps)
+typedef void (*tma_fn)(u8*, u8*, const u32*, u64*, u32, u32, u32, u32);
+struct TmaVariant { u32 tile, stages, ctas_per_sm; tma_fn fn[3]; };
+#define TMA_V(T, S, C) {T, S, C, {k_move_hash_tma<MV_GATHER, S, T>, k_move_hash_tma<MV_SCATTER, S, T>, k_move_hash_tma<MV_DIGEST, S, T>}}
+// Measured on B200 (profiles/r01_mover_sweep.md): about 96 KiB of bulk loads in flight per SM is the sweet
+// spot -- 32 KiB tiles x 3 stages x 1 CTA/SM (variant 7) or 16 KiB x 3 x 2 CTAs/SM (variant 3); more bytes in
+// flight lowers DRAM efficiency, fewer leaves the latency uncovered.
+static const TmaVariant kTma[] = {TMA_V(4096, 4, 2), TMA_V(8192, 4, 2), TMA_V(8192, 8, 1), TMA_V(16384, 3, 2), TMA_V(16384, 4, 1),
+                                  TMA_V(16384, 6, 1), TMA_V(32768, 2, 2), TMA_V(32768, 3, 1), TMA_V(16384, 12, 1), TMA_V(32768, 6, 1)};
+constexpr int kTmaN = sizeof(kTma) / sizeof(kTma[0]);
+
 template <int MODE>
 static void launch_move(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
-  if (c->mover == RC_MOVER_TMA) launch_tma<MODE>(c, s, staging, phys, part, n_items);
-  else launch_ldg<MODE>(c, s, staging, phys, part, n_items);
+  if (c->mover == RC_MOVER_TMA) {
+    const TmaVariant& v = kTma[c->tma_variant];
+    const u32 grid = std::min(n_items * c->G, c->grid);
+    v.fn[MODE]<<<grid, TMA_THREADS, v.tile * v.stages, s>>>(c->pool, staging, phys, part, n_items, c->G, c->NB, (u32)c->page);
+  } else launch_ldg<MODE>(c, s, staging, phys, part, n_items);
   c->st.kernel_launches++;
-}
-
-template <int MODE, int TILE>
-static cudaError_t tma_attr(int& occ) {
-  cudaError_t e = cudaFuncSetAttribute(k_move_hash_tma<MODE, TMA_STAGES, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       TMA_STAGES * TILE);
-  if (e != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hash_tma<MODE, TMA_STAGES, TILE>, LANES,
-                                                       TMA_STAGES * TILE);
 }
 
 // ---- create / destroy ------------------------------------------------------------------------
@@ -312,25 +304,26 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   if (c->host_blocks) CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocDefault), RC_ERR_NOMEM);
   // launch geometry of the movers
   c->mover = cfg->mover == RC_MOVER_AUTO ? RC_MOVER_TMA : cfg->mover;
-  c->tile = page % 16384 == 0 ? 16384 : (page % 8192 == 0 ? 8192 : 4096);
   int occ = 0;
   if (c->mover == RC_MOVER_TMA) {
-    int o2 = 0, o3 = 0;
-    if (c->tile == 16384) {
-      CC((tma_attr<MV_GATHER, 16384>(occ)), RC_ERR_CUDA); CC((tma_attr<MV_SCATTER, 16384>(o2)), RC_ERR_CUDA);
-      CC((tma_attr<MV_DIGEST, 16384>(o3)), RC_ERR_CUDA);
-    } else if (c->tile == 8192) {
-      CC((tma_attr<MV_GATHER, 8192>(occ)), RC_ERR_CUDA); CC((tma_attr<MV_SCATTER, 8192>(o2)), RC_ERR_CUDA);
-      CC((tma_attr<MV_DIGEST, 8192>(o3)), RC_ERR_CUDA);
-    } else {
-      CC((tma_attr<MV_GATHER, 4096>(occ)), RC_ERR_CUDA); CC((tma_attr<MV_SCATTER, 4096>(o2)), RC_ERR_CUDA);
-      CC((tma_attr<MV_DIGEST, 4096>(o3)), RC_ERR_CUDA);
+    int want = page % 32768 == 0 ? 7 : (page % 16384 == 0 ? 3 : (page % 8192 == 0 ? 1 : 0));
+    if (const char* e = getenv("RC_TMA_VARIANT")) want = atoi(e);
+    if (want < 0 || want >= kTmaN || page % kTma[want].tile != 0) return fail(RC_ERR_INVALID, "RC_TMA_VARIANT", cudaSuccess);
+    c->tma_variant = want;
+    const TmaVariant& v = kTma[want];
+    occ = 1 << 30;
+    for (int m = 0; m < 3; ++m) {
+      int o = 0;
+      CC(cudaFuncSetAttribute(v.fn[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(v.tile * v.stages)), RC_ERR_CUDA);
+      CC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, v.fn[m], TMA_THREADS, v.tile * v.stages), RC_ERR_CUDA);
+      occ = std::min(occ, o);
     }
-    occ = std::min(occ, std::min(o2, o3));
   } else {
     CC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hash<MV_GATHER, 8>, LANES, 0), RC_ERR_CUDA);
   }
   if (occ < 1) occ = 1;
+  if (c->mover == RC_MOVER_TMA) occ = std::min<int>(occ, kTma[c->tma_variant].ctas_per_sm);
+  else occ = std::min(occ, 2);
   c->grid = cfg->grid_ctas ? cfg->grid_ctas : c->sms * (u32)occ;
 #undef CC
   *out = c;

@@ -169,22 +169,33 @@ template <int N> __device__ __forceinline__ void bulk_wait_read() {
 }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+__device__ __forceinline__ void mbar_arrive(u64* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(bar)) : "memory");
+}
+
+// Warp roles: warps 0..7 = the 256 checksum lanes (consumers); warp 8 lane 0 = load producer; warp 9
+// lane 0 = store issuer.  full[s]: tile landed (tx bytes).  empty[s]: 8 consumer warps (+ the store
+// issuer once its bulk store has finished reading the stage) released the stage.  No block barrier in
+// the steady state: the producer runs STAGES tiles ahead, consumers and stores follow at their own pace.
+constexpr int TMA_THREADS = LANES + 64;
+
 template <int MODE, int STAGES, int TILE>
-__global__ void __launch_bounds__(LANES)
+__global__ void __launch_bounds__(TMA_THREADS)
 k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __restrict__ phys,
                 u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 page_bytes) {
   extern __shared__ __align__(128) u8 smem[];
   __shared__ __align__(8) u64 full[STAGES];
-  const u32 t = threadIdx.x;
+  __shared__ __align__(8) u64 empty[STAGES];
+  const u32 t = threadIdx.x, warp = t >> 5;
   const u32 n_pages = n_items * G;
   const u32 tpp = page_bytes / TILE;                     // tiles per page (page % TILE == 0)
-  constexpr u32 VT = TILE / (16 * LANES);                // vectors per thread per tile
+  constexpr u32 VT = TILE / (16 * LANES);                // vectors per lane per tile
   if (t == 0) {
-    for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], WPC + (MODE != MV_DIGEST ? 1 : 0)); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  // this CTA's tile sequence: for page u = blockIdx.x + k*grid, tiles 0..tpp-1
+  // this CTA's tile sequence: pages blockIdx.x + k*grid, tiles 0..tpp-1 of each
   const u32 my_pages = (n_pages > blockIdx.x) ? (n_pages - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
   const u64 n_tiles = (u64)my_pages * tpp;
   auto addr = [&](u64 q, u8*& gsrc, u8*& gdst, bool& skip) {
@@ -199,38 +210,51 @@ k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __re
     gsrc = (MODE == MV_GATHER) ? pp : sp;
     gdst = (MODE == MV_GATHER) ? sp : pp;
   };
-  if (t == 0) {                                            // prologue: fill the ring
-    for (u64 q = 0; q < n_tiles && q < STAGES; ++q) {
-      u8 *gs, *gd; bool skip; addr(q, gs, gd, skip);
-      mbar_expect_tx(&full[q], TILE);
-      bulk_g2s(smem + (u32)q * TILE, gs, TILE, &full[q]);
+  if (warp == WPC) {                                       // ---- load producer
+    if (t == LANES) {
+      for (u64 q = 0; q < n_tiles; ++q) {
+        const u32 s = (u32)(q % STAGES);
+        if (q >= STAGES) mbar_wait(&empty[s], (u32)(((q / STAGES) - 1) & 1));
+        u8 *gs, *gd; bool skip; addr(q, gs, gd, skip);
+        mbar_expect_tx(&full[s], TILE);
+        bulk_g2s(smem + s * TILE, gs, TILE, &full[s]);
+      }
     }
-  }
-  u64 h = 0;
-  for (u64 q = 0; q < n_tiles; ++q) {
-    const u32 s = (u32)(q % STAGES), ph = (u32)((q / STAGES) & 1);
-    const u32 tile = (u32)(q % tpp);
-    if (tile == 0) h = (u64)(t + 1) * C1;
-    mbar_wait(&full[s], ph);
-    u8 *gs, *gd; bool skip; addr(q, gs, gd, skip);
-    if (MODE != MV_DIGEST && t == 0 && !skip) { bulk_s2g(gd, smem + s * TILE, TILE); bulk_commit(); }
-    const uint4* sv = reinterpret_cast<const uint4*>(smem + s * TILE) + t;
+  } else if (warp == WPC + 1) {                            // ---- store issuer
+    if (MODE != MV_DIGEST && t == LANES + 32) {
+      for (u64 q = 0; q < n_tiles; ++q) {
+        const u32 s = (u32)(q % STAGES);
+        mbar_wait(&full[s], (u32)((q / STAGES) & 1));
+        u8 *gs, *gd; bool skip; addr(q, gs, gd, skip);
+        if (!skip) bulk_s2g(gd, smem + s * TILE, TILE);
+        bulk_commit();
+        if (q > 0) { bulk_wait_read<1>(); mbar_arrive(&empty[(u32)((q - 1) % STAGES)]); }   // store q-1 drained its stage
+      }
+      if (n_tiles) { bulk_wait_read<0>(); mbar_arrive(&empty[(u32)((n_tiles - 1) % STAGES)]); }
+      asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    }
+  } else {                                                 // ---- consumers: lane t folds vectors t, t+256, ...
+    u64 h = 0;
+    for (u64 q = 0; q < n_tiles; ++q) {
+      const u32 s = (u32)(q % STAGES);
+      const u32 k = (u32)(q / tpp), tile = (u32)(q - (u64)k * tpp);
+      if (tile == 0) h = (u64)(t + 1) * C1;
+      mbar_wait(&full[s], (u32)((q / STAGES) & 1));
+      const uint4* sv = reinterpret_cast<const uint4*>(smem + s * TILE) + t;
 #pragma unroll
-    for (u32 j = 0; j < VT; ++j) h = fold(h, sv[j * LANES]);
-    if (tile == tpp - 1 && !skip) {
-      const u64 sum = warp_sum64(mixL(h));
-      const u32 k = (u32)(q / tpp), u = blockIdx.x + k * gridDim.x;
-      if ((t & 31) == 0) part[(u64)u * WPC + (t >> 5)] = sum;
-    }
-    __syncthreads();                                       // every thread is done reading stage s
-    if (t == 0 && q + STAGES < n_tiles) {
-      if (MODE != MV_DIGEST) bulk_wait_read<0>();          // the store that reads stage s has drained it
-      u8 *ngs, *ngd; bool nskip; addr(q + STAGES, ngs, ngd, nskip);
-      mbar_expect_tx(&full[s], TILE);
-      bulk_g2s(smem + s * TILE, ngs, TILE, &full[s]);
+      for (u32 j = 0; j < VT; ++j) h = fold(h, sv[j * LANES]);
+      asm volatile("" :: "l"(h) : "memory");               // the fold consumed the tile: its shared loads have completed
+      __syncwarp();
+      if ((t & 31) == 0) mbar_arrive(&empty[s]);           // this warp releases the stage
+      if (tile == tpp - 1) {
+        bool skip = false;
+        const u32 u = blockIdx.x + k * gridDim.x;
+        if (MODE != MV_DIGEST) skip = __ldg(phys + u / G) == SKIP;
+        const u64 sum = warp_sum64(mixL(h));
+        if ((t & 31) == 0 && !skip) part[(u64)u * WPC + warp] = sum;
+      }
     }
   }
-  if (MODE != MV_DIGEST && t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // Per-block digest from the warp partial sums: page_digest(g) = sum of its 8 partials,
