@@ -335,6 +335,13 @@ def main():
                 "traffic": a.traffic, "peak_source": peak_src, "launches": launches,
                 "avg_launch_ms": ms_k / launches, "algorithmic_bytes_per_launch": per_launch}
 
+    if a.traffic is None:      # dram__bytes_read+write of the gather kernel from the committed ncu capture, scaled per block
+        try:
+            with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+                tj = json.load(f)
+            a.traffic = (tj["dram_bytes_read"] + tj["dram_bytes_write"]) / tj["launch_blocks"] * st["gather_blocks"] / max(1, st["gather_launches"])
+        except Exception:
+            a.traffic = None
     roofline = roof(st["ms_gather"], st["gather_launches"], st["gather_blocks"])
     if roofline:
         roofline["kernel"] = "k_move_hash%s<GATHER> (K2 gather+checksum)" % ("_tma" if mover != rc.MOVER_LDG else "")
