@@ -82,7 +82,7 @@ def host_ram_bytes():
 class Job:
     """One rank's workload: context, resident pool, pre-marshalled waves."""
 
-    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=4):
+    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=8):
         import torch
         from paper_2606_01387_b200 import rc
         self.torch, self.rc = torch, rc
@@ -242,6 +242,21 @@ def run_oracle(index, steps, warmup):
             "claims_per_s": claims / dt, "seconds": dt, "steps": steps}
 
 
+def reduce_scalar(dist, x, op, device="cuda"):
+    """Cross-rank reduction of one number (the only collective of the multi-GPU run): max for times, sum for units."""
+    if dist is None:
+        return x
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def shard_claims(items, rank, world):
+    """Claim sharding for one shared workload: claims are independent, rank r takes items r, r+world, ..."""
+    return list(items[rank::world])
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -253,7 +268,7 @@ def main():
     ap.add_argument("--mover", default="auto", choices=["auto", "ldg", "tma"])
     ap.add_argument("--grid", type=int, default=0)
     ap.add_argument("--serial", action="store_true", help="one wave at a time: offload, then restore (no duplex overlap)")
-    ap.add_argument("--wave-frac", type=int, default=4, help="pipelined schedule: a wave uses 1/N of the pool (N >= 2)")
+    ap.add_argument("--wave-frac", type=int, default=8, help="pipelined schedule: a wave uses 1/N of the pool (N >= 2)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per gather launch (profiles/), if known")
@@ -305,20 +320,13 @@ def main():
         ms2, _, st2 = time_steps(job, a.steps, min(a.warmup, 1), True, dist)
         e2e = (ms2, st2)
 
-    def allred(x, op):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=op)
-        return float(t.item())
-
-    ms_max = allred(ms, dist.ReduceOp.MAX if dist else None)
-    payload_all = allred(float(payload), dist.ReduceOp.SUM if dist else None)
-    claims_all = allred(float(claims), dist.ReduceOp.SUM if dist else None)
-    launches_all = allred(float(st["kernel_launches"]), dist.ReduceOp.SUM if dist else None)
+    ms_max = reduce_scalar(dist, ms, "max")
+    payload_all = reduce_scalar(dist, float(payload), "sum")
+    claims_all = reduce_scalar(dist, float(claims), "sum")
+    launches_all = reduce_scalar(dist, float(st["kernel_launches"]), "sum")
     if e2e:
-        ms2_max = allred(e2e[0], dist.ReduceOp.MAX if dist else None)
-        pay2_all = allred(float(e2e[1]["bytes_d2h"] + e2e[1]["bytes_h2d"]), dist.ReduceOp.SUM if dist else None)
+        ms2_max = reduce_scalar(dist, e2e[0], "max")
+        pay2_all = reduce_scalar(dist, float(e2e[1]["bytes_d2h"] + e2e[1]["bytes_h2d"]), "sum")
     if rank != 0:
         dist.destroy_process_group()
         return
