@@ -24,7 +24,10 @@
  * every later call returns RC_ERR_CUDA.  A call-level error (negative return) emits
  * no event and changes no claim.  There is no CPU fallback anywhere behind this
  * interface: every step of the path runs in the library's sm_100a kernels and its
- * copy-engine transfers.
+ * copy-engine transfers.  Stream order: the library's streams are not ordered against
+ * the caller's; writes the caller makes to pool_dev / fill_dev must have completed
+ * (stream or device synchronise) before a call that reads them, and the library's
+ * writes are complete when a synchronous call or rc_wait returns.
  */
 #ifndef RC_H_
 #define RC_H_

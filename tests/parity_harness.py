@@ -41,6 +41,7 @@ class Pair:
         self.fill_h[ids] = vals
         self.fill_t[torch.from_numpy(np.asarray(ids).astype(np.int64)).cuda()] = torch.from_numpy(
             np.asarray(vals, np.uint8)).cuda()
+        torch.cuda.synchronize()
 
     def poison_free(self):
         used, _ = self.o.pool_state()
@@ -48,6 +49,7 @@ class Pair:
         self.view_h[:, free, :] = W.POISON
         if free.size:
             self.view_t[:, torch.from_numpy(free.astype(np.int64)).cuda(), :] = W.POISON
+            torch.cuda.synchronize()          # torch's stream is not ordered against the library's non-blocking streams
 
     def logical(self, cid):
         """Claim-logical KV [block][page g][bytes] read with torch indexing (not with librc)."""

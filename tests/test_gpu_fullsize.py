@@ -72,6 +72,7 @@ def test_config1_full_size_bench_configuration():
         used, _ = r.pool_state()
         free = torch.from_numpy(np.nonzero(used == 0)[0].astype(np.int64)).to(dev)
         view[:, free, :] = W.POISON                                                               # restore must read the host copy
+        torch.cuda.synchronize()              # torch's stream is not ordered against the library's non-blocking streams
         assert r.set_faults([(c.claim_id,) + c.fault for c in cl if c.fault]) == 0
         r.restore_begin(ids)
         if nxt:
