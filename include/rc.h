@@ -186,6 +186,28 @@ int rc_measure_link(rc_ctx* ctx, uint64_t bytes, int direction, int reps, double
  * a HOST array (may be NULL); ms (may be NULL) receives the device time of the digest kernel. */
 int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64_t* digests, float* ms);
 
+/* NEXT-1: the paper's artifact analyzer as a device pass.  Validates an event
+ * array (HOST, n records in stream order; may contain the harness marker codes RC_EV_USE and
+ * RC_EV_REQUEST_FINISHED) against the per-claim language
+ *   ACCEPTED MATERIALIZED ( OFFLOADED RESTORE_REQUIRED ( RESTORED USE* | LOAD_FAILED RESTORATION_FAILED REFUSED ) )*
+ * (any prefix valid; only REQUEST_FINISHED may follow REFUSED; REQUEST_FINISHED also ends ACCEPTED /
+ * MATERIALIZED / RESTORED), seq strictly increasing, no event with claim id 0, REFUSED carrying [C].
+ * report->ok = 1 iff the whole stream is accepted; first_bad_index = stream position of the first
+ * violation (UINT64_MAX if none).  claims (HOST, may be NULL) receives up to cap per-claim records in
+ * unspecified order: final automaton state, gate bits (RC_GATE_FAILURE: the claim's subsequence ends with
+ * the seven steps of P:L27; RC_GATE_OBSERVATION: path A; both 0 unless the stream is valid),
+ * its first violating position.  Needs no context; allocates and frees its own device memory. */
+enum { RC_EV_USE = 100, RC_EV_REQUEST_FINISHED = 101 };
+enum { RC_GATE_FAILURE = 1, RC_GATE_OBSERVATION = 2 };
+typedef struct rc_trace_claim { uint64_t claim_id; uint64_t first_bad; uint32_t state; uint32_t gates; uint32_t n_events; uint32_t pad; } rc_trace_claim;
+typedef struct rc_trace_report {
+  uint64_t first_bad_index, n_events, n_claims, n_failure_gate, n_observation_gate;
+  uint32_t ok, pad;
+  float ms_kernels;       /* device time of the four validator kernels */
+  float ms_total;         /* including the H2D of the events and the D2H of the records */
+} rc_trace_report;
+int rc_validate_trace(const rc_event* events, uint64_t n, rc_trace_report* report, rc_trace_claim* claims, uint64_t cap);
+
 const char* rc_strerror(int err);
 const char* rc_last_cuda_error(rc_ctx* ctx);
 

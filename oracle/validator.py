@@ -104,3 +104,23 @@ def observation_gate(events, cid):
     codes = [c for c in codes_of(events, cid) if c not in (USE, REQUEST_FINISHED)]
     return bool(ok and len(codes) >= 5 and codes[:2] == SUCCESS_ORDER[:2] and codes[-3:] == SUCCESS_ORDER[-3:]
                 and LOAD_FAILED not in codes and REFUSED not in codes)
+
+
+def validate_index(events):
+    """validate() with the stream position of the first violation: (True, -1) or (False, index).
+    Same loop as validate(); the position is where that loop stops."""
+    state = {}
+    last_seq = None
+    for i, (seq, cid, code, aux, arg) in enumerate(_rows(events)):
+        if last_seq is not None and seq <= last_seq:
+            return False, i
+        last_seq = seq
+        if cid == 0:
+            return False, i
+        nxt = _NEXT.get((state.get(cid, _S0), code))
+        if nxt is None:
+            return False, i
+        if code == REFUSED and (arg != cid or aux != 1):
+            return False, i
+        state[cid] = nxt
+    return True, -1

@@ -12,6 +12,7 @@
 // while every observable result equals the synchronous calls in _begin order.
 #include "../../include/rc.h"
 #include "rc_kernels.cuh"
+#include "rc_trace.cuh"
 
 #include <algorithm>
 #include <cstdio>
@@ -1035,6 +1036,69 @@ extern "C" int rc_digest_blocks(rc_ctx* c, const void* src, uint32_t n_blocks, u
   c->ev_pool.push_back(t0); c->ev_pool.push_back(t1);
   if (ms_out) *ms_out = total;
   return RC_OK;
+}
+
+// ---- NEXT-1: trace validator ----------------------------------------------------------------------------------------
+extern "C" int rc_validate_trace(const rc_event* events, uint64_t n, rc_trace_report* rep, rc_trace_claim* claims, uint64_t cap) {
+  using namespace rct;
+  if (!rep || (n && !events) || n > 0xFFFFFFF0ull) return RC_ERR_INVALID;
+  memset(rep, 0, sizeof(*rep));
+  rep->first_bad_index = NO_BAD; rep->n_events = n; rep->ok = 1;
+  if (n == 0) return RC_OK;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return RC_ERR_CUDA;
+  u32 slots = 1024;
+  while ((u64)slots < 2 * n) slots <<= 1;
+  Event* d_ev = nullptr; u64* d_keys = nullptr; u32 *d_count = nullptr, *d_base = nullptr, *d_dense = nullptr, *d_fill = nullptr;
+  u32 *d_slot = nullptr, *d_bucket = nullptr, *d_cur = nullptr; unsigned long long* d_bad = nullptr; ClaimOut* d_out = nullptr;
+  cudaStream_t st = nullptr; cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr, e3 = nullptr;
+  int rc = RC_OK;
+  std::vector<ClaimOut> host_out;
+#define TV(call) do { if ((call) != cudaSuccess) { rc = RC_ERR_CUDA; goto done; } } while (0)
+  TV(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+  TV(cudaEventCreate(&e0)); TV(cudaEventCreate(&e1)); TV(cudaEventCreate(&e2)); TV(cudaEventCreate(&e3));
+  TV(cudaMalloc(&d_ev, n * sizeof(Event))); TV(cudaMalloc(&d_keys, (u64)slots * 8)); TV(cudaMalloc(&d_count, (u64)slots * 4));
+  TV(cudaMalloc(&d_base, (u64)slots * 4)); TV(cudaMalloc(&d_dense, (u64)slots * 4)); TV(cudaMalloc(&d_fill, (u64)slots * 4));
+  TV(cudaMalloc(&d_slot, n * 4)); TV(cudaMalloc(&d_bucket, n * 4)); TV(cudaMalloc(&d_cur, 8)); TV(cudaMalloc(&d_bad, 8));
+  TV(cudaMalloc(&d_out, n * sizeof(ClaimOut)));
+  TV(cudaEventRecord(e0, st));
+  TV(cudaMemcpyAsync(d_ev, events, n * sizeof(Event), cudaMemcpyHostToDevice, st));
+  TV(cudaMemsetAsync(d_keys, 0, (u64)slots * 8, st)); TV(cudaMemsetAsync(d_count, 0, (u64)slots * 4, st));
+  TV(cudaMemsetAsync(d_fill, 0, (u64)slots * 4, st)); TV(cudaMemsetAsync(d_cur, 0, 8, st));
+  TV(cudaMemsetAsync(d_bad, 0xFF, 8, st));
+  TV(cudaEventRecord(e1, st));
+  tv_insert<<<(u32)((n + 255) / 256), 256, 0, st>>>((const Event*)d_ev, n, d_keys, d_count, slots - 1, d_slot, d_bad);
+  tv_alloc<<<(slots + 255) / 256, 256, 0, st>>>(d_count, slots, d_base, d_dense, d_cur);
+  tv_scatter<<<(u32)((n + 255) / 256), 256, 0, st>>>(n, d_slot, d_base, d_fill, d_bucket);
+  tv_walk<<<(slots + 127) / 128, 128, 0, st>>>((const Event*)d_ev, d_keys, d_count, slots, d_base, d_dense, d_bucket, d_out, d_bad);
+  TV(cudaGetLastError());
+  TV(cudaEventRecord(e2, st));
+  {
+    u32 cur[2]; unsigned long long bad;
+    TV(cudaMemcpyAsync(cur, d_cur, 8, cudaMemcpyDeviceToHost, st));
+    TV(cudaMemcpyAsync(&bad, d_bad, 8, cudaMemcpyDeviceToHost, st));
+    TV(cudaStreamSynchronize(st));
+    rep->n_claims = cur[1]; rep->first_bad_index = bad; rep->ok = bad == NO_BAD;
+    host_out.resize(cur[1]);
+    if (cur[1]) TV(cudaMemcpyAsync(host_out.data(), d_out, (u64)cur[1] * sizeof(ClaimOut), cudaMemcpyDeviceToHost, st));
+    TV(cudaEventRecord(e3, st));
+    TV(cudaStreamSynchronize(st));
+    for (u64 k = 0; k < host_out.size(); ++k) {
+      if (!rep->ok) host_out[k].gates = 0;                // the gates presuppose a valid stream
+      rep->n_failure_gate += (host_out[k].gates & G_FAILURE) != 0;
+      rep->n_observation_gate += (host_out[k].gates & G_OBSERVATION) != 0;
+      if (claims && k < cap) memcpy(&claims[k], &host_out[k], sizeof(ClaimOut));
+    }
+    TV(cudaEventElapsedTime(&rep->ms_kernels, e1, e2));
+    TV(cudaEventElapsedTime(&rep->ms_total, e0, e3));
+  }
+done:
+#undef TV
+  cudaFree(d_ev); cudaFree(d_keys); cudaFree(d_count); cudaFree(d_base); cudaFree(d_dense); cudaFree(d_fill);
+  cudaFree(d_slot); cudaFree(d_bucket); cudaFree(d_cur); cudaFree(d_bad); cudaFree(d_out);
+  if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); if (e2) cudaEventDestroy(e2); if (e3) cudaEventDestroy(e3);
+  if (st) cudaStreamDestroy(st);
+  return rc;
 }
 
 extern "C" const char* rc_strerror(int err) {

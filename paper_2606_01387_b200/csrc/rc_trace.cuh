@@ -1,0 +1,131 @@
+// rc_trace.cuh -- NEXT-1: the paper's artifact analyzer ("supplies no runtime
+// behavior; it only checks order, claim match, and controls after the run") as a data-parallel pass over
+// an event array.  Events are grouped by claim with a device hash table (no global sort), every claim's
+// subsequence is replayed through the per-claim automaton of DESIGN.md "Validator" by one thread, and the
+// first violating stream position is a min-reduction.  Rules and passages:
+//   seq strictly increasing; an event naming no claim (id 0) is invalid;
+//   nothing names a claim before its ACCEPTED;
+//   USE(C) while C is offloaded / restore-required is invalid: restore-after-use;
+//   REQUEST_FINISHED(C) between LOAD_FAILED and REFUSED is invalid: outcome precedes terminal handling;
+//   LOAD_FAILED / RESTORATION_FAILED / REFUSED without RESTORE_REQUIRED(C) in the same cycle is invalid;
+//   REFUSED must carry blocking_claim_ids = [C] (aux 1, arg C).
+#pragma once
+#include "rc_kernels.cuh"
+
+namespace rct {
+using namespace rck;
+
+enum { S0 = 0, ACC, MAT, OFF, RREQ, LF, RF, REF, RES, FIN, BAD, NSTATE };
+enum { EV_USE = 100, EV_FIN = 101 };
+enum { G_FAILURE = 1, G_OBSERVATION = 2 };
+constexpr u64 NO_BAD = ~0ull;
+
+struct ClaimOut { u64 claim_id; u64 first_bad; u32 state; u32 gates; u32 n_events; u32 pad; };
+
+__device__ __forceinline__ int col_of(u32 code) { return code >= 1 && code <= 8 ? (int)code - 1 : (code == EV_USE ? 8 : (code == EV_FIN ? 9 : -1)); }
+
+// next-state table [state][column]; BAD = not in the accepted language
+__device__ __forceinline__ u32 next_state(u32 s, int col) {
+  // columns: 0 ACCEPTED 1 MATERIALIZED 2 OFFLOADED 3 RESTORE_REQUIRED 4 LOAD_FAILED 5 RESTORED 6 RESTORATION_FAILED 7 REFUSED 8 USE 9 FIN
+  switch (s) {
+    case S0:   return col == 0 ? ACC : BAD;
+    case ACC:  return col == 1 ? MAT : (col == 9 ? FIN : BAD);
+    case MAT:  return col == 2 ? OFF : (col == 8 ? MAT : (col == 9 ? FIN : BAD));
+    case OFF:  return col == 3 ? RREQ : BAD;
+    case RREQ: return col == 5 ? RES : (col == 4 ? LF : BAD);
+    case LF:   return col == 6 ? RF : BAD;
+    case RF:   return col == 7 ? REF : BAD;
+    case REF:  return col == 9 ? FIN : BAD;
+    case RES:  return col == 2 ? OFF : (col == 8 ? RES : (col == 9 ? FIN : BAD));
+    default:   return BAD;
+  }
+}
+
+__device__ __forceinline__ u64 hash64(u64 x) { return mixF(x); }
+
+// pass 1: stream-level checks, hash insert, per-slot event count
+__global__ void tv_insert(const Event* __restrict__ ev, u64 n, u64* __restrict__ keys, u32* __restrict__ count, u32 mask,
+                          u32* __restrict__ slot_of, unsigned long long* __restrict__ first_bad) {
+  const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Event e = ev[i];
+  if (i > 0 && e.seq <= ev[i - 1].seq) atomicMin(first_bad, (unsigned long long)i);
+  if (e.claim_id == 0) { atomicMin(first_bad, (unsigned long long)i); slot_of[i] = 0xFFFFFFFFu; return; }
+  u32 h = (u32)hash64(e.claim_id) & mask;
+  for (;;) {
+    const u64 k = keys[h];
+    if (k == e.claim_id) break;
+    if (k == 0) {
+      const u64 old = atomicCAS((unsigned long long*)&keys[h], 0ull, (unsigned long long)e.claim_id);
+      if (old == 0 || old == e.claim_id) break;
+    }
+    h = (h + 1) & mask;
+  }
+  slot_of[i] = h;
+  atomicAdd(&count[h], 1u);
+}
+
+// pass 2: bucket space and a dense claim index per occupied slot
+__global__ void tv_alloc(const u32* __restrict__ count, u32 slots, u32* __restrict__ base, u32* __restrict__ dense,
+                         u32* __restrict__ cursors /*[0] events, [1] claims*/) {
+  const u32 s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= slots || count[s] == 0) return;
+  base[s] = atomicAdd(&cursors[0], count[s]);
+  dense[s] = atomicAdd(&cursors[1], 1u);
+}
+
+// pass 3: event indices into their claim's bucket (arrival order is arbitrary; pass 4 orders them)
+__global__ void tv_scatter(u64 n, const u32* __restrict__ slot_of, const u32* __restrict__ base, u32* __restrict__ fill,
+                           u32* __restrict__ bucket) {
+  const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const u32 s = slot_of[i];
+  if (s == 0xFFFFFFFFu) return;
+  bucket[base[s] + atomicAdd(&fill[s], 1u)] = (u32)i;
+}
+
+// pass 4: one thread per claim: order its events by stream position, replay the automaton, derive the gates
+__global__ void tv_walk(const Event* __restrict__ ev, const u64* __restrict__ keys, const u32* __restrict__ count, u32 slots,
+                        const u32* __restrict__ base, const u32* __restrict__ dense, u32* __restrict__ bucket,
+                        ClaimOut* __restrict__ out, unsigned long long* __restrict__ first_bad) {
+  const u32 s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= slots) return;
+  const u32 c = count[s];
+  if (c == 0) return;
+  u32* b = bucket + base[s];
+  for (u32 i = 1; i < c; ++i) {                 // insertion sort: a claim has a handful of events
+    const u32 x = b[i];
+    u32 j = i;
+    while (j > 0 && b[j - 1] > x) { b[j] = b[j - 1]; --j; }
+    b[j] = x;
+  }
+  const u64 cid = keys[s];
+  u32 st = S0, n_codes = 0, c0 = 0, c1 = 0, tail = 0;   // tail: last five lifecycle codes, 4 bits each
+  bool saw_fail = false;
+  u64 bad = NO_BAD;
+  for (u32 i = 0; i < c; ++i) {
+    const Event e = ev[b[i]];
+    const int col = col_of(e.code);
+    u32 nx = col < 0 ? (u32)BAD : next_state(st, col);
+    if (nx != BAD && e.code == EV_ACTIVE_REQUEST_REFUSED && (e.arg != cid || e.aux != 1)) nx = BAD;
+    if (nx == BAD) { bad = b[i]; st = BAD; break; }
+    st = nx;
+    if (col < 8) {
+      if (n_codes == 0) c0 = e.code; else if (n_codes == 1) c1 = e.code;
+      tail = ((tail << 4) | e.code) & 0xFFFFFu;
+      ++n_codes;
+      saw_fail |= (e.code == EV_LOAD_FAILED || e.code == EV_ACTIVE_REQUEST_REFUSED);
+    }
+  }
+  u32 gates = 0;
+  if (bad == NO_BAD && c0 == EV_ACCEPTED && c1 == EV_MATERIALIZED) {
+    // failure gate: subsequence ends OFFLOADED RESTORE_REQUIRED LOAD_FAILED RESTORATION_FAILED REFUSED
+    if (n_codes >= 7 && tail == 0x34578u) gates |= G_FAILURE;
+    // observation gate: ends OFFLOADED RESTORE_REQUIRED RESTORED, no failure record names C
+    if (n_codes >= 5 && (tail & 0xFFFu) == 0x346u && !saw_fail) gates |= G_OBSERVATION;
+  }
+  if (bad != NO_BAD) atomicMin(first_bad, (unsigned long long)bad);
+  out[dense[s]] = ClaimOut{cid, bad, st, gates, c, 0};
+}
+
+}  // namespace rct

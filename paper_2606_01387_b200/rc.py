@@ -24,7 +24,7 @@ MOVER_AUTO, MOVER_LDG, MOVER_TMA = 0, 1, 2
 EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_accept", "rc_materialize", "rc_offload",
            "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_outcomes", "rc_set_faults",
            "rc_release", "rc_claim_info", "rc_claim_blocks", "rc_claim_digests", "rc_host_read", "rc_pool_state",
-           "rc_stats_get", "rc_stats_reset", "rc_measure_link", "rc_digest_blocks", "rc_strerror",
+           "rc_stats_get", "rc_stats_reset", "rc_measure_link", "rc_digest_blocks", "rc_validate_trace", "rc_strerror",
            "rc_last_cuda_error"]
 
 
@@ -53,6 +53,17 @@ class Stats(C.Structure):
                 ("ms_d2h", C.c_float), ("ms_h2d", C.c_float), ("gather_launches", C.c_uint64),
                 ("scatter_launches", C.c_uint64), ("gather_blocks", C.c_uint64), ("scatter_blocks", C.c_uint64)]
 
+
+class TraceReport(C.Structure):
+    _fields_ = [("first_bad_index", C.c_uint64), ("n_events", C.c_uint64), ("n_claims", C.c_uint64),
+                ("n_failure_gate", C.c_uint64), ("n_observation_gate", C.c_uint64), ("ok", C.c_uint32), ("pad", C.c_uint32),
+                ("ms_kernels", C.c_float), ("ms_total", C.c_float)]
+
+
+TRACE_CLAIM_DTYPE = np.dtype([("claim_id", "<u8"), ("first_bad", "<u8"), ("state", "<u4"), ("gates", "<u4"),
+                              ("n_events", "<u4"), ("pad", "<u4")])
+GATE_FAILURE, GATE_OBSERVATION = 1, 2
+NO_BAD = (1 << 64) - 1
 
 _lib = None
 
@@ -248,3 +259,16 @@ class RC:
         self._ck(self.L.rc_digest_blocks(self.h, C.c_void_p(src_ptr), n_blocks, _p(d) if want else None, C.byref(ms)),
                  "rc_digest_blocks")
         return d, ms.value
+
+
+def validate_trace(events, want_claims=True):
+    """rc_validate_trace over a numpy record array (EVENT_DTYPE).  Returns (report dict, per-claim records)."""
+    ev = np.ascontiguousarray(events, dtype=EVENT_DTYPE)
+    rep = TraceReport()
+    cap = ev.size if want_claims else 0
+    claims = np.zeros(max(1, cap), TRACE_CLAIM_DTYPE)
+    rc = lib().rc_validate_trace(_p(ev), C.c_uint64(ev.size), C.byref(rep), _p(claims) if want_claims else None, C.c_uint64(cap))
+    if rc != 0:
+        raise RcError(rc, "rc_validate_trace")
+    out = {k: getattr(rep, k) for k, _ in TraceReport._fields_ if k != "pad"}
+    return out, claims[: min(cap, rep.n_claims)].copy()

@@ -253,3 +253,117 @@ def pool_torch(geom, device, seed=None):
 
 
 POISON = 0xA5   # byte written over freed blocks between offload and restore (DESIGN R5)
+
+
+# ---- synthetic event traces (inputs of the trace validator, NEXT-1) -----------------------------------
+TRACE_DTYPE = np.dtype([("seq", "<u8"), ("claim_id", "<u8"), ("code", "<u4"), ("aux", "<u4"), ("arg", "<u8")])
+T_USE, T_FIN = 100, 101
+TRACE_MUTATIONS = ["wrong_claim", "unclaimed", "restore_after_use", "finish_before_refused", "drop_restore_required",
+                   "swap_adjacent", "bad_blocking_ids", "seq_not_increasing", "generic_failure", "fallback_recompute"]
+
+
+def make_trace(n_claims, seed=0, fail_frac=0.1, cycles=(1, 3), markers=True):
+    """A valid interleaved stream: each claim runs ACCEPTED, MATERIALIZED, then 1..3 offload/restore cycles;
+    a fraction end in the failure path (the seven steps of P:L27); optional USE / REQUEST_FINISHED markers.
+    Events of different claims are interleaved at random, per-claim order kept.  Vectorised (10^6 claims ok)."""
+    rng = np.random.default_rng(SEED0 + 5000 + seed)
+    ids = rng.integers(1, 1 << 62, n_claims, dtype=np.uint64) * np.uint64(2) + np.uint64(1)
+    ids = np.unique(ids)
+    rng.shuffle(ids)
+    n = ids.size
+    ncyc = rng.integers(cycles[0], cycles[1] + 1, n)
+    fail = rng.random(n) < fail_frac
+    use = (rng.random(n) < 0.3) & ~fail & markers
+    fin = (rng.random(n) < 0.3) & markers
+    cols = []                                              # per-claim code sequences as padded columns
+    L = 2 + 3 * cycles[1] + 2 + 2
+    seqs = np.zeros((n, L), np.uint32)
+    ln = np.zeros(n, np.int64)
+
+    def push(mask, code):
+        idx = np.nonzero(mask)[0]
+        seqs[idx, ln[idx]] = code
+        ln[idx] += 1
+    allm = np.ones(n, bool)
+    push(allm, 1); push(allm, 2)
+    for cyc in range(cycles[1]):
+        act = ncyc > cyc
+        last = ncyc == cyc + 1
+        push(act, 3); push(act, 4)
+        push(act & ~(last & fail), 6)
+        push(act & last & fail, 5); push(act & last & fail, 7); push(act & last & fail, 8)
+    push(use, T_USE)
+    push(fin, T_FIN)
+    total = int(ln.sum())
+    owner = np.repeat(np.arange(n), ln)
+    within = np.arange(total) - np.repeat(np.cumsum(ln) - ln, ln)
+    t = rng.random(total)
+    # per-claim sorted times keep the claim's own order
+    order_in = np.lexsort((t, owner))
+    t_sorted = np.empty(total)
+    t_sorted[np.arange(total)] = t[order_in]
+    glob = np.argsort(t_sorted, kind="stable")
+    ev = np.zeros(total, TRACE_DTYPE)
+    code = seqs[owner, within]
+    ev["claim_id"] = ids[owner][glob]
+    ev["code"] = code[glob]
+    ev["seq"] = np.arange(total, dtype=np.uint64) * np.uint64(3) + np.uint64(7)
+    ref = ev["code"] == 8
+    ev["aux"][ref] = 1
+    ev["arg"][ref] = ev["claim_id"][ref]
+    return ev
+
+
+def mutate_trace(ev, kind, seed=0):
+    """One control-class mutation applied to a valid stream; returns a new array."""
+    rng = np.random.default_rng(SEED0 + 6000 + seed)
+    ev = ev.copy()
+    code, cid = ev["code"], ev["claim_id"]
+
+    def pick(mask):
+        idx = np.nonzero(mask)[0]
+        return int(idx[rng.integers(0, idx.size)]) if idx.size else None
+
+    def insert(pos, c, code_):
+        rec = np.zeros(1, TRACE_DTYPE)
+        rec["claim_id"], rec["code"] = c, code_
+        out = np.concatenate([ev[:pos], rec, ev[pos:]])
+        out["seq"] = np.arange(out.size, dtype=np.uint64) + np.uint64(1)
+        return out
+    if kind == "wrong_claim":                    # a failure record attributed to another claim
+        i = pick(code == 5)
+        other = cid[pick(cid != cid[i])]
+        ev["claim_id"][i] = other
+    elif kind == "unclaimed":
+        ev["claim_id"][pick(code == 5)] = 0
+    elif kind == "restore_after_use":            # USE(C) while C is offloaded
+        i = pick(code == 3)
+        return insert(i + 1, cid[i], T_USE)
+    elif kind == "finish_before_refused":        # terminal handling before the outcome (P:L380)
+        i = pick(code == 5)
+        return insert(i + 1, cid[i], T_FIN)
+    elif kind == "drop_restore_required":
+        i = pick(code == 4)
+        return np.delete(ev, i)
+    elif kind == "swap_adjacent":                # two consecutive events of one claim exchanged
+        i = pick(code == 3)
+        j = i + 1 + int(np.nonzero(cid[i + 1:] == cid[i])[0][0])
+        tmp = ev[["code", "aux", "arg"]][i].copy()
+        for f in ("code", "aux", "arg"):
+            a, b = ev[f][i], ev[f][j]
+            ev[f][i], ev[f][j] = b, a
+    elif kind == "bad_blocking_ids":             # blocking_claim_ids smeared onto another claim (P:L269)
+        i = pick(code == 8)
+        ev["arg"][i] = cid[pick(cid != cid[i])]
+    elif kind == "seq_not_increasing":
+        i = int(rng.integers(1, ev.size))
+        ev["seq"][i] = ev["seq"][i - 1]
+    elif kind == "generic_failure":              # failure records for a claim that was never restore-required
+        i = pick(code == 2)
+        return insert(i + 1, cid[i], 5)
+    elif kind == "fallback_recompute":           # RESTORED after a failed load (P:L492)
+        i = pick(code == 7)
+        ev["code"][i] = 6
+    else:
+        raise ValueError(kind)
+    return ev

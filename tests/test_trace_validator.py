@@ -1,0 +1,90 @@
+"""NEXT-1: trace validator.  CPU part pins oracle.validator.validate_index and the trace generator;
+GPU part compares rc_validate_trace with the oracle on valid streams and on every control class
+(P:L463)."""
+import numpy as np
+import pytest
+
+from oracle import validator as V
+from paper_2606_01387_b200 import workloads as W
+
+
+def test_validate_index_is_the_first_position_whose_prefix_is_rejected():
+    ev = W.make_trace(60, 4)
+    assert V.validate_index(ev) == (True, -1) and V.validate(ev)[0]
+    for kind in W.TRACE_MUTATIONS:
+        m = W.mutate_trace(ev, kind, 1)
+        ok, i = V.validate_index(m)
+        assert not ok and not V.validate(m)[0], kind
+        assert V.validate(m[:i])[0] and not V.validate(m[: i + 1])[0], kind     # brute-force prefix property
+
+
+def test_generated_traces_keep_per_claim_order_and_carry_both_paths():
+    ev = W.make_trace(500, 9)
+    cids = np.unique(ev["claim_id"])
+    fails = sum(V.failure_outcome_gate(ev, int(c)) for c in cids[:40])
+    obs = sum(V.observation_gate(ev, int(c)) for c in cids[:40])
+    assert fails > 0 and obs > 0 and fails + obs <= 40
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", [0, 1])
+def test_gpu_validator_matches_oracle_on_valid_and_mutated_streams(seed):
+    from paper_2606_01387_b200 import rc
+    ev = W.make_trace(3000, seed)
+    rep, claims = rc.validate_trace(ev)
+    assert rep["ok"] == 1 and rep["first_bad_index"] == rc.NO_BAD and rep["n_events"] == ev.size
+    assert rep["n_claims"] == np.unique(ev["claim_id"]).size == claims.size
+    assert sorted(claims["claim_id"]) == sorted(np.unique(ev["claim_id"]))
+    assert int(claims["n_events"].sum()) == ev.size
+    for kind in W.TRACE_MUTATIONS:
+        for ms in range(3):
+            m = W.mutate_trace(ev, kind, 10 * seed + ms)
+            ok, i = V.validate_index(m)
+            rep, claims = rc.validate_trace(m)
+            assert (rep["ok"] == 1) == ok and not ok, kind
+            assert rep["first_bad_index"] == i, (kind, rep["first_bad_index"], i)
+            assert rep["n_failure_gate"] == 0 and rep["n_observation_gate"] == 0     # gates presuppose a valid stream
+
+
+@pytest.mark.gpu
+def test_gpu_validator_gates_per_claim_match_oracle():
+    from paper_2606_01387_b200 import rc
+    ev = W.make_trace(250, 7)
+    rep, claims = rc.validate_trace(ev)
+    nf = no = 0
+    for c in claims:
+        cid = int(c["claim_id"])
+        f, o = V.failure_outcome_gate(ev, cid), V.observation_gate(ev, cid)
+        assert bool(c["gates"] & rc.GATE_FAILURE) == f and bool(c["gates"] & rc.GATE_OBSERVATION) == o, hex(cid)
+        nf += f
+        no += o
+    assert rep["n_failure_gate"] == nf and rep["n_observation_gate"] == no and nf > 0 and no > 0
+
+
+@pytest.mark.gpu
+def test_gpu_validator_edge_cases_and_scale():
+    from paper_2606_01387_b200 import rc
+    rep, claims = rc.validate_trace(np.zeros(0, rc.EVENT_DTYPE))
+    assert rep["ok"] == 1 and rep["n_claims"] == 0
+    one = np.zeros(1, rc.EVENT_DTYPE)
+    one["claim_id"], one["code"] = 5, 2                   # MATERIALIZED before ACCEPTED: post-hoc naming
+    rep, _ = rc.validate_trace(one)
+    assert rep["ok"] == 0 and rep["first_bad_index"] == 0 and V.validate_index(one) == (False, 0)
+    big = W.make_trace(100000, 3)                         # ~0.9 M events: properties that hold at any size
+    rep, claims = rc.validate_trace(big)
+    assert rep["ok"] == 1 and rep["n_claims"] == np.unique(big["claim_id"]).size
+    n_ref = int((big["code"] == 8).sum())
+    assert rep["n_failure_gate"] == n_ref                 # every refused claim of a valid generated stream took path B
+    m = W.mutate_trace(big, "wrong_claim", 2)
+    rep, _ = rc.validate_trace(m, want_claims=False)
+    assert rep["ok"] == 0 and (False, rep["first_bad_index"]) == V.validate_index(m)
+
+
+def test_real_stream_from_the_oracle_run_validates_both_ways():
+    from conftest import build_tiny_oracle
+    o, wl, wave, pool, fill = build_tiny_oracle()
+    ids = [c.claim_id for c in wl.claims]
+    o.accept(ids, [c.P for c in wl.claims], [c.N for c in wl.claims], wave.bt_off, wave.bt_ids)
+    o.materialize(ids); o.offload(ids); o.set_faults(wave.faults); o.restore(ids)
+    ev = o.outcomes()
+    assert V.validate_index(ev) == (True, -1)
