@@ -219,3 +219,84 @@ def test_standalone_digest_matches_oracle():
     want = [rco.block_digest(xh[i * g.blk_bytes:(i + 1) * g.blk_bytes], 2 * g.layers) for i in range(20)]
     assert [int(v) for v in d] == want
     p.close()
+
+
+def test_host_store_fragmentation_ring_wrap_and_capacity():
+    """Host-store extents split across free holes (space is granted by byte count, not contiguity), event
+    ring wrap-around, RC_ERR_CAPACITY without side effects, release in every state."""
+    wl = W.make_workload(0)
+    g = wl.geom
+    wave = W.plan_waves(wl, 1 << 30)[0]
+    cl = wl.claims
+    ids = [c.claim_id for c in cl]
+    ok = [k for k in range(len(cl)) if k != 6]
+    nb = {c.claim_id: (c.M + g.block_size - 1) // g.block_size for c in cl}
+    host_blocks = sum(nb[ids[k]] for k in ok[:4]) + 3                     # room for four claims and a bit
+    p = Pair(wl, host_blocks * g.blk_bytes, chunk_blocks=13, max_events=24)
+    o, r = p.o, p.r
+    p.set_fill(wave.fill_ids, wave.fill_val)
+    for x in (o, r):
+        assert x.mark_used(wave.used_ids) == 0
+    args = (ids, [c.P for c in cl], [c.N for c in cl], wave.bt_off, wave.bt_ids)
+    assert np.array_equal(o.accept(*args), r.accept(*args))
+    assert np.array_equal(o.materialize(ids), r.materialize(ids))
+    ea = p.check_events("drain 1")                                        # 8 + 7 events: ring of 24 wraps below
+    a4 = [ids[k] for k in ok[:4]]
+    assert np.array_equal(o.offload(a4), r.offload(a4))
+    # free the 1st and 3rd slots, then offload a claim that only fits split across the two holes + tail
+    p.poison_free()
+    assert np.array_equal(o.restore([a4[0], a4[2]]), r.restore([a4[0], a4[2]]))
+    p.check_events("drain 2")
+    big = [ids[k] for k in ok[4:6]]
+    sa, sb = o.offload(big), r.offload(big)
+    assert np.array_equal(sa, sb) and sa[0] == 0
+    p.check_claims(ids, "fragmented offload", host=True)
+    p.poison_free()
+    q = [a4[1], a4[3]] + big
+    assert np.array_equal(o.restore(q), r.restore(q))
+    p.check_claims(ids, "fragmented restore")
+    p.check_pool_state("fragmented restore")
+    ev = p.check_events("drain 3")
+    assert int(ev["seq"][-1]) > 24                                        # the ring wrapped and stayed gap-free
+    # event capacity: with 13 records pending, 3 more restores (up to 12 records) do not fit a ring of 24:
+    # RC_ERR_CAPACITY, and nothing changes
+    more = [ids[k] for k in ok]
+    sa, sb = o.offload(more), r.offload(more)
+    assert np.array_equal(sa, sb) and list(sa).count(0) == 4
+    live = [c for c, s_ in zip(more, sa) if s_ == 0]
+    for _ in range(3):
+        assert np.array_equal(o.restore(live[:1]), r.restore(live[:1]))
+        assert np.array_equal(o.offload(live[:1]), r.offload(live[:1]))
+    rcode, st = r.restore(live[1:], check=False)
+    assert rcode == rc.ERR_CAPACITY
+    assert all(r.claim_info(c)["state"] == 3 for c in live)
+    p.check_pool_state("capacity error", bytes_too=False)
+    p.check_events("drain after capacity error")
+    more = live
+    # release in every state: ACCEPTED (claim 6), OFFLOADED, then restored ones
+    assert np.array_equal(o.restore(more[:3]), r.restore(more[:3]))
+    p.check_events("drain 4")
+    assert np.array_equal(o.release(ids + [ids[0]]), r.release(ids + [ids[0]]))
+    p.check_pool_state("release all", bytes_too=False)
+    assert r.stats()["host_used_bytes"] == 0 == o.stats()["host_used"]
+    p.close()
+
+
+def test_bitflip_positions_across_chunk_boundaries():
+    """The injected corruption lands in the first / last byte of the claim and on both sides of a staging
+    chunk boundary; LOAD_FAILED.aux is the block that holds the flipped byte (affected-block evidence)."""
+    wl = W.make_workload(0)
+    g = wl.geom
+    wave = W.plan_waves(wl, 1 << 30)[0]
+    cl = wl.claims
+    ids = [c.claim_id for c in cl]
+    blk = g.blk_bytes
+    nb0 = (cl[0].M + g.block_size - 1) // g.block_size
+    params = [0, nb0 * blk - 1, 7 * blk - 1, 7 * blk, 3 * blk + 12345]      # chunk = 7 blocks
+    for prm, k in zip(params, (0, 0, 0, 0, 1)):
+        p = Pair(wl, 1 << 30, chunk_blocks=7)
+        ev, st = p.run_wave(wave, faults=[(ids[k], W.FK_BITFLIP, prm)])
+        lf = [e for e in ev if int(e["code"]) == 5]
+        assert len(lf) == 1 and int(lf[0]["claim_id"]) == ids[k] and int(lf[0]["aux"]) == prm // blk
+        assert st[k] == rc.ST_RESTORE_FAILED and st.count(rc.ST_RESTORE_FAILED) == 1
+        p.close()
