@@ -410,6 +410,15 @@ def main():
                        "ms_per_step": ms2_max / a.steps,
                        "what": "same step through the C ABI with host arrays; fill[] sent from pinned host memory, "
                                "statuses and the event stream read back, inside the timed region"}
+    if world == 1 and not a.no_cpu_baseline:   # NEXT-1: device trace validator on a 200k-claim synthetic stream (not part of `value`)
+        tr = W.make_trace(200000, 1)
+        best = None
+        for _ in range(3):
+            rep, _c = rc.validate_trace(tr, want_claims=False)
+            best = rep if best is None or rep["ms_kernels"] < best["ms_kernels"] else best
+        line["trace_validator"] = {"events": int(tr.size), "claims": int(best["n_claims"]), "ok": int(best["ok"]),
+                                   "ms_kernels": best["ms_kernels"], "ms_with_copies": best["ms_total"],
+                                   "events_per_s_kernels": tr.size / (best["ms_kernels"] * 1e-3)}
     if world == 1 and not a.no_cpu_baseline:
         line["cpu_baseline"] = {k: v for k, v in run_oracle(a.config, 1, 0).items() if k in
                                 ("value", "unit", "cores", "kind", "sample", "claims_per_s", "seconds")}
