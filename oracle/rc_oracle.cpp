@@ -27,6 +27,7 @@
 #include <cstdlib>
 #include <vector>
 #include <map>
+#include <set>
 #include <algorithm>
 
 typedef uint64_t u64;
@@ -99,6 +100,7 @@ struct Claim {
   std::vector<u64> d;         // per-block digests recorded at offload
   u64 chain = 0;
   std::vector<u8> host;       // claim-scoped host copy (nb*blk bytes)
+  std::vector<u64> hkeys;     // dedup mode (NEXT-2): the claim's blocks as keys into the content-addressed store
 };
 
 struct Ctx {
@@ -112,6 +114,11 @@ struct Ctx {
   std::vector<Fault> faults; u32 fault_flags = 0;
   std::vector<Event> events; u64 drained = 0;
   u64 generic_failures = 0;
+  // NEXT-2: content-addressed host store keyed by block digest, so blocks shared between claims
+  // are held (and cross the link) once.  DESIGN.md "Dedup".
+  bool dedup = false;
+  std::map<u64, std::pair<std::vector<u8>, u32>> store;   // digest -> (blk bytes, references)
+  u64 link_d2h = 0, link_h2d = 0;                          // bytes that have to cross the host link, by definition
   void emit(u64 c, u32 code, u32 aux, u64 arg) {
     Event ev; ev.seq = events.size(); ev.claim_id = c; ev.code = code; ev.aux = aux; ev.arg = arg;
     events.push_back(ev);
@@ -166,6 +173,23 @@ static void drop_refs(Ctx* c, Claim& cl) {
   cl.bt.clear();
 }
 
+static std::vector<u8> host_bytes_of(Ctx* c, const Claim& cl) {     // the claim-logical host copy
+  if (!c->dedup) return cl.host;
+  std::vector<u8> out;
+  for (u64 k : cl.hkeys) { const auto& b = c->store[k].first; out.insert(out.end(), b.begin(), b.end()); }
+  return out;
+}
+static u64 host_size_of(Ctx* c, const Claim& cl) { return c->dedup ? (u64)cl.hkeys.size() * c->blk : (u64)cl.host.size(); }
+static void drop_host(Ctx* c, Claim& cl) {
+  if (c->dedup) {
+    for (u64 k : cl.hkeys) { auto it = c->store.find(k); if (--it->second.second == 0) { c->store.erase(it); c->host_used -= c->blk; } }
+    cl.hkeys.clear();
+  } else {
+    c->host_used -= cl.host.size();
+    std::vector<u8>().swap(cl.host);
+  }
+}
+
 // offload: P:L343-346 (E2-E5).  Host bytes = concatenation, block-major,
 // then page g = l*2+kv.  Never failed by injection (CPU->GPU only).
 static void do_offload_one(Ctx* c, u64 id, Claim& cl) {
@@ -177,7 +201,19 @@ static void do_offload_one(Ctx* c, u64 id, Claim& cl) {
   cl.d.resize(cl.nb);
   for (u32 i = 0; i < cl.nb; ++i) cl.d[i] = block_digest(cl.host.data() + (u64)i * c->blk, G, c->page);
   cl.chain = chain_of(id, cl.d.data(), cl.nb);
-  c->host_used += cl.host.size();
+  if (c->dedup) {                                         // keep one copy per distinct block content
+    for (u32 i = 0; i < cl.nb; ++i) {
+      auto it = c->store.find(cl.d[i]);
+      if (it != c->store.end()) { it->second.second++; continue; }
+      const u8* b = cl.host.data() + (u64)i * c->blk;
+      c->store[cl.d[i]] = std::make_pair(std::vector<u8>(b, b + c->blk), 1u);
+      c->host_used += c->blk; c->link_d2h += c->blk;
+    }
+    cl.hkeys = cl.d;
+    std::vector<u8>().swap(cl.host);
+  } else {
+    c->host_used += cl.host.size(); c->link_d2h += cl.host.size();
+  }
   drop_refs(c, cl);
   cl.state = CS_OFFLOADED;
   c->emit(id, EV_OFFLOADED, cl.nb, cl.chain);
@@ -233,6 +269,7 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st) {
     }
   }
   bool any_served = false;
+  std::set<u64> call_keys;
   for (u32 k = 0; k < n; ++k) {
     if (!served[k]) continue;
     any_served = true;
@@ -246,7 +283,10 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st) {
     if (flt.kind == FK_XFER_ERROR) {
       ok = false;                                       // nothing is written to the pool
     } else {
-      std::vector<u8> staged(cl.host);                  // host copy itself stays intact
+      std::vector<u8> staged = host_bytes_of(c, cl);    // host copy itself stays intact
+      if (c->dedup && flt.kind != FK_BITFLIP) {           // one transfer per distinct block of the call; a corrupted
+        for (u64 k : cl.hkeys) if (call_keys.insert(k).second) c->link_h2d += c->blk;   // copy is private to its claim
+      } else c->link_h2d += staged.size();
       if (flt.kind == FK_BITFLIP && !staged.empty()) staged[flt.param % staged.size()] ^= 0x01;
       std::vector<u64> d2(cl.nb);
       for (u32 i = 0; i < cl.nb; ++i) {
@@ -260,8 +300,7 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st) {
       for (u32 i = 0; i < cl.nb && !found; ++i) if (d2[i] != cl.d[i]) { bad = i; found = true; }
       ok = !found && chain_of(id, d2.data(), cl.nb) == cl.chain;
     }
-    c->host_used -= cl.host.size();
-    std::vector<u8>().swap(cl.host);
+    drop_host(c, cl);
     if (ok) {
       cl.state = CS_RESIDENT_AGAIN;
       c->emit(id, EV_RESTORED, cl.nb, cl.chain);
@@ -335,7 +374,7 @@ int rco_release(void* h, u32 n, const u64* id, int32_t* st) {
     auto it = c->claims.find(id[k]);
     if (it == c->claims.end()) { st[k] = ST_UNKNOWN_CLAIM; continue; }
     drop_refs(c, it->second);
-    c->host_used -= it->second.host.size();
+    drop_host(c, it->second);
     c->claims.erase(it); st[k] = ST_OK;
   }
   return E_OK;
@@ -358,7 +397,7 @@ int rco_claim_info(void* h, u64 id, ClaimInfo* o) {
   Ctx* c = (Ctx*)h; auto it = c->claims.find(id);
   if (it == c->claims.end()) return E_INVALID;
   const Claim& cl = it->second;
-  o->claim_id = id; o->chain = cl.chain; o->host_bytes = cl.host.size(); o->state = cl.state;
+  o->claim_id = id; o->chain = cl.chain; o->host_bytes = host_size_of(c, cl); o->state = cl.state;
   o->P = cl.P; o->N = cl.N; o->M = cl.M; o->nb = cl.nb; o->n_table = (u32)cl.bt.size();
   return E_OK;
 }
@@ -379,8 +418,9 @@ int rco_claim_digests(void* h, u64 id, u64* d, u32 cap, u32* n) {
 int rco_host_read(void* h, u64 id, void* dst, u64 cap, u64* bytes) {
   Ctx* c = (Ctx*)h; auto it = c->claims.find(id);
   if (it == c->claims.end()) return E_INVALID;
-  *bytes = it->second.host.size();
-  if (dst && cap >= *bytes && *bytes) memcpy(dst, it->second.host.data(), *bytes);
+  const std::vector<u8> hb = host_bytes_of(c, it->second);
+  *bytes = hb.size();
+  if (dst && cap >= *bytes && *bytes) memcpy(dst, hb.data(), *bytes);
   return E_OK;
 }
 int rco_pool_state(void* h, u8* used, u32* ref) {       // copies used[NB], ref[NB]
@@ -394,6 +434,12 @@ int rco_stats(void* h, u64* out4) {                     // host_used, n_claims, 
   out4[0] = c->host_used; out4[1] = c->claims.size(); out4[2] = c->events.size(); out4[3] = c->generic_failures;
   return E_OK;
 }
+int rco_set_dedup(void* h, int on) {                    // only while no claim holds host bytes
+  Ctx* c = (Ctx*)h;
+  if (c->host_used != 0) return E_INVALID;
+  c->dedup = on != 0; return E_OK;
+}
+int rco_link_bytes(void* h, u64* out2) { Ctx* c = (Ctx*)h; out2[0] = c->link_d2h; out2[1] = c->link_h2d; return E_OK; }
 // checksum primitives, exported so the pins can reach each one directly
 u64 rco_mixL(u64 x) { return mixL(x); }
 u64 rco_mixF(u64 x) { return mixF(x); }

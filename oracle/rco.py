@@ -201,6 +201,14 @@ class Oracle:
         self.L.rco_pool_state(self.h, _p(used), _p(ref))
         return used, ref
 
+    def set_dedup(self, on=True):
+        return self.L.rco_set_dedup(self.h, int(on))
+
+    def link_bytes(self):
+        o = np.zeros(2, np.uint64)
+        self.L.rco_link_bytes(self.h, _p(o))
+        return int(o[0]), int(o[1])
+
     def stats(self):
         o = np.zeros(4, np.uint64)
         self.L.rco_stats(self.h, _p(o))
