@@ -89,6 +89,9 @@ typedef struct rc_config {
   void*    stream_h2d;      /* restore: pinned host -> staging copies                                */
   uint32_t mover;           /* RC_MOVER_*                                                            */
   uint32_t grid_ctas;       /* CTAs of a gather / scatter launch; 0 = library default                */
+  uint32_t dedup;           /* NEXT-2: 1 = content-addressed host store keyed by block digest: a block shared
+                               between claims is held and crosses the link once       */
+  uint32_t pad_;
 } rc_config;
 
 typedef struct rc_claim_info_t {

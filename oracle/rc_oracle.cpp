@@ -221,12 +221,14 @@ static void do_offload_one(Ctx* c, u64 id, Claim& cl) {
 
 static void do_offload(Ctx* c, u32 n, const u64* ids, int32_t* st) {
   bool full = false;                                    // prefix rule (DESIGN R7)
+  u64 worst = c->host_used;                             // space is granted as if every block were new (dedup charges less)
   for (u32 k = 0; k < n; ++k) {
     auto it = c->claims.find(ids[k]);
     if (it == c->claims.end()) { st[k] = ST_UNKNOWN_CLAIM; continue; }
     Claim& cl = it->second;
     if (cl.state != CS_MATERIALIZED && cl.state != CS_RESIDENT_AGAIN) { st[k] = ST_BAD_STATE; continue; }
-    if (full || c->host_used + (u64)cl.nb * c->blk > c->host_cap) { full = true; st[k] = ST_NO_HOST_SPACE; continue; }
+    if (full || worst + (u64)cl.nb * c->blk > c->host_cap) { full = true; st[k] = ST_NO_HOST_SPACE; continue; }
+    worst += (u64)cl.nb * c->blk;
     do_offload_one(c, ids[k], cl);
     st[k] = ST_OK;
   }

@@ -82,6 +82,8 @@ struct Claim {
   u32 bt_off = 0, bt_len = 0;            // live table extent (bt_len == 0: no table)
   u32 dg_off = 0, dg_len = 0;            // recorded digests
   std::vector<std::pair<u64, u64>> host; // host-store extents in blk units
+  std::vector<u32> hslots;               // dedup mode: host-store slot of each block
+  std::vector<u64> hkeys;                // dedup mode: content key (digest) of each block
   bool busy = false;
 };
 
@@ -130,6 +132,11 @@ struct rc_ctx {
   bool poisoned = false;
   std::string cuda_err;
   int accept_ctas = 32;
+  // NEXT-2: content-addressed host store
+  bool dedup = false;
+  std::unordered_map<u64, std::pair<u32, u32>> store;    // digest -> (slot, references)
+  std::vector<u32> pending_free;                         // slots of an in-flight restore, recycled at its completion
+  u64* h_dig = nullptr; u32 *h_iw = nullptr, *h_ispos = nullptr, *d_iw = nullptr, *d_ispos = nullptr;
 };
 
 #define CK(call)                                                                      \
@@ -155,20 +162,20 @@ static cudaEvent_t get_event(rc_ctx* c) {
 
 // ---- data movers -----------------------------------------------------------------------------
 template <int MODE>
-static void launch_ldg(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
+static void launch_ldg(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items, const u32* iw, const u32* ispos) {
   const u32 pages = n_items * c->G;
   const u32 grid = std::min(pages, c->grid);
   const u32 vpt = c->vpp / LANES;
   if (vpt % 8 == 0)
-    k_move_hash<MODE, 8><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp);
+    k_move_hash<MODE, 8><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos);
   else if (vpt % 4 == 0)
-    k_move_hash<MODE, 4><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp);
+    k_move_hash<MODE, 4><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos);
   else
-    k_move_hash<MODE, 1><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp);
+    k_move_hash<MODE, 1><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos);
 }
 
 // (TILE, STAGES) variants of the TMA mover; RC_TMA_VARIANT=<index> overrides the default choice (tuning sweeps)
-typedef void (*tma_fn)(u8*, u8*, const u32*, u64*, u32, u32, u32, u32);
+typedef void (*tma_fn)(u8*, u8*, const u32*, u64*, u32, u32, u32, u32, const u32*, const u32*);
 struct TmaVariant { u32 tile, stages, ctas_per_sm; tma_fn fn[3]; };
 #define TMA_V(T, S, C) {T, S, C, {k_move_hash_tma<MV_GATHER, S, T>, k_move_hash_tma<MV_SCATTER, S, T>, k_move_hash_tma<MV_DIGEST, S, T>}}
 // Measured on B200 (profiles/r01_mover_sweep.md): about 96 KiB of bulk loads in flight per SM is the sweet
@@ -179,12 +186,13 @@ static const TmaVariant kTma[] = {TMA_V(4096, 4, 2), TMA_V(8192, 4, 2), TMA_V(81
 constexpr int kTmaN = sizeof(kTma) / sizeof(kTma[0]);
 
 template <int MODE>
-static void launch_move(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items) {
+static void launch_move(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items,
+                        const u32* iw = nullptr, const u32* ispos = nullptr) {
   if (c->mover == RC_MOVER_TMA) {
     const TmaVariant& v = kTma[c->tma_variant];
     const u32 grid = std::min(n_items * c->G, c->grid);
-    v.fn[MODE]<<<grid, TMA_THREADS, v.tile * v.stages, s>>>(c->pool, staging, phys, part, n_items, c->G, c->NB, (u32)c->page);
-  } else launch_ldg<MODE>(c, s, staging, phys, part, n_items);
+    v.fn[MODE]<<<grid, TMA_THREADS, v.tile * v.stages, s>>>(c->pool, staging, phys, part, n_items, c->G, c->NB, (u32)c->page, iw, ispos);
+  } else launch_ldg<MODE>(c, s, staging, phys, part, n_items, iw, ispos);
   c->st.kernel_launches++;
 }
 
@@ -197,7 +205,8 @@ extern "C" int rc_destroy(rc_ctx* c) {
   F(c->d_used); F(c->d_ref); F(c->d_bt); F(c->d_dg); F(c->d_ring); F(c->d_evcount); F(c->d_bitmaps); F(c->d_up);
   F(c->d_counters); F(c->d_alloc); F(c->d_flip);
   for (int i = 0; i < 3; ++i) { F(c->d_desc[i]); F(c->d_res[i]); F(c->d_off[i]); FH(c->h_desc[i]); FH(c->h_res[i]); }
-  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store);
+  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store); FH(c->h_dig); FH(c->h_iw); FH(c->h_ispos);
+  F(c->d_iw); F(c->d_ispos);
   for (int d = 0; d < 2; ++d) {
     F(c->d_phys[d]); F(c->d_dtmp[d]);
     for (auto p : c->staging[d]) F(p);
@@ -285,6 +294,14 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   CC(cudaHostAlloc(&c->h_up, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
   CC(cudaHostAlloc(&c->h_flip, dc * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
   CC(cudaHostAlloc(&c->h_counters, 16, cudaHostAllocDefault), RC_ERR_NOMEM);
+  c->dedup = cfg->dedup != 0;
+  if (c->dedup) {
+    CC(cudaHostAlloc(&c->h_dig, cap * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_iw, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_ispos, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_iw, cap * 4), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_ispos, cap * 4), RC_ERR_NOMEM);
+  }
   for (int d = 0; d < 2; ++d) {
     CC(cudaMalloc(&c->d_phys[d], cap * 4), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_dtmp[d], cap * 8), RC_ERR_NOMEM);
@@ -517,8 +534,12 @@ static int copy_chunk(rc_ctx* c, int dir, cudaStream_t s, u8* stg, u64 w0, u64 w
 
 extern "C" int rc_wait(rc_ctx* c, int which);
 // ---- a1-a4 offload ------------------------------------------------------------------------------------
+static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st);
+static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st);
+
 extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
   GUARD();
+  if (c->dedup) return offload_begin_dedup(c, n, id, st);
   Op& op = c->ops[0];
   if (op.active) return RC_ERR_BUSY;
   if (n == 0) return RC_OK;
@@ -593,7 +614,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     CK(cudaEventRecord(t1, c->gather));
     op.t_kernel.push_back({t0, t1});
     op.launches++;
-    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, m, c->G);
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, m, c->G, nullptr);
     CKL();
     c->st.kernel_launches++;
     CK(cudaEventRecord(c->ev_ready[0][slot], c->gather));
@@ -657,6 +678,7 @@ static int wait_offload(rc_ctx* c) {
 // ---- a5-a8 restore ---------------------------------------------------------------------------------------
 extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
   GUARD();
+  if (c->dedup) return restore_begin_dedup(c, n, id, st);
   Op& op = c->ops[1];
   if (op.active) return RC_ERR_BUSY;
   if (n == 0) return RC_OK;
@@ -771,7 +793,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     CK(cudaEventRecord(t1, c->scatter));
     op.t_kernel.push_back({t0, t1});
     op.launches++;
-    k_block_digest<<<warps_grid(m), 256, 0, c->scatter>>>(c->part[1][slot], c->d_phys[1] + w0, c->d_dtmp[1] + w0, m, c->G);
+    k_block_digest<<<warps_grid(m), 256, 0, c->scatter>>>(c->part[1][slot], c->d_phys[1] + w0, c->d_dtmp[1] + w0, m, c->G, nullptr);
     CKL();
     c->st.kernel_launches++;
     CK(cudaEventRecord(c->ev_free[1][slot], c->scatter));
@@ -818,6 +840,8 @@ static int wait_restore(rc_ctx* c) {
       op.status[k] = RC_ST_RESTORE_FAILED;
     }
   }
+  for (u32 sl : c->pending_free) c->host_alloc.release(sl, 1);
+  c->pending_free.clear();
   c->st.bytes_h2d += op.copy_bytes;
   c->st.scatter_launches += op.launches; c->st.scatter_blocks += op.blocks;
   return collect_times(c, op, c->st.ms_scatter, c->st.ms_h2d);
@@ -837,6 +861,8 @@ extern "C" int rc_restore(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st
   const int rc = rc_restore_begin(c, n, id, st);
   return rc ? rc : wait_restore(c);
 }
+
+#include "rc_dedup.inl"
 
 // ---- outcomes, faults, release -----------------------------------------------------------------------------
 extern "C" int rc_outcomes(rc_ctx* c, rc_event* buf, uint64_t cap, uint64_t* n_out) {
@@ -886,6 +912,7 @@ extern "C" int rc_release(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st
     if (cl.dg_len) c->dg_alloc.release(cl.dg_off, cl.dg_len);
     for (auto& e : cl.host) c->host_alloc.release(e.first, e.second);
     if (!cl.host.empty()) c->host_used -= (u64)cl.nb * c->blk;
+    if (!cl.hkeys.empty()) dedup_drop(c, cl, c->ops[1].active);
     c->claims.erase(it);
     st[k] = RC_ST_OK;
   }
@@ -906,7 +933,7 @@ extern "C" int rc_claim_info(rc_ctx* c, uint64_t id, rc_claim_info_t* o) {
   auto it = c->claims.find(id);
   if (it == c->claims.end() || !o) return RC_ERR_INVALID;
   const Claim& cl = it->second;
-  o->claim_id = id; o->chain = cl.chain; o->host_bytes = cl.host.empty() ? 0 : (u64)cl.nb * c->blk;
+  o->claim_id = id; o->chain = cl.chain; o->host_bytes = (cl.host.empty() && cl.hslots.empty()) ? 0 : (u64)cl.nb * c->blk;
   o->state = cl.state; o->P = cl.P; o->N = cl.N; o->M = cl.M; o->nb = cl.nb; o->n_table = cl.bt_len;
   return RC_OK;
 }
@@ -941,9 +968,10 @@ extern "C" int rc_host_read(rc_ctx* c, uint64_t id, void* dst, uint64_t cap, uin
   auto it = c->claims.find(id);
   if (it == c->claims.end() || !bytes) return RC_ERR_INVALID;
   const Claim& cl = it->second;
-  *bytes = cl.host.empty() ? 0 : (u64)cl.nb * c->blk;
+  *bytes = (cl.host.empty() && cl.hslots.empty()) ? 0 : (u64)cl.nb * c->blk;
   if (dst && cap >= *bytes && *bytes) {
     u8* o = (u8*)dst;
+    for (u32 sl : cl.hslots) { memcpy(o, c->h_store + (u64)sl * c->blk, c->blk); o += c->blk; }
     for (auto& e : cl.host) { memcpy(o, c->h_store + e.first * c->blk, e.second * c->blk); o += e.second * c->blk; }
   }
   return RC_OK;
@@ -1022,7 +1050,7 @@ extern "C" int rc_digest_blocks(rc_ctx* c, const void* src, uint32_t n_blocks, u
     launch_move<MV_DIGEST>(c, c->gather, (u8*)src + w0 * c->blk, nullptr, c->part[0][0], m);
     CKL();
     CK(cudaEventRecord(t1, c->gather));
-    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][0], nullptr, c->d_dtmp[0] + w0, m, c->G);
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][0], nullptr, c->d_dtmp[0] + w0, m, c->G, nullptr);
     CKL();
     CK(cudaStreamSynchronize(c->gather));
     float ms = 0;

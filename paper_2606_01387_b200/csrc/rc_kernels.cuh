@@ -104,16 +104,18 @@ enum { MV_GATHER = 0, MV_SCATTER = 1, MV_DIGEST = 2 };
 template <int MODE, int UNR>
 __global__ void __launch_bounds__(LANES)
 k_move_hash(uint4* __restrict__ pool, uint4* __restrict__ staging, const u32* __restrict__ phys,
-            u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 vpp) {
+            u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 vpp,
+            const u32* __restrict__ iw /*item -> work position (nullptr: identity)*/,
+            const u32* __restrict__ ispos /*item -> staged block (nullptr: identity; NEXT-2 shared staging)*/) {
   const u32 t = threadIdx.x;
   const u32 n_pages = n_items * G;
   const u32 vpt = vpp / LANES;
   for (u32 u = blockIdx.x; u < n_pages; u += gridDim.x) {
     const u32 w = u / G, g = u - w * G;
     u32 b = 0;
-    if (MODE != MV_DIGEST) { b = __ldg(phys + w); if (b == SKIP) continue; }
+    if (MODE != MV_DIGEST) { b = __ldg(phys + (iw ? __ldg(iw + w) : w)); if (b == SKIP) continue; }
     uint4* pp = pool + ((u64)g * NB + b) * vpp + t;
-    uint4* sp = staging + (u64)u * vpp + t;
+    uint4* sp = staging + (ispos ? ((u64)__ldg(ispos + w) * G + g) : (u64)u) * vpp + t;
     const uint4* src = (MODE == MV_GATHER) ? pp : sp;
     uint4* dst = (MODE == MV_GATHER) ? sp : pp;
     u64 h = (u64)(t + 1) * C1;
@@ -182,7 +184,8 @@ constexpr int TMA_THREADS = LANES + 64;
 template <int MODE, int STAGES, int TILE>
 __global__ void __launch_bounds__(TMA_THREADS)
 k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __restrict__ phys,
-                u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 page_bytes) {
+                u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 page_bytes,
+                const u32* __restrict__ iw, const u32* __restrict__ ispos) {
   extern __shared__ __align__(128) u8 smem[];
   __shared__ __align__(8) u64 full[STAGES];
   __shared__ __align__(8) u64 empty[STAGES];
@@ -204,9 +207,9 @@ k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __re
     const u32 w = u / G, g = u - w * G;
     u32 b = 0;
     skip = false;
-    if (MODE != MV_DIGEST) { b = __ldg(phys + w); skip = (b == SKIP); if (skip) b = 0; }
+    if (MODE != MV_DIGEST) { b = __ldg(phys + (iw ? __ldg(iw + w) : w)); skip = (b == SKIP); if (skip) b = 0; }
     u8* pp = pool + ((u64)g * NB + b) * page_bytes + (u64)tile * TILE;
-    u8* sp = staging + (u64)u * page_bytes + (u64)tile * TILE;
+    u8* sp = staging + (ispos ? ((u64)__ldg(ispos + w) * G + g) : (u64)u) * page_bytes + (u64)tile * TILE;
     gsrc = (MODE == MV_GATHER) ? pp : sp;
     gdst = (MODE == MV_GATHER) ? sp : pp;
   };
@@ -249,7 +252,7 @@ k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __re
       if (tile == tpp - 1) {
         bool skip = false;
         const u32 u = blockIdx.x + k * gridDim.x;
-        if (MODE != MV_DIGEST) skip = __ldg(phys + u / G) == SKIP;
+        if (MODE != MV_DIGEST) { const u32 w = u / G; skip = __ldg(phys + (iw ? __ldg(iw + w) : w)) == SKIP; }
         const u64 sum = warp_sum64(mixL(h));
         if ((t & 31) == 0 && !skip) part[(u64)u * WPC + warp] = sum;
       }
@@ -260,10 +263,11 @@ k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __re
 // Per-block digest from the warp partial sums: page_digest(g) = sum of its 8 partials,
 // d = mixF( sum_g mixL(page_digest(g) ^ (g+1)*C3) ).  One warp per work item.
 __global__ void k_block_digest(const u64* __restrict__ part, const u32* __restrict__ phys, u64* __restrict__ d_out,
-                               u32 n_items, u32 G) {
+                               u32 n_items, u32 G, const u32* __restrict__ iw) {
   const u32 w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (w >= n_items) return;
-  if (phys && __ldg(phys + w) == SKIP) { if (lane == 0) d_out[w] = 0; return; }
+  const u32 wo = iw ? __ldg(iw + w) : w;            // output (and phys) position of item w
+  if (phys && __ldg(phys + wo) == SKIP) { if (lane == 0) d_out[wo] = 0; return; }
   u64 s = 0;
   for (u32 g = lane; g < G; g += 32) {
     const u64* p = part + ((u64)w * G + g) * WPC;
@@ -273,7 +277,7 @@ __global__ void k_block_digest(const u64* __restrict__ part, const u32* __restri
     s += mixL(pd ^ ((u64)(g + 1) * C3));
   }
   s = warp_sum64(s);
-  if (lane == 0) d_out[w] = mixF(s);
+  if (lane == 0) d_out[wo] = mixF(s);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -14,11 +14,15 @@ from paper_2606_01387_b200 import rc, workloads as W
 
 class Pair:
     def __init__(self, wl, host_store_bytes, chunk_blocks=None, staging_chunks=2, mover=rc.MOVER_AUTO,
-                 grid_ctas=0, oracle_host_store_bytes=None, max_events=1 << 17, seed=None):
+                 grid_ctas=0, oracle_host_store_bytes=None, max_events=1 << 17, seed=None, dedup=False, copies=()):
         g = wl.geom
         self.wl, self.g = wl, g
         dev = torch.device("cuda:0")
         self.pool_t = W.pool_torch(g, dev, seed)
+        v = self.pool_t.view(2 * g.layers, g.pool_blocks, g.page_bytes)
+        for src, dst in copies:                            # identical content in different physical blocks
+            v[:, dst, :] = v[:, src, :]
+        torch.cuda.synchronize()
         self.pool_h = self.pool_t.cpu().numpy()
         self.fill_t = torch.zeros(g.pool_blocks, dtype=torch.uint8, device=dev)
         self.fill_h = np.zeros(g.pool_blocks, np.uint8)
@@ -28,7 +32,10 @@ class Pair:
         self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks,
                        self.pool_t, self.fill_t, host_store_bytes,
                        staging_chunk_bytes=(chunk_blocks * g.blk_bytes) if chunk_blocks else None,
-                       staging_chunks=staging_chunks, mover=mover, grid_ctas=grid_ctas, max_events=max_events)
+                       staging_chunks=staging_chunks, mover=mover, grid_ctas=grid_ctas, max_events=max_events, dedup=dedup)
+        if dedup:
+            assert self.o.set_dedup(True) == 0
+        self.dedup = dedup
         self.view_h = self.pool_h.reshape(2 * g.layers, g.pool_blocks, g.page_bytes)
         self.view_t = self.pool_t.view(2 * g.layers, g.pool_blocks, g.page_bytes)
 
@@ -129,6 +136,8 @@ class Pair:
         ev = self.check_events("wave")
         sa, sb = self.o.stats(), self.r.stats()
         assert sa["generic_failures"] == sb["generic_failures"] and sa["host_used"] == sb["host_used_bytes"]
+        assert self.o.link_bytes() == (sb["bytes_d2h"], sb["bytes_h2d"]), "link bytes: oracle %r, cuda %r" % (
+            self.o.link_bytes(), (sb["bytes_d2h"], sb["bytes_h2d"]))
         if release:
             sa, sb = self.o.release(ids), self.r.release(ids)
             assert np.array_equal(sa, sb)

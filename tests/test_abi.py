@@ -30,13 +30,13 @@ def test_no_cpu_fallback_without_a_device():
     import torch
     if torch.cuda.is_available():
         pytest.skip("a device is present")
-    cfg = rc.Config(2, 2, 64, 2, 16, 256, 64, 4096, 4096, 2, 1 << 20, 1 << 20, 256, 256, 0, 0, 0, 0, 0, 0, 0)
+    cfg = rc.Config(2, 2, 64, 2, 16, 256, 64, 4096, 4096, 2, 1 << 20, 1 << 20, 256, 256, 0, 0, 0, 0, 0, 0, 0, 0, 0)
     h = ctypes.c_void_p()
     assert rc.lib().rc_create(ctypes.byref(cfg), ctypes.byref(h)) == rc.ERR_CUDA and not h.value
 
 
 def test_rc_create_rejects_bad_geometry():
     h = ctypes.c_void_p()
-    cfg = rc.Config(2, 2, 64, 2, 3, 256, 64, 4096, 4096, 2, 1 << 20, 1 << 20, 256, 256, 0, 0, 0, 0, 0, 0, 0)  # page % 4096 != 0
+    cfg = rc.Config(2, 2, 64, 2, 3, 256, 64, 4096, 4096, 2, 1 << 20, 1 << 20, 256, 256, 0, 0, 0, 0, 0, 0, 0, 0, 0)  # page % 4096 != 0
     assert rc.lib().rc_create(ctypes.byref(cfg), ctypes.byref(h)) == rc.ERR_INVALID
     assert rc.lib().rc_strerror(rc.ERR_CAPACITY).decode().startswith("capacity")

@@ -300,3 +300,70 @@ def test_bitflip_positions_across_chunk_boundaries():
         assert len(lf) == 1 and int(lf[0]["claim_id"]) == ids[k] and int(lf[0]["aux"]) == prm // blk
         assert st[k] == rc.ST_RESTORE_FAILED and st.count(rc.ST_RESTORE_FAILED) == 1
         p.close()
+
+
+# ---- NEXT-2: content-addressed host store (dedup) ------------------------------------------------------
+@pytest.mark.parametrize("mover", [rc.MOVER_TMA, rc.MOVER_LDG])
+@pytest.mark.parametrize("chunk_blocks", [9, 64])
+def test_dedup_shared_tiny_full_parity(mover, chunk_blocks):
+    """Shared prefixes + identical content in different blocks: one held copy and one link transfer per
+    distinct block, everything else (bytes, digests, chains, events, allocation) as without dedup."""
+    wl, wave, copies = W.make_shared_tiny()
+    ids = [c.claim_id for c in wl.claims]
+    p = Pair(wl, 1 << 30, chunk_blocks=chunk_blocks, mover=mover, dedup=True, copies=copies)
+    g = wl.geom
+    wave.faults = [(ids[0], W.FK_BITFLIP, 5 * g.blk_bytes + 17), (ids[3], W.FK_XFER_ERROR, 0)]
+    ev, st = p.run_wave(wave, restore_batches=[ids[:3], ids[3:]])
+    assert st == [8, 0, 0, 8, 0, 0]                              # the shared block's corruption stays on claim 0 (P:L384)
+    s = p.r.stats()
+    total = sum((c.M + g.block_size - 1) // g.block_size for c in wl.claims) * g.blk_bytes
+    assert s["bytes_d2h"] < total - 20 * g.blk_bytes and s["bytes_h2d"] < total
+    ok, why = V.validate(ev)
+    assert ok, why
+    p.close()
+
+
+def test_dedup_config2_shared_prefixes_reduced():
+    wl = W.make_workload(2, n_claims=4, pool_blocks=1300)
+    host = 6 << 30
+    p = Pair(wl, host, chunk_blocks=50, dedup=True)
+    for wave in W.plan_waves(wl, host):
+        ids = [wl.claims[k].claim_id for k in wave.claim_idx]
+        ev, _ = p.run_wave(wave, restore_batches=[ids[i:i + 2] for i in range(0, len(ids), 2)])
+        ok, why = V.validate(ev)
+        assert ok, why
+    p.close()
+
+
+def test_dedup_overlapped_begin_wait_matches_synchronous_order():
+    """restore(k) in flight while offload(k+1) dedups against the store: the restore's reference drops
+    take effect at _begin, so the overlapped run equals the oracle's synchronous order."""
+    wl, wave, copies = W.make_shared_tiny()
+    ids = [c.claim_id for c in wl.claims]
+    p = Pair(wl, 1 << 30, chunk_blocks=11, dedup=True, copies=copies)
+    o, r = p.o, p.r
+    p.set_fill(wave.fill_ids, wave.fill_val)
+    for x in (o, r):
+        assert x.mark_used(wave.used_ids) == 0
+    args = (ids, [c.P for c in wl.claims], [c.N for c in wl.claims], wave.bt_off, wave.bt_ids)
+    assert np.array_equal(o.accept(*args), r.accept(*args))
+    assert np.array_equal(o.materialize(ids), r.materialize(ids))
+    a, b = ids[:3], ids[3:]
+    assert np.array_equal(o.offload(a), r.offload(a))
+    p.poison_free()
+    sa_r, sa_o = o.restore(a), o.offload(b)
+    r.restore_begin(a)
+    r.offload_begin(b)
+    sb_o, sb_r = r.wait(0), r.wait(1)
+    assert np.array_equal(sa_r, sb_r) and np.array_equal(sa_o, sb_o)
+    p.check_claims(ids, "overlap", host=True)
+    p.check_pool_state("overlap")
+    s = r.stats()
+    assert o.link_bytes() == (s["bytes_d2h"], s["bytes_h2d"]) and o.stats()["host_used"] == s["host_used_bytes"]
+    p.poison_free()
+    assert np.array_equal(o.restore(b), r.restore(b))
+    p.check_pool_state("final")
+    p.check_events("overlap")
+    assert np.array_equal(o.release(ids), r.release(ids))
+    assert r.stats()["host_used_bytes"] == 0
+    p.close()
