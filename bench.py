@@ -82,7 +82,7 @@ def host_ram_bytes():
 class Job:
     """One rank's workload: context, resident pool, pre-marshalled waves."""
 
-    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=8):
+    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=8, dedup=False):
         import torch
         from paper_2606_01387_b200 import rc
         self.torch, self.rc = torch, rc
@@ -114,9 +114,18 @@ class Job:
         self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, self.pool, self.fill,
                        self.host_store, staging_chunk_bytes=min(chunk_bytes, self.host_store), staging_chunks=2,
                        max_claims=max(1024, 2 * n_max), max_table_entries=max(4 * g.pool_blocks, 1 << 16),
-                       max_events=max(1 << 16, 16 * n_max), mover=mover, grid_ctas=grid_ctas)
+                       max_events=max(1 << 16, 16 * n_max), mover=mover, grid_ctas=grid_ctas, dedup=dedup)
         self.prep = []
-        for w in self.waves:
+        region = g.pool_blocks // wave_frac if pipelined else 0
+        for wi, w in enumerate(self.waves):
+            if pipelined:
+                # waves alternate between the two top regions of the pool; restored blocks (lowest free ids) land
+                # below them, so every wave reads pristine, pairwise distinct content (matters for --dedup: copies
+                # left behind by earlier restores must not masquerade as shared prefixes)
+                base = np.uint32(g.pool_blocks - (1 + wi % 2) * region)
+                w.bt_ids = w.bt_ids + base
+                w.used_ids = w.used_ids + base
+                w.fill_ids = w.fill_ids + base
             cl = [self.wl.claims[k] for k in w.claim_idx]
             ids = np.array([c.claim_id for c in cl], np.uint64)
             fid_h = torch.from_numpy(w.fill_ids.astype(np.int64)).pin_memory()
@@ -278,6 +287,7 @@ def main():
     ap.add_argument("--grid", type=int, default=0)
     ap.add_argument("--serial", action="store_true", help="one wave at a time: offload, then restore (no duplex overlap)")
     ap.add_argument("--wave-frac", type=int, default=8, help="pipelined schedule: a wave uses 1/N of the pool (N >= 2)")
+    ap.add_argument("--dedup", action="store_true", help="NEXT-2: content-addressed host store; value counts claim-logical bytes")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per gather launch (profiles/), if known")
@@ -312,7 +322,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2606_01387_b200 import rc
     mover = {"auto": rc.MOVER_AUTO, "ldg": rc.MOVER_LDG, "tma": rc.MOVER_TMA}[a.mover]
-    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac))
+    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac), dedup=a.dedup)
     g = job.g
     link = {}
     if world == 1:
@@ -323,6 +333,9 @@ def main():
     ms, wall_ms, st = time_steps(job, a.steps, a.warmup, False, dist)
     clocks = sampler.stop() if sampler else None
     payload = st["bytes_d2h"] + st["bytes_h2d"]
+    link_bytes = payload
+    if a.dedup:                # claim-logical bytes moved (what the claims hold), not the smaller number that crossed the link
+        payload = (st["gather_blocks"] + st["scatter_blocks"]) * job.g.blk_bytes
     claims = sum(p["n"] for p in job.prep) * a.steps
     e2e = None
     if not a.no_e2e:
@@ -399,6 +412,8 @@ def main():
                        "parallelism": "claims independent: one replica of the workload per GPU, no collective"},
             "claims_per_s": claims_all / (ms_max / 1e3), "payload_bytes_per_step": payload_all / a.steps,
             "wall_ms_per_step": wall_ms / a.steps, "clocks": clocks, "gpu_launches": int(launches_all),
+            "dedup": ({"link_bytes_per_step": link_bytes / a.steps, "logical_bytes_per_step": payload / a.steps,
+                       "link_over_logical": link_bytes / max(1, payload)} if a.dedup else None),
             "roofline": roofline, "roofline_scatter": roof_sc, "roofline_digest": roof_dg, "host_link": links}
     if links:
         links["value_over_duplex_ceiling"] = line["value"] / link["both"]
