@@ -82,10 +82,14 @@ static u64 chain_of(u64 claim_id, const u64* d, u32 nb) {
 // ---- codes (restated; the ABI header of the product is not included) --------
 enum { EV_ACCEPTED = 1, EV_MATERIALIZED = 2, EV_OFFLOADED = 3, EV_RESTORE_REQUIRED = 4,
        EV_LOAD_FAILED = 5, EV_RESTORED = 6, EV_RESTORATION_FAILED = 7,
-       EV_ACTIVE_REQUEST_REFUSED = 8 };
+       EV_ACTIVE_REQUEST_REFUSED = 8,
+       EV_DEMOTED = 9, EV_EXPIRED = 10 };   // NEXT-3: the other claim-scoped outcomes of a failed restoration (Table "offloadable")
+enum { POL_REFUSE = 0, POL_DEMOTE = 1, POL_EXPIRE = 2 };
+static const u32 REQ_FLAG = 0x80000000u;     // REFUSED.aux of a request-level refusal: flag | size of blocking_claim_ids
 enum { ST_OK = 0, ST_PRED_FALSE = 1, ST_UNKNOWN_CLAIM = 2, ST_BAD_STATE = 3, ST_DUPLICATE_ID = 4,
        ST_BAD_TABLE = 5, ST_NO_FREE_BLOCKS = 6, ST_NO_HOST_SPACE = 7, ST_RESTORE_FAILED = 8 };
-enum { CS_ACCEPTED = 1, CS_MATERIALIZED = 2, CS_OFFLOADED = 3, CS_RESIDENT_AGAIN = 4, CS_REFUSED = 5 };
+enum { CS_ACCEPTED = 1, CS_MATERIALIZED = 2, CS_OFFLOADED = 3, CS_RESIDENT_AGAIN = 4, CS_REFUSED = 5,
+       CS_DEMOTED = 6, CS_EXPIRED = 7 };
 enum { FK_XFER_ERROR = 1, FK_BITFLIP = 2 };
 enum { FF_ALLOW_UNCLAIMED = 1 };
 enum { E_OK = 0, E_INVALID = -1 };
@@ -95,7 +99,7 @@ struct Fault { u64 claim_id; u32 kind, param; };
 struct ClaimInfo { u64 claim_id, chain, host_bytes; u32 state, P, N, M, nb, n_table; };
 
 struct Claim {
-  u32 state = 0, P = 0, N = 0, M = 0, nb = 0;
+  u32 state = 0, P = 0, N = 0, M = 0, nb = 0, policy = 0;
   std::vector<u32> bt;        // current block table
   std::vector<u64> d;         // per-block digests recorded at offload
   u64 chain = 0;
@@ -244,7 +248,11 @@ static void do_offload(Ctx* c, u32 n, const u64* ids, int32_t* st) {
 //      entry whose id == C, one-shot; other ids have no effect: P:L25, P:L463,
 //      P:L493), write + re-digest + compare, verdict events;
 //   5. blocks of failed claims are freed after step 4 of that claim.
-static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st) {
+// request_id == 0: every claim is its own reuse request (blocking_claim_ids=[C]).  request_id != 0 (NEXT-3): the
+// batch is ONE reuse request naming several claims; its refusal is emitted once, after the per-claim records, as
+// one REFUSED record per failed claim (claim_id = the blocking claim, aux = REQ_FLAG | size of the failed subset,
+// arg = request id) -- blocking_claim_ids is exactly the failed subset ("smeared" ids fail closed).
+static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_id = 0) {
   u32 G = 2 * c->L;
   std::vector<Claim*> served(n, nullptr);
   u64 nfree = 0;
@@ -272,6 +280,7 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st) {
   }
   bool any_served = false;
   std::set<u64> call_keys;
+  std::vector<u64> blocking;
   for (u32 k = 0; k < n; ++k) {
     if (!served[k]) continue;
     any_served = true;
@@ -310,13 +319,17 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st) {
     } else {
       c->emit(id, EV_LOAD_FAILED, bad, 0);
       c->emit(id, EV_RESTORATION_FAILED, 0, 0);
-      c->emit(id, EV_ACTIVE_REQUEST_REFUSED, 1, id);    // blocking_claim_ids=[C]: aux = count, arg = C
+      if (cl.policy == POL_DEMOTE) c->emit(id, EV_DEMOTED, 0, 0);        // ordered responsibility boundary
+      else if (cl.policy == POL_EXPIRE) c->emit(id, EV_EXPIRED, 0, 0);
+      else if (request_id == 0) c->emit(id, EV_ACTIVE_REQUEST_REFUSED, 1, id);    // blocking_claim_ids=[C]: aux = count, arg = C
+      else blocking.push_back(id);
       for (u32 b : cl.bt) { c->used[b] = 0; c->ref[b] = 0; c->fill[b] = 0; }
       cl.bt.clear(); cl.d.clear();
-      cl.state = CS_REFUSED;                            // terminal
+      cl.state = cl.policy == POL_DEMOTE ? CS_DEMOTED : (cl.policy == POL_EXPIRE ? CS_EXPIRED : CS_REFUSED);   // terminal
       st[k] = ST_RESTORE_FAILED;
     }
   }
+  for (u64 b : blocking) c->emit(b, EV_ACTIVE_REQUEST_REFUSED, REQ_FLAG | (u32)blocking.size(), request_id);
   if (any_served && (c->fault_flags & FF_ALLOW_UNCLAIMED)) {   // P:L337; generic counter only
     for (size_t f = 0; f < c->faults.size();)
       if (c->faults[f].claim_id == 0) { c->generic_failures++; c->faults.erase(c->faults.begin() + f); }
@@ -370,6 +383,16 @@ int rco_materialize(void* h, u32 n, const u64* id, int32_t* st) {
 }
 int rco_offload(void* h, u32 n, const u64* id, int32_t* st) { do_offload((Ctx*)h, n, id, st); return E_OK; }
 int rco_restore(void* h, u32 n, const u64* id, int32_t* st) { do_restore((Ctx*)h, n, id, st); return E_OK; }
+int rco_restore_request(void* h, u64 request_id, u32 n, const u64* id, int32_t* st) {
+  if (request_id == 0) return E_INVALID;
+  do_restore((Ctx*)h, n, id, st, request_id); return E_OK;
+}
+int rco_set_policy(void* h, u32 n, const u64* id, const u32* policy) {   // what a failed restoration means for the claim
+  Ctx* c = (Ctx*)h;
+  for (u32 k = 0; k < n; ++k) if (!c->claims.count(id[k]) || policy[k] > POL_EXPIRE) return E_INVALID;
+  for (u32 k = 0; k < n; ++k) c->claims[id[k]].policy = policy[k];
+  return E_OK;
+}
 int rco_release(void* h, u32 n, const u64* id, int32_t* st) {
   Ctx* c = (Ctx*)h;
   for (u32 k = 0; k < n; ++k) {

@@ -16,7 +16,8 @@ EVENT_DTYPE = np.dtype([("seq", "<u8"), ("claim_id", "<u8"), ("code", "<u4"), ("
 FAULT_DTYPE = np.dtype([("claim_id", "<u8"), ("kind", "<u4"), ("param", "<u4")])
 
 EV_NAMES = {1: "ACCEPTED", 2: "MATERIALIZED", 3: "OFFLOADED", 4: "RESTORE_REQUIRED", 5: "LOAD_FAILED",
-            6: "RESTORED", 7: "RESTORATION_FAILED", 8: "ACTIVE_REQUEST_REFUSED"}
+            6: "RESTORED", 7: "RESTORATION_FAILED", 8: "ACTIVE_REQUEST_REFUSED", 9: "DEMOTED", 10: "EXPIRED"}
+REQ_FLAG = 0x80000000
 
 
 class _Cfg(C.Structure):
@@ -148,6 +149,17 @@ class Oracle:
 
     def restore(self, ids):
         return self._batch(self.L.rco_restore, ids)
+
+    def restore_request(self, request_id, ids):
+        ids = _u64(ids)
+        st = np.zeros(ids.size, np.int32)
+        rc = self.L.rco_restore_request(self.h, C.c_uint64(request_id), ids.size, _p(ids), _p(st))
+        assert rc == 0
+        return st
+
+    def set_policy(self, ids, policy):
+        ids, policy = _u64(ids), _u32(policy)
+        return self.L.rco_set_policy(self.h, ids.size, _p(ids), _p(policy))
 
     def release(self, ids):
         return self._batch(self.L.rco_release, ids)

@@ -23,10 +23,12 @@ Rules and the passages that fix them:
   * REFUSED.arg (blocking_claim_ids) must be [C], the refused claim itself.
 """
 ACCEPTED, MATERIALIZED, OFFLOADED, RESTORE_REQUIRED, LOAD_FAILED, RESTORED, RESTORATION_FAILED, REFUSED = range(1, 9)
+DEMOTED, EXPIRED = 9, 10          # NEXT-3: the other claim-scoped outcomes of a failed restoration (P:L105, P:L120)
 USE, REQUEST_FINISHED = 100, 101
+REQ_FLAG = 0x80000000             # REFUSED.aux of a request-level refusal: flag | size of blocking_claim_ids
 
 # per-claim automaton states
-_S0, _ACC, _MAT, _OFF, _RREQ, _LF, _RF, _REF, _RES, _FIN = range(10)
+_S0, _ACC, _MAT, _OFF, _RREQ, _LF, _RF, _REF, _RES, _FIN, _DEM, _EXP = range(12)
 
 _NEXT = {
     (_S0, ACCEPTED): _ACC,
@@ -38,9 +40,13 @@ _NEXT = {
     (_RREQ, LOAD_FAILED): _LF,
     (_LF, RESTORATION_FAILED): _RF,
     (_RF, REFUSED): _REF,
+    (_RF, DEMOTED): _DEM,
+    (_RF, EXPIRED): _EXP,
     (_MAT, USE): _MAT,
     (_RES, USE): _RES,
     (_REF, REQUEST_FINISHED): _FIN,
+    (_DEM, REQUEST_FINISHED): _FIN,
+    (_EXP, REQUEST_FINISHED): _FIN,
     (_ACC, REQUEST_FINISHED): _FIN,
     (_MAT, REQUEST_FINISHED): _FIN,
     (_RES, REQUEST_FINISHED): _FIN,
@@ -58,24 +64,56 @@ def _rows(events):
     return out
 
 
-def validate(events):
-    """Returns (ok, reason).  ok is True iff the whole stream is in the accepted language."""
+def _scan(events):
+    """The analyzer loop: (ok, index of the first violation or -1, reason).
+
+    Request-level refusals (NEXT-3; P:L87 blocking_claim_ids, "smear blocking ids across claims ...
+    fails closed"): a reuse request naming several claims is refused once, by a run of consecutive
+    REFUSED records with the same arg (request id) and aux = REQ_FLAG | k, one per blocking claim.  The run must
+    name exactly the k claims whose restoration failed and is still unanswered (state RF) -- neither a claim
+    that did not fail (the automaton rejects it) nor fewer than all that did (k must equal the pending count),
+    and nothing may interrupt the run."""
     state = {}
     last_seq = None
-    for seq, cid, code, aux, arg in _rows(events):
+    pending = 0                     # claims in state RF: failed, outcome not yet emitted
+    group = None                    # [arg, aux, records still to come]
+    for i, (seq, cid, code, aux, arg) in enumerate(_rows(events)):
         if last_seq is not None and seq <= last_seq:
-            return False, "seq not strictly increasing at %d" % seq
+            return False, i, "seq not strictly increasing at %d" % seq
         last_seq = seq
         if cid == 0:
-            return False, "event names no claim (unclaimed) at seq %d" % seq
+            return False, i, "event names no claim (unclaimed) at seq %d" % seq
+        if group is not None and not (code == REFUSED and arg == group[0] and aux == group[1]):
+            return False, i, "blocking_claim_ids run of request %#x interrupted (seq %d)" % (group[0], seq)
         s = state.get(cid, _S0)
         nxt = _NEXT.get((s, code))
         if nxt is None:
-            return False, "claim %#x: code %d not allowed in state %d (seq %d)" % (cid, code, s, seq)
-        if code == REFUSED and (arg != cid or aux != 1):
-            return False, "claim %#x: blocking_claim_ids is not [C] (seq %d)" % (cid, seq)
+            return False, i, "claim %#x: code %d not allowed in state %d (seq %d)" % (cid, code, s, seq)
+        if code == RESTORATION_FAILED:
+            pending += 1
+        elif code in (DEMOTED, EXPIRED):
+            pending -= 1
+        elif code == REFUSED:
+            if aux & REQ_FLAG:
+                if group is None:
+                    k = aux & ~REQ_FLAG
+                    if k == 0 or k != pending:
+                        return False, i, "request %#x: blocking_claim_ids is not the exact failed subset (seq %d)" % (arg, seq)
+                    group = [arg, aux, k]
+                group[2] -= 1
+                if group[2] == 0:
+                    group = None
+            elif arg != cid or aux != 1:
+                return False, i, "claim %#x: blocking_claim_ids is not [C] (seq %d)" % (cid, seq)
+            pending -= 1
         state[cid] = nxt
-    return True, "ok"
+    return True, -1, "ok"
+
+
+def validate(events):
+    """Returns (ok, reason).  ok is True iff the whole stream is in the accepted language."""
+    ok, _, why = _scan(events)
+    return ok, why
 
 
 FAILURE_ORDER = [ACCEPTED, MATERIALIZED, OFFLOADED, RESTORE_REQUIRED, LOAD_FAILED, RESTORATION_FAILED, REFUSED]
@@ -107,20 +145,6 @@ def observation_gate(events, cid):
 
 
 def validate_index(events):
-    """validate() with the stream position of the first violation: (True, -1) or (False, index).
-    Same loop as validate(); the position is where that loop stops."""
-    state = {}
-    last_seq = None
-    for i, (seq, cid, code, aux, arg) in enumerate(_rows(events)):
-        if last_seq is not None and seq <= last_seq:
-            return False, i
-        last_seq = seq
-        if cid == 0:
-            return False, i
-        nxt = _NEXT.get((state.get(cid, _S0), code))
-        if nxt is None:
-            return False, i
-        if code == REFUSED and (arg != cid or aux != 1):
-            return False, i
-        state[cid] = nxt
-    return True, -1
+    """validate() with the stream position of the first violation: (True, -1) or (False, index)."""
+    ok, i, _ = _scan(events)
+    return ok, i
