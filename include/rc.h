@@ -54,11 +54,15 @@ enum { RC_EV_ACCEPTED = 1,          /* aux = N (predicate threshold), arg = P (p
        RC_EV_LOAD_FAILED = 5,       /* aux = first bad block index, 0xFFFFFFFF = transfer error    */
        RC_EV_RESTORED = 6,          /* aux = nb, arg = chain checksum                              */
        RC_EV_RESTORATION_FAILED = 7,
-       RC_EV_ACTIVE_REQUEST_REFUSED = 8 /* aux = 1 = |blocking_claim_ids|, arg = C                 */ };
+       RC_EV_ACTIVE_REQUEST_REFUSED = 8, /* aux = 1 = |blocking_claim_ids|, arg = C; request form below */
+       RC_EV_DEMOTED = 9, RC_EV_EXPIRED = 10 /* NEXT-3: the other claim-scoped outcomes of a failed restoration */ };
+/* request-level refusal (rc_restore_request): aux = RC_REFUSED_REQUEST | size of blocking_claim_ids, arg = request id */
+#define RC_REFUSED_REQUEST 0x80000000u
 
 /* claim states */
 enum { RC_CS_ACCEPTED = 1, RC_CS_MATERIALIZED = 2, RC_CS_OFFLOADED = 3, RC_CS_RESIDENT_AGAIN = 4,
-       RC_CS_REFUSED = 5 };
+       RC_CS_REFUSED = 5, RC_CS_DEMOTED = 6, RC_CS_EXPIRED = 7 };
+enum { RC_POLICY_REFUSE = 0, RC_POLICY_DEMOTE = 1, RC_POLICY_EXPIRE = 2 };
 
 enum { RC_FAULT_XFER_ERROR = 1, RC_FAULT_BITFLIP = 2 };
 enum { RC_FAULT_ALLOW_UNCLAIMED = 1 };
@@ -158,6 +162,19 @@ int rc_restore(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* statu
 int rc_offload_begin(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
 int rc_restore_begin(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
 int rc_wait(rc_ctx* ctx, int which);
+
+/* NEXT-3.  rc_set_policy: what a failed restoration means for each named claim -- refusal
+ * (default), demotion or expiry ("claim-scoped restoration failure/refusal, demotion, expiry");
+ * a demoted / expired claim gets RESTORE_REQUIRED, LOAD_FAILED, RESTORATION_FAILED, DEMOTED | EXPIRED and is
+ * terminal.  Unknown id or policy -> RC_ERR_INVALID, nothing changes.
+ * rc_restore_request: the batch is ONE reuse request (request_id != 0) naming several claims.  Per-claim records
+ * are as in rc_restore except that refusals are deferred: after all of them the request is refused once, by one
+ * ACTIVE_REQUEST_REFUSED record per blocking claim in batch order (claim_id = the blocking claim,
+ * aux = RC_REFUSED_REQUEST | k, arg = request_id) -- blocking_claim_ids is exactly the k claims whose restoration
+ * failed under the refusal policy (smeared or partial attribution fails closed). */
+int rc_set_policy(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, const uint32_t* policy);
+int rc_restore_request(rc_ctx* ctx, uint64_t request_id, uint32_t n, const uint64_t* claim_id, int32_t* status);
+int rc_restore_request_begin(rc_ctx* ctx, uint64_t request_id, uint32_t n, const uint64_t* claim_id, int32_t* status);
 
 /* Drains up to cap not-yet-returned events of completed calls, in seq order. */
 int rc_outcomes(rc_ctx* ctx, rc_event* buf, uint64_t cap, uint64_t* n_out);

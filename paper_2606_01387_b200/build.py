@@ -9,8 +9,8 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(_HERE, "librc.so")
 SRCS = [os.path.join(_HERE, "csrc", "librc.cu")]
-DEPS = SRCS + [os.path.join(_HERE, "csrc", "rc_kernels.cuh"),
-               os.path.join(os.path.dirname(_HERE), "include", "rc.h")]
+DEPS = [os.path.join(_HERE, "csrc", f) for f in sorted(os.listdir(os.path.join(_HERE, "csrc")))] + [
+    os.path.join(os.path.dirname(_HERE), "include", "rc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]

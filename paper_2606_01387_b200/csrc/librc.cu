@@ -78,7 +78,7 @@ struct ExtAlloc {
 
 struct Claim {
   u64 id = 0, chain = 0;
-  u32 state = 0, P = 0, N = 0, M = 0, nb = 0;
+  u32 state = 0, P = 0, N = 0, M = 0, nb = 0, policy = 0;
   u32 bt_off = 0, bt_len = 0;            // live table extent (bt_len == 0: no table)
   u32 dg_off = 0, dg_len = 0;            // recorded digests
   std::vector<std::pair<u64, u64>> host; // host-store extents in blk units
@@ -133,6 +133,7 @@ struct rc_ctx {
   std::string cuda_err;
   int accept_ctas = 32;
   // NEXT-2: content-addressed host store
+  u64 request_id = 0;                                    // NEXT-3: the reuse request of the restore being begun (0: per-claim)
   bool dedup = false;
   std::unordered_map<u64, std::pair<u32, u32>> store;    // digest -> (slot, references)
   std::vector<u32> pending_free;                         // slots of an in-flight restore, recycled at its completion
@@ -360,8 +361,8 @@ static int fetch_res(rc_ctx* c, int set, u32 n) {
   CK(cudaMemcpyAsync(c->h_res[set], c->d_res[set], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
   return RC_OK;
 }
-static int emit(rc_ctx* c, int set, u32 n, int mode) {
-  k_emit<<<1, 256, 0, c->meta>>>(c->d_desc[set], c->d_res[set], n, mode, c->d_ring, c->cfg.max_events, c->d_evcount);
+static int emit(rc_ctx* c, int set, u32 n, int mode, u64 request_id = 0) {
+  k_emit<<<1, 256, 0, c->meta>>>(c->d_desc[set], c->d_res[set], n, mode, c->d_ring, c->cfg.max_events, c->d_evcount, request_id);
   CKL();
   c->st.kernel_launches++;
   return RC_OK;
@@ -700,7 +701,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     u64 o;
     if (Te + cl.nb > c->cap_entries || !c->bt_alloc.alloc(cl.nb, o)) { rollback(); return RC_ERR_CAPACITY; }
     hd[k].chain = cl.chain; hd[k].P = cl.P; hd[k].N = cl.N; hd[k].M = cl.M; hd[k].nb = cl.nb;
-    hd[k].bt_off = (u32)o; hd[k].bt_len = cl.nb; hd[k].dg_off = cl.dg_off; hd[k].flags = D_ELIG;
+    hd[k].bt_off = (u32)o; hd[k].bt_len = cl.nb; hd[k].dg_off = cl.dg_off; hd[k].flags = D_ELIG; hd[k].pad = cl.policy;
     op.cl[k] = &cl;
     elig.push_back(k);
     Te += cl.nb;
@@ -805,7 +806,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
                                                c->d_used, c->d_ref, c->fill, c->cfg.block_size);
   CKL();
   c->st.kernel_launches++;
-  if ((rc = emit(c, 1, n, EM_RESTORE))) return rc;
+  if ((rc = emit(c, 1, n, EM_RESTORE, c->request_id))) return rc;
   CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
   CK(cudaEventRecord(op.done, c->meta));
   c->ev_reserved += 4ull * n_served;
@@ -835,7 +836,7 @@ static int wait_restore(rc_ctx* c) {
       c->bt_alloc.release(hd[k].bt_off, cl->nb);
       if (cl->dg_len) { c->dg_alloc.release(cl->dg_off, cl->dg_len); cl->dg_len = 0; }
       cl->bt_len = 0;
-      cl->state = RC_CS_REFUSED;                             // terminal (fail-closed active outcome)
+      cl->state = cl->policy == POL_DEMOTE ? RC_CS_DEMOTED : (cl->policy == POL_EXPIRE ? RC_CS_EXPIRED : RC_CS_REFUSED);   // terminal
       c->ev_emitted += 4; c->st.claims_refused++;
       op.status[k] = RC_ST_RESTORE_FAILED;
     }
@@ -863,6 +864,27 @@ extern "C" int rc_restore(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st
 }
 
 #include "rc_dedup.inl"
+
+// NEXT-3: one reuse request naming several claims; refusal carries exactly the failed subset (rc.h)
+extern "C" int rc_restore_request_begin(rc_ctx* c, uint64_t request_id, uint32_t n, const uint64_t* id, int32_t* st) {
+  GUARD();
+  if (request_id == 0) return RC_ERR_INVALID;
+  c->request_id = request_id;
+  const int rc = rc_restore_begin(c, n, id, st);
+  c->request_id = 0;
+  return rc;
+}
+extern "C" int rc_restore_request(rc_ctx* c, uint64_t request_id, uint32_t n, const uint64_t* id, int32_t* st) {
+  const int rc = rc_restore_request_begin(c, request_id, n, id, st);
+  return rc ? rc : wait_restore(c);
+}
+extern "C" int rc_set_policy(rc_ctx* c, uint32_t n, const uint64_t* id, const uint32_t* policy) {
+  GUARD();
+  if (n && (!id || !policy)) return RC_ERR_INVALID;
+  for (u32 k = 0; k < n; ++k) if (!c->claims.count(id[k]) || policy[k] > RC_POLICY_EXPIRE) return RC_ERR_INVALID;
+  for (u32 k = 0; k < n; ++k) c->claims[id[k]].policy = policy[k];
+  return RC_OK;
+}
 
 // ---- outcomes, faults, release -----------------------------------------------------------------------------
 extern "C" int rc_outcomes(rc_ctx* c, rc_event* buf, uint64_t cap, uint64_t* n_out) {

@@ -172,7 +172,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     u64 o;
     if (Te + cl.nb > c->cap_entries || !c->bt_alloc.alloc(cl.nb, o)) { rollback(); return RC_ERR_CAPACITY; }
     hd[k].chain = cl.chain; hd[k].P = cl.P; hd[k].N = cl.N; hd[k].M = cl.M; hd[k].nb = cl.nb;
-    hd[k].bt_off = (u32)o; hd[k].bt_len = cl.nb; hd[k].dg_off = cl.dg_off; hd[k].flags = D_ELIG;
+    hd[k].bt_off = (u32)o; hd[k].bt_len = cl.nb; hd[k].dg_off = cl.dg_off; hd[k].flags = D_ELIG; hd[k].pad = cl.policy;
     op.cl[k] = &cl;
     elig.push_back(k);
     Te += cl.nb;
@@ -306,7 +306,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
                                                c->d_used, c->d_ref, c->fill, c->cfg.block_size);
   CKL();
   c->st.kernel_launches++;
-  if ((rc = emit(c, 1, n, EM_RESTORE))) return rc;
+  if ((rc = emit(c, 1, n, EM_RESTORE, c->request_id))) return rc;
   CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
   CK(cudaEventRecord(op.done, c->meta));
   c->ev_reserved += 4ull * n_served;

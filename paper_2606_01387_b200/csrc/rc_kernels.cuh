@@ -41,7 +41,7 @@ struct Desc {
   u32 dg_off;             // digest extent in the digest arena (nb entries)
   u32 flags;              // D_* below
   u32 src_off;            // accept: offset of the candidate table in the upload buffer
-  u32 pad;
+  u32 pad;                // restore: the claim's failure policy (POL_*)
 };
 enum { D_ELIG = 1, D_XFER = 2 };
 
@@ -57,6 +57,9 @@ struct Event { u64 seq, claim_id; u32 code, aux; u64 arg; };
 enum { EV_ACCEPTED = 1, EV_MATERIALIZED = 2, EV_OFFLOADED = 3, EV_RESTORE_REQUIRED = 4, EV_LOAD_FAILED = 5,
        EV_RESTORED = 6, EV_RESTORATION_FAILED = 7, EV_ACTIVE_REQUEST_REFUSED = 8 };
 enum { EM_ACCEPT = 0, EM_MATERIALIZE = 1, EM_OFFLOAD = 2, EM_RESTORE = 3 };
+enum { EV_DEMOTED = 9, EV_EXPIRED = 10 };            // NEXT-3: other claim-scoped outcomes of a failed restoration
+enum { POL_REFUSE = 0, POL_DEMOTE = 1, POL_EXPIRE = 2 };   // Desc.pad carries the claim's failure policy
+constexpr u32 REQ_FLAG = 0x80000000u;                // REFUSED.aux of a request-level refusal: flag | subset size
 
 __device__ __forceinline__ u64 mixL(u64 x) { u64 y = x ^ (x >> 32); y *= C2; return y ^ (y >> 29); }
 __device__ __forceinline__ u64 mixF(u64 x) { u64 y = mixL(x); y *= C1; return y ^ (y >> 32); }
@@ -535,16 +538,20 @@ __global__ void k_accept(const Desc* __restrict__ desc, Res* __restrict__ res, u
 // records of claim k precede those of claim k+1 and seq is gap-free (P:L27 order per claim).
 // ---------------------------------------------------------------------------------------------
 __global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ res, u32 n, int mode,
-                       Event* __restrict__ ring, u32 ring_cap, u64* __restrict__ ev_count) {
+                       Event* __restrict__ ring, u32 ring_cap, u64* __restrict__ ev_count, u64 request_id) {
   __shared__ u32 wt[32];
   const u64 seq0 = *ev_count;
-  u32 carry = 0;
+  u32 carry = 0, carry_b = 0;
+  // what a failed restoration means for claim k: refusal (per claim, or deferred to the request's run), demotion, expiry
+  auto blocks_request = [&](const Desc& d, const Res& r) {
+    return mode == EM_RESTORE && request_id != 0 && (r.flag & R_SERVED) && !(r.flag & R_OK) && d.pad == POL_REFUSE;
+  };
   for (u32 base = 0; base < n; base += blockDim.x) {
     const u32 k = base + threadIdx.x;
     Desc d; Res r; u32 c = 0;
     if (k < n) {
       d = desc[k]; r = res[k];
-      if (mode == EM_RESTORE) c = (r.flag & R_SERVED) ? ((r.flag & R_OK) ? 2u : 4u) : 0u;
+      if (mode == EM_RESTORE) c = (r.flag & R_SERVED) ? ((r.flag & R_OK) ? 2u : (blocks_request(d, r) ? 3u : 4u)) : 0u;
       else c = (r.flag & R_OK) ? 1u : 0u;
     }
     u32 tot;
@@ -564,7 +571,9 @@ __global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ re
         else {
           put(EV_LOAD_FAILED, r.val, 0);
           put(EV_RESTORATION_FAILED, 0, 0);
-          put(EV_ACTIVE_REQUEST_REFUSED, 1, d.id);
+          if (d.pad == POL_DEMOTE) put(EV_DEMOTED, 0, 0);
+          else if (d.pad == POL_EXPIRE) put(EV_EXPIRED, 0, 0);
+          else if (request_id == 0) put(EV_ACTIVE_REQUEST_REFUSED, 1, d.id);
         }
       }
     }
@@ -572,7 +581,33 @@ __global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ re
     __syncthreads();
   }
   __syncthreads();
-  if (threadIdx.x == 0) *ev_count = seq0 + carry;
+  if (mode == EM_RESTORE && request_id != 0) {
+    // request-level refusal: one record per blocking claim, batch order, after the per-claim records;
+    // aux = REQ_FLAG | size of the failed subset, arg = request id (blocking_claim_ids = the run's claim ids)
+    u32 K = 0;
+    for (u32 base = 0; base < n; base += blockDim.x) {
+      const u32 k = base + threadIdx.x;
+      const u32 b = (k < n && blocks_request(desc[k], res[k])) ? 1u : 0u;
+      u32 tot;
+      block_scan_incl(b, wt, tot);
+      K += tot;
+      __syncthreads();
+    }
+    for (u32 base = 0; base < n; base += blockDim.x) {
+      const u32 k = base + threadIdx.x;
+      const u32 b = (k < n && blocks_request(desc[k], res[k])) ? 1u : 0u;
+      u32 tot;
+      const u32 o = carry_b + block_scan_incl(b, wt, tot) - b;
+      if (b) {
+        const u64 s = seq0 + carry + o;
+        ring[s % ring_cap] = Event{s, desc[k].id, EV_ACTIVE_REQUEST_REFUSED, REQ_FLAG | K, request_id};
+      }
+      carry_b += tot;
+      __syncthreads();
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) *ev_count = seq0 + carry + carry_b;
 }
 
 // fault injection (CPU->GPU transfers only): flip bit 0 of the listed staged bytes

@@ -20,9 +20,12 @@ ST_OK, ST_PRED_FALSE, ST_UNKNOWN_CLAIM, ST_BAD_STATE, ST_DUPLICATE_ID, ST_BAD_TA
 ST_NO_FREE_BLOCKS, ST_NO_HOST_SPACE, ST_RESTORE_FAILED = 6, 7, 8
 FAULT_XFER_ERROR, FAULT_BITFLIP, FAULT_ALLOW_UNCLAIMED = 1, 2, 1
 MOVER_AUTO, MOVER_LDG, MOVER_TMA = 0, 1, 2
+REQ_FLAG = 0x80000000
+POLICY_REFUSE, POLICY_DEMOTE, POLICY_EXPIRE = 0, 1, 2
 
 EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_accept", "rc_materialize", "rc_offload",
-           "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_outcomes", "rc_set_faults",
+           "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_set_policy", "rc_restore_request",
+           "rc_restore_request_begin", "rc_outcomes", "rc_set_faults",
            "rc_release", "rc_claim_info", "rc_claim_blocks", "rc_claim_digests", "rc_host_read", "rc_pool_state",
            "rc_stats_get", "rc_stats_reset", "rc_measure_link", "rc_digest_blocks", "rc_validate_trace", "rc_strerror",
            "rc_last_cuda_error"]
@@ -186,6 +189,27 @@ class RC:
         self._ck(self.L.rc_restore_begin(self.h, ids.size, _p(ids), _p(st)), "rc_restore_begin")
         self._pending[1] = (ids, st)
         return st
+
+    def restore_request(self, request_id, ids, check=True):
+        ids = _u64(ids)
+        st = np.full(ids.size, -1, np.int32)
+        rc = self.L.rc_restore_request(self.h, C.c_uint64(request_id), ids.size, _p(ids), _p(st))
+        if check:
+            self._ck(rc, "rc_restore_request")
+            return st
+        return rc, st
+
+    def restore_request_begin(self, request_id, ids):
+        ids = _u64(ids)
+        st = np.full(ids.size, -1, np.int32)
+        self._ck(self.L.rc_restore_request_begin(self.h, C.c_uint64(request_id), ids.size, _p(ids), _p(st)),
+                 "rc_restore_request_begin")
+        self._pending[1] = (ids, st)
+        return st
+
+    def set_policy(self, ids, policy):
+        ids, policy = _u64(ids), _u32(policy)
+        return self.L.rc_set_policy(self.h, ids.size, _p(ids), _p(policy))
 
     def wait(self, which):
         self._ck(self.L.rc_wait(self.h, which), "rc_wait")

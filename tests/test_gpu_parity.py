@@ -367,3 +367,53 @@ def test_dedup_overlapped_begin_wait_matches_synchronous_order():
     assert np.array_equal(o.release(ids), r.release(ids))
     assert r.stats()["host_used_bytes"] == 0
     p.close()
+
+
+# ---- NEXT-3: multi-claim reuse requests, demotion / expiry ------------------------------------------------
+@pytest.mark.parametrize("dedup", [False, True])
+def test_requests_and_failure_policies_parity(dedup):
+    """One reuse request over several claims: refusal names exactly the failed subset (P:L87, P:L269, P:L384);
+    demotion / expiry as the claim's outcome of a failed restoration.  Events, statuses, states and
+    pool state equal the oracle's; overlapped begin/wait form included."""
+    wl = W.make_workload(0)
+    wave = W.plan_waves(wl, 1 << 30)[0]
+    cl = wl.claims
+    ids = [c.claim_id for c in cl]
+    p = Pair(wl, 1 << 30, chunk_blocks=10, dedup=dedup)
+    o, r = p.o, p.r
+    p.set_fill(wave.fill_ids, wave.fill_val)
+    for x in (o, r):
+        assert x.mark_used(wave.used_ids) == 0
+    args = (ids, [c.P for c in cl], [c.N for c in cl], wave.bt_off, wave.bt_ids)
+    assert np.array_equal(o.accept(*args), r.accept(*args))
+    assert np.array_equal(o.materialize(ids), r.materialize(ids))
+    ok = [ids[k] for k in range(8) if k != 6]
+    assert np.array_equal(o.offload(ok), r.offload(ok))
+    p.poison_free()
+    for x in (o, r):
+        assert x.set_policy([ok[0], ok[1]], [1, 2]) == 0
+        assert x.set_policy([0xBAD], [1]) != 0 and x.set_policy([ok[2]], [7]) != 0
+        assert x.set_faults([(ok[0], W.FK_XFER_ERROR, 0), (ok[1], W.FK_BITFLIP, 3), (ok[2], W.FK_XFER_ERROR, 0),
+                             (ok[4], W.FK_BITFLIP, 77777)]) == 0
+    req = 0x5151
+    q = ok[:5] + [ids[6], 0xFEED]                               # + a PRED_FALSE claim and an unknown id
+    sa, sb = o.restore_request(req, q), r.restore_request(req, q)
+    assert np.array_equal(sa, sb) and list(sa) == [8, 8, 8, 0, 8, 3, 2]
+    p.check_claims(ids, "request")
+    p.check_pool_state("request")
+    ev = p.check_events("request")
+    grp = [e for e in ev if int(e["code"]) == 8]
+    assert [int(e["claim_id"]) for e in grp] == [ok[2], ok[4]] and all(int(e["aux"]) == (rc.REQ_FLAG | 2) for e in grp)
+    ok_, why = V.validate(ev)
+    assert ok_, why
+    # second request, overlapped form, no failure -> no refusal record
+    sa = o.restore_request(req + 1, ok[5:])
+    r.restore_request_begin(req + 1, ok[5:])
+    sb = r.wait(1)
+    assert np.array_equal(sa, sb) and not sa.any()
+    ev2 = p.check_events("request 2")
+    assert 8 not in [int(e["code"]) for e in ev2]
+    assert np.array_equal(o.restore(ok), r.restore(ok))         # all terminal or resident: BAD_STATE everywhere
+    rcode, _ = r.restore_request(0, ok, check=False)
+    assert rcode == rc.ERR_INVALID
+    p.close()
