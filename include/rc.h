@@ -209,9 +209,12 @@ int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64
 /* NEXT-1: the paper's artifact analyzer as a device pass.  Validates an event
  * array (HOST, n records in stream order; may contain the harness marker codes RC_EV_USE and
  * RC_EV_REQUEST_FINISHED) against the per-claim language
- *   ACCEPTED MATERIALIZED ( OFFLOADED RESTORE_REQUIRED ( RESTORED USE* | LOAD_FAILED RESTORATION_FAILED REFUSED ) )*
+ *   ACCEPTED MATERIALIZED ( OFFLOADED RESTORE_REQUIRED ( RESTORED USE* | LOAD_FAILED RESTORATION_FAILED
+ *                                                          ( REFUSED | DEMOTED | EXPIRED ) ) )*
  * (any prefix valid; only REQUEST_FINISHED may follow REFUSED; REQUEST_FINISHED also ends ACCEPTED /
- * MATERIALIZED / RESTORED), seq strictly increasing, no event with claim id 0, REFUSED carrying [C].
+ * MATERIALIZED / RESTORED), seq strictly increasing, no event with claim id 0, REFUSED carrying [C] (aux 1, arg C)
+ * or belonging to a request run (aux = RC_REFUSED_REQUEST | k, arg = request id: k consecutive records that name
+ * exactly the k claims whose restoration failed and is unanswered).
  * report->ok = 1 iff the whole stream is accepted; first_bad_index = stream position of the first
  * violation (UINT64_MAX if none).  claims (HOST, may be NULL) receives up to cap per-claim records in
  * unspecified order: final automaton state, gate bits (RC_GATE_FAILURE: the claim's subsequence ends with

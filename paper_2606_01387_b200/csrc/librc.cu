@@ -1100,7 +1100,7 @@ extern "C" int rc_validate_trace(const rc_event* events, uint64_t n, rc_trace_re
   u32 slots = 1024;
   while ((u64)slots < 2 * n) slots <<= 1;
   Event* d_ev = nullptr; u64* d_keys = nullptr; u32 *d_count = nullptr, *d_base = nullptr, *d_dense = nullptr, *d_fill = nullptr;
-  u32 *d_slot = nullptr, *d_bucket = nullptr, *d_cur = nullptr; unsigned long long* d_bad = nullptr; ClaimOut* d_out = nullptr;
+  u32 *d_slot = nullptr, *d_bucket = nullptr, *d_cur = nullptr, *d_bsum = nullptr; unsigned long long* d_bad = nullptr; ClaimOut* d_out = nullptr;
   cudaStream_t st = nullptr; cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr, e3 = nullptr;
   int rc = RC_OK;
   std::vector<ClaimOut> host_out;
@@ -1120,6 +1120,13 @@ extern "C" int rc_validate_trace(const rc_event* events, uint64_t n, rc_trace_re
   tv_insert<<<(u32)((n + 255) / 256), 256, 0, st>>>((const Event*)d_ev, n, d_keys, d_count, slots - 1, d_slot, d_bad);
   tv_alloc<<<(slots + 255) / 256, 256, 0, st>>>(d_count, slots, d_base, d_dense, d_cur);
   tv_scatter<<<(u32)((n + 255) / 256), 256, 0, st>>>(n, d_slot, d_base, d_fill, d_bucket);
+  {                                                        // request-level refusal runs (cross-claim rule)
+    const u32 nbk = (u32)((n + 1023) / 1024);
+    TV(cudaMalloc(&d_bsum, (u64)nbk * 4));
+    tv_delta_sum<<<nbk, 1024, 0, st>>>((const Event*)d_ev, n, d_bsum);
+    tv_scan_bsum<<<1, 1024, 0, st>>>(d_bsum, nbk);
+    tv_groups<<<nbk, 1024, 0, st>>>((const Event*)d_ev, n, d_bsum, d_bad);
+  }
   tv_walk<<<(slots + 127) / 128, 128, 0, st>>>((const Event*)d_ev, d_keys, d_count, slots, d_base, d_dense, d_bucket, d_out, d_bad);
   TV(cudaGetLastError());
   TV(cudaEventRecord(e2, st));
@@ -1145,7 +1152,7 @@ extern "C" int rc_validate_trace(const rc_event* events, uint64_t n, rc_trace_re
 done:
 #undef TV
   cudaFree(d_ev); cudaFree(d_keys); cudaFree(d_count); cudaFree(d_base); cudaFree(d_dense); cudaFree(d_fill);
-  cudaFree(d_slot); cudaFree(d_bucket); cudaFree(d_cur); cudaFree(d_bad); cudaFree(d_out);
+  cudaFree(d_slot); cudaFree(d_bucket); cudaFree(d_cur); cudaFree(d_bad); cudaFree(d_out); cudaFree(d_bsum);
   if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); if (e2) cudaEventDestroy(e2); if (e3) cudaEventDestroy(e3);
   if (st) cudaStreamDestroy(st);
   return rc;

@@ -15,18 +15,21 @@
 namespace rct {
 using namespace rck;
 
-enum { S0 = 0, ACC, MAT, OFF, RREQ, LF, RF, REF, RES, FIN, BAD, NSTATE };
+enum { S0 = 0, ACC, MAT, OFF, RREQ, LF, RF, REF, RES, FIN, DEM, EXP, BAD, NSTATE };
 enum { EV_USE = 100, EV_FIN = 101 };
 enum { G_FAILURE = 1, G_OBSERVATION = 2 };
 constexpr u64 NO_BAD = ~0ull;
 
 struct ClaimOut { u64 claim_id; u64 first_bad; u32 state; u32 gates; u32 n_events; u32 pad; };
 
-__device__ __forceinline__ int col_of(u32 code) { return code >= 1 && code <= 8 ? (int)code - 1 : (code == EV_USE ? 8 : (code == EV_FIN ? 9 : -1)); }
+__device__ __forceinline__ int col_of(u32 code) {
+  return code >= 1 && code <= 8 ? (int)code - 1 : (code == EV_USE ? 8 : (code == EV_FIN ? 9 : (code == EV_DEMOTED ? 10 : (code == EV_EXPIRED ? 11 : -1))));
+}
 
 // next-state table [state][column]; BAD = not in the accepted language
 __device__ __forceinline__ u32 next_state(u32 s, int col) {
   // columns: 0 ACCEPTED 1 MATERIALIZED 2 OFFLOADED 3 RESTORE_REQUIRED 4 LOAD_FAILED 5 RESTORED 6 RESTORATION_FAILED 7 REFUSED 8 USE 9 FIN
+  //          10 DEMOTED 11 EXPIRED (NEXT-3)
   switch (s) {
     case S0:   return col == 0 ? ACC : BAD;
     case ACC:  return col == 1 ? MAT : (col == 9 ? FIN : BAD);
@@ -34,8 +37,10 @@ __device__ __forceinline__ u32 next_state(u32 s, int col) {
     case OFF:  return col == 3 ? RREQ : BAD;
     case RREQ: return col == 5 ? RES : (col == 4 ? LF : BAD);
     case LF:   return col == 6 ? RF : BAD;
-    case RF:   return col == 7 ? REF : BAD;
+    case RF:   return col == 7 ? REF : (col == 10 ? DEM : (col == 11 ? EXP : BAD));
     case REF:  return col == 9 ? FIN : BAD;
+    case DEM:  return col == 9 ? FIN : BAD;
+    case EXP:  return col == 9 ? FIN : BAD;
     case RES:  return col == 2 ? OFF : (col == 8 ? RES : (col == 9 ? FIN : BAD));
     default:   return BAD;
   }
@@ -107,10 +112,11 @@ __global__ void tv_walk(const Event* __restrict__ ev, const u64* __restrict__ ke
     const Event e = ev[b[i]];
     const int col = col_of(e.code);
     u32 nx = col < 0 ? (u32)BAD : next_state(st, col);
-    if (nx != BAD && e.code == EV_ACTIVE_REQUEST_REFUSED && (e.arg != cid || e.aux != 1)) nx = BAD;
+    // per-claim refusal carries [C] itself; the request form (REQ_FLAG) is checked across claims by tv_groups
+    if (nx != BAD && e.code == EV_ACTIVE_REQUEST_REFUSED && !(e.aux & REQ_FLAG) && (e.arg != cid || e.aux != 1)) nx = BAD;
     if (nx == BAD) { bad = b[i]; st = BAD; break; }
     st = nx;
-    if (col < 8) {
+    if (col < 8 || col >= 10) {
       if (n_codes == 0) c0 = e.code; else if (n_codes == 1) c1 = e.code;
       tail = ((tail << 4) | e.code) & 0xFFFFFu;
       ++n_codes;
@@ -126,6 +132,56 @@ __global__ void tv_walk(const Event* __restrict__ ev, const u64* __restrict__ ke
   }
   if (bad != NO_BAD) atomicMin(first_bad, (unsigned long long)bad);
   out[dense[s]] = ClaimOut{cid, bad, st, gates, c, 0};
+}
+
+// ---- request-level refusal runs (NEXT-3) -----------------------------------------------------
+// pending(i) = claims whose restoration failed and is unanswered before stream position i
+//            = #RESTORATION_FAILED - #(REFUSED | DEMOTED | EXPIRED) among events [0, i)   (valid up to the first violation).
+__device__ __forceinline__ u32 pend_delta(u32 code) {
+  return code == EV_RESTORATION_FAILED ? 1u : ((code == EV_ACTIVE_REQUEST_REFUSED || code == EV_DEMOTED || code == EV_EXPIRED) ? 0xFFFFFFFFu : 0u);
+}
+__global__ void tv_delta_sum(const Event* __restrict__ ev, u64 n, u32* __restrict__ bsum) {
+  __shared__ u32 wt[32];
+  const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+  u32 tot;
+  block_scan_incl(i < n ? pend_delta(ev[i].code) : 0u, wt, tot);
+  if (threadIdx.x == 0) bsum[blockIdx.x] = tot;
+}
+__global__ void tv_scan_bsum(u32* __restrict__ bsum, u32 nb) {          // exclusive scan in place, one CTA
+  __shared__ u32 wt[32];
+  u32 carry = 0;
+  for (u32 base = 0; base < nb; base += blockDim.x) {
+    const u32 k = base + threadIdx.x;
+    const u32 v = k < nb ? bsum[k] : 0u;
+    u32 tot;
+    const u32 inc = block_scan_incl(v, wt, tot);
+    if (k < nb) bsum[k] = carry + inc - v;
+    carry += tot;
+    __syncthreads();
+  }
+}
+__device__ __forceinline__ bool same_run(const Event& a, u64 arg, u32 aux) {
+  return a.code == EV_ACTIVE_REQUEST_REFUSED && a.arg == arg && a.aux == aux;
+}
+// A run of REFUSED records with the same (arg = request id, aux = REQ_FLAG | k) starts where the previous record does
+// not match.  The start checks: k >= 1 and k == pending (the run names exactly the failed, unanswered claims: neither
+// fewer nor -- via the per-claim automaton -- others); records 1..k-1 continue the run; a matching record at k would
+// open a second run with nothing pending.
+__global__ void tv_groups(const Event* __restrict__ ev, u64 n, const u32* __restrict__ boff, unsigned long long* __restrict__ first_bad) {
+  __shared__ u32 wt[32];
+  const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+  Event e; e.code = 0; e.aux = 0; e.arg = 0;
+  if (i < n) e = ev[i];
+  const u32 d = i < n ? pend_delta(e.code) : 0u;
+  u32 tot;
+  const u32 pending = boff[blockIdx.x] + block_scan_incl(d, wt, tot) - d;
+  if (i >= n || e.code != EV_ACTIVE_REQUEST_REFUSED || !(e.aux & REQ_FLAG)) return;
+  if (i > 0 && same_run(ev[i - 1], e.arg, e.aux)) return;                // not a run start
+  const u32 k = e.aux & ~REQ_FLAG;
+  if (k == 0 || k != pending) { atomicMin(first_bad, (unsigned long long)i); return; }
+  for (u32 j = 1; j < k && i + j < n; ++j)
+    if (!same_run(ev[i + j], e.arg, e.aux)) { atomicMin(first_bad, (unsigned long long)(i + j)); return; }
+  if (i + k < n && same_run(ev[i + k], e.arg, e.aux)) atomicMin(first_bad, (unsigned long long)(i + k));
 }
 
 }  // namespace rct

@@ -401,3 +401,103 @@ def make_shared_tiny(n_claims=6, seed=0, pool_blocks=256):
     wave = Wave(list(range(n_claims)), np.array(offs, np.uint32), np.array(tab_all, np.uint32),
                 np.unique(np.array(tab_all, np.uint32)), fb, np.array([fill[int(b)] for b in fb], np.uint8), [], 0)
     return Workload(0, g, claims), wave, copies
+
+
+REQ_FLAG = 0x80000000
+REQUEST_MUTATIONS = ["smeared_ids", "short_subset", "dropped_record", "extra_record", "other_request_id", "interrupted_run",
+                     "zero_subset", "early_finish"]
+
+
+def make_request_trace(n_requests, seed=0):
+    """Valid streams with multi-claim reuse requests (NEXT-3): every request names 2..5 offloaded claims; some fail
+    and are refused (request-level run), demoted or expired.  Returns (events, runs) where runs lists, per refused
+    request, the stream positions of its REFUSED records."""
+    rng = np.random.default_rng(SEED0 + 8000 + seed)
+    rows, hist, runs = [], [], []
+    next_id = 1
+    for r in range(n_requests):
+        m = int(rng.integers(2, 6))
+        cids = [int(next_id + 2 * j + 1) * 1000003 for j in range(m)]
+        next_id += 2 * m
+        for c in cids:
+            hist.append([(c, 1, 0, 0), (c, 2, 0, 0), (c, 3, 0, 0)])
+        req = 10 ** 12 + r
+        blocking = []
+        block = []
+        for c in cids:
+            block.append((c, 4, 0, 0))
+            u = rng.random()
+            if u < 0.55:
+                block.append((c, 6, 0, 0))
+            else:
+                block += [(c, 5, 0, 0), (c, 7, 0, 0)]
+                if u < 0.65:
+                    block.append((c, 9, 0, 0))
+                elif u < 0.75:
+                    block.append((c, 10, 0, 0))
+                else:
+                    blocking.append(c)
+        grp = [(c, 8, REQ_FLAG | len(blocking), req) for c in blocking]
+        rows.append((block, grp))
+    # histories interleaved at random (per-claim order kept), then the request blocks one after another
+    order = np.repeat(np.arange(len(hist)), 3)
+    rng.shuffle(order)
+    it = [iter(h) for h in hist]
+    flat = [next(it[k]) for k in order]
+    for block, grp in rows:
+        flat += block
+        if grp:
+            runs.append(list(range(len(flat), len(flat) + len(grp))))
+        flat += grp
+    ev = np.zeros(len(flat), TRACE_DTYPE)
+    for i, (c, code, aux, arg) in enumerate(flat):
+        ev[i] = (2 * i + 1, c, code, aux, arg)
+    return ev, runs
+
+
+def mutate_request_trace(ev, runs, kind, seed=0):
+    rng = np.random.default_rng(SEED0 + 9000 + seed)
+    ev = ev.copy()
+    big = [r for r in runs if len(r) >= 2] or runs
+    run = big[int(rng.integers(0, len(big)))]
+    req = ev["arg"][run[0]]
+
+    def reseq(a):
+        a["seq"] = np.arange(a.size, dtype=np.uint64) + np.uint64(1)
+        return a
+    if kind == "smeared_ids":                    # names a claim of the request that restored fine (P:L269)
+        start = run[0]
+        i = start - 1
+        while i >= 0 and ev["code"][i] != 6:
+            i -= 1
+        ev["claim_id"][run[-1]] = ev["claim_id"][i]
+    elif kind == "short_subset":                 # fewer ids than claims that failed
+        if len(run) >= 2:
+            ev["aux"][run] = REQ_FLAG | (len(run) - 1)
+            return reseq(np.delete(ev, run[-1]))
+        ev["aux"][run] = REQ_FLAG | 2
+    elif kind == "dropped_record":
+        return reseq(np.delete(ev, run[0])) if len(run) >= 2 else reseq(np.delete(ev, run[0] - 1))
+    elif kind == "extra_record":
+        return reseq(np.concatenate([ev[:run[-1] + 1], ev[run[-1]:run[-1] + 1], ev[run[-1] + 1:]]))
+    elif kind == "other_request_id":
+        ev["arg"][run[-1]] = req + np.uint64(12345)
+    elif kind == "interrupted_run":              # something else between the records of one run
+        if len(run) < 2:
+            ev["aux"][run] = REQ_FLAG | 2
+        else:
+            i = run[0] - 1
+            while ev["code"][i] not in (6, 9, 10, 3):
+                i -= 1
+            rec = np.zeros(1, TRACE_DTYPE)
+            rec["claim_id"], rec["code"] = ev["claim_id"][i], T_FIN
+            return reseq(np.concatenate([ev[:run[1]], rec, ev[run[1]:]]))
+    elif kind == "zero_subset":
+        ev["aux"][run] = REQ_FLAG
+    elif kind == "early_finish":                 # terminal handling before the request's outcome (P:L267, P:L380)
+        rec = np.zeros(1, TRACE_DTYPE)
+        rec["claim_id"], rec["code"] = ev["claim_id"][run[0]], T_FIN
+        return reseq(np.concatenate([ev[:run[0]], rec, ev[run[0]:]]))
+    else:
+        raise ValueError(kind)
+    return ev

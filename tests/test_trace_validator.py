@@ -88,3 +88,36 @@ def test_real_stream_from_the_oracle_run_validates_both_ways():
     o.materialize(ids); o.offload(ids); o.set_faults(wave.faults); o.restore(ids)
     ev = o.outcomes()
     assert V.validate_index(ev) == (True, -1)
+
+
+def test_request_traces_validate_and_every_request_mutation_is_rejected():
+    ev, runs = W.make_request_trace(120, 2)
+    assert V.validate_index(ev) == (True, -1) and len(runs) > 20
+    assert {9, 10} <= set(int(c) for c in ev["code"])
+    for kind in W.REQUEST_MUTATIONS:
+        m = W.mutate_request_trace(ev, runs, kind, 1)
+        ok, i = V.validate_index(m)
+        assert not ok and V.validate(m[:i])[0], kind
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", [0, 3])
+def test_gpu_validator_request_runs_and_policies_match_oracle(seed):
+    """NEXT-3 on the validator: demotion / expiry transitions and the cross-claim rule for request-level
+    refusal runs (exact failed subset, contiguous, one request id) -- P:L87."""
+    from paper_2606_01387_b200 import rc
+    ev, runs = W.make_request_trace(1500, seed)
+    rep, claims = rc.validate_trace(ev)
+    assert rep["ok"] == 1 and rep["first_bad_index"] == rc.NO_BAD
+    n_ref = len({int(e["claim_id"]) for e in ev if int(e["code"]) == 8})
+    assert rep["n_failure_gate"] == n_ref and rep["n_observation_gate"] == int((ev["code"] == 6).sum())
+    for kind in W.REQUEST_MUTATIONS:
+        for ms in range(4):
+            m = W.mutate_request_trace(ev, runs, kind, 10 * seed + ms)
+            ok, i = V.validate_index(m)
+            rep, _ = rc.validate_trace(m, want_claims=False)
+            assert not ok and rep["ok"] == 0 and rep["first_bad_index"] == i, (kind, ms, rep["first_bad_index"], i)
+    both = np.concatenate([W.make_trace(800, seed), ev])          # per-claim refusals and request runs in one stream
+    both["seq"] = np.arange(both.size)
+    rep, _ = rc.validate_trace(both, want_claims=False)
+    assert rep["ok"] == 1 and V.validate_index(both) == (True, -1)
