@@ -82,7 +82,7 @@ def host_ram_bytes():
 class Job:
     """One rank's workload: context, resident pool, pre-marshalled waves."""
 
-    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=8, dedup=False):
+    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=8, dedup=False, direct=False):
         import torch
         from paper_2606_01387_b200 import rc
         self.torch, self.rc = torch, rc
@@ -114,7 +114,7 @@ class Job:
         self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, self.pool, self.fill,
                        self.host_store, staging_chunk_bytes=min(chunk_bytes, self.host_store), staging_chunks=2,
                        max_claims=max(1024, 2 * n_max), max_table_entries=max(4 * g.pool_blocks, 1 << 16),
-                       max_events=max(1 << 16, 16 * n_max), mover=mover, grid_ctas=grid_ctas, dedup=dedup)
+                       max_events=max(1 << 16, 16 * n_max), mover=mover, grid_ctas=grid_ctas, dedup=dedup, direct_offload=direct)
         self.prep = []
         region = g.pool_blocks // wave_frac if pipelined else 0
         for wi, w in enumerate(self.waves):
@@ -288,6 +288,7 @@ def main():
     ap.add_argument("--serial", action="store_true", help="one wave at a time: offload, then restore (no duplex overlap)")
     ap.add_argument("--wave-frac", type=int, default=8, help="pipelined schedule: a wave uses 1/N of the pool (N >= 2)")
     ap.add_argument("--dedup", action="store_true", help="NEXT-2: content-addressed host store; value counts claim-logical bytes")
+    ap.add_argument("--direct-offload", action="store_true", help="NEXT-4 experiment: gather straight into the mapped pinned store")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per gather launch (profiles/), if known")
@@ -322,7 +323,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2606_01387_b200 import rc
     mover = {"auto": rc.MOVER_AUTO, "ldg": rc.MOVER_LDG, "tma": rc.MOVER_TMA}[a.mover]
-    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac), dedup=a.dedup)
+    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac), dedup=a.dedup, direct=a.direct_offload)
     g = job.g
     link = {}
     if world == 1:

@@ -95,7 +95,8 @@ typedef struct rc_config {
   uint32_t grid_ctas;       /* CTAs of a gather / scatter launch; 0 = library default                */
   uint32_t dedup;           /* NEXT-2: 1 = content-addressed host store keyed by block digest: a block shared
                                between claims is held and crosses the link once       */
-  uint32_t pad_;
+  uint32_t direct_offload;  /* NEXT-4 (experimental): 1 = the gather kernel stores straight into the mapped pinned
+                               store (no staging, no copy engine); ignored with dedup                          */
 } rc_config;
 
 typedef struct rc_claim_info_t {

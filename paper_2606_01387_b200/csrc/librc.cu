@@ -138,6 +138,8 @@ struct rc_ctx {
   std::unordered_map<u64, std::pair<u32, u32>> store;    // digest -> (slot, references)
   std::vector<u32> pending_free;                         // slots of an in-flight restore, recycled at its completion
   u64* h_dig = nullptr; u32 *h_iw = nullptr, *h_ispos = nullptr, *d_iw = nullptr, *d_ispos = nullptr;
+  // NEXT-4 (first half): gather straight into the mapped pinned store, no staging, no copy engine
+  bool direct = false; u8* h_store_dev = nullptr; u32 *h_hpos = nullptr, *d_hpos = nullptr;
 };
 
 #define CK(call)                                                                      \
@@ -206,8 +208,8 @@ extern "C" int rc_destroy(rc_ctx* c) {
   F(c->d_used); F(c->d_ref); F(c->d_bt); F(c->d_dg); F(c->d_ring); F(c->d_evcount); F(c->d_bitmaps); F(c->d_up);
   F(c->d_counters); F(c->d_alloc); F(c->d_flip);
   for (int i = 0; i < 3; ++i) { F(c->d_desc[i]); F(c->d_res[i]); F(c->d_off[i]); FH(c->h_desc[i]); FH(c->h_res[i]); }
-  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store); FH(c->h_dig); FH(c->h_iw); FH(c->h_ispos);
-  F(c->d_iw); F(c->d_ispos);
+  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store); FH(c->h_dig); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
+  F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
   for (int d = 0; d < 2; ++d) {
     F(c->d_phys[d]); F(c->d_dtmp[d]);
     for (auto p : c->staging[d]) F(p);
@@ -296,6 +298,11 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   CC(cudaHostAlloc(&c->h_flip, dc * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
   CC(cudaHostAlloc(&c->h_counters, 16, cudaHostAllocDefault), RC_ERR_NOMEM);
   c->dedup = cfg->dedup != 0;
+  c->direct = cfg->direct_offload != 0 && !c->dedup;
+  if (c->direct) {
+    CC(cudaHostAlloc(&c->h_hpos, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_hpos, cap * 4), RC_ERR_NOMEM);
+  }
   if (c->dedup) {
     CC(cudaHostAlloc(&c->h_dig, cap * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
     CC(cudaHostAlloc(&c->h_iw, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
@@ -320,7 +327,8 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
     CC(cudaEventCreateWithFlags(&c->ev_body_b[d], cudaEventDisableTiming), RC_ERR_CUDA);
     CC(cudaEventCreateWithFlags(&c->ops[d].done, cudaEventDisableTiming), RC_ERR_CUDA);
   }
-  if (c->host_blocks) CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocDefault), RC_ERR_NOMEM);
+  if (c->host_blocks) CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocMapped), RC_ERR_NOMEM);
+  if (c->host_blocks && c->direct) CC(cudaHostGetDevicePointer((void**)&c->h_store_dev, c->h_store, 0), RC_ERR_CUDA);
   // launch geometry of the movers
   c->mover = cfg->mover == RC_MOVER_AUTO ? RC_MOVER_TMA : cfg->mover;
   int occ = 0;
@@ -607,6 +615,27 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks, ++ci) {
     const u64 w1 = std::min(T, w0 + c->chunk_blocks);
     const u32 slot = ci % c->R, m = (u32)(w1 - w0);
+    if (c->direct) {
+      // the mover's destination is the claim's place in the mapped pinned store: the bulk stores of the gather
+      // kernel cross the link themselves (item -> host block through the same indirection the dedup restore uses)
+      while (si < segs.size() && segs[si].w0 < w1) {
+        const Seg& g = segs[si];
+        for (u64 w = std::max(g.w0, w0); w < std::min(g.w0 + g.n, w1); ++w) c->h_hpos[w] = (u32)(g.hoff + (w - g.w0));
+        if (g.w0 + g.n <= w1) ++si; else break;
+      }
+      CK(cudaMemcpyAsync(c->d_hpos + w0, c->h_hpos + w0, (u64)m * 4, cudaMemcpyHostToDevice, c->gather));
+      cudaEvent_t t0 = get_event(c), t1 = get_event(c);
+      CK(cudaEventRecord(t0, c->gather));
+      launch_move<MV_GATHER>(c, c->gather, c->h_store_dev, c->d_phys[0] + w0, c->part[0][slot], m, nullptr, c->d_hpos + w0);
+      CKL();
+      CK(cudaEventRecord(t1, c->gather));
+      op.t_copy.push_back({t0, t1});                       // the kernel IS the transfer
+      op.copy_bytes += (u64)m * c->blk;
+      k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, m, c->G, nullptr);
+      CKL();
+      c->st.kernel_launches += 2;
+      continue;
+    }
     if (c->slot_used[0][slot]) CK(cudaStreamWaitEvent(c->gather, c->ev_free[0][slot], 0));
     cudaEvent_t t0 = get_event(c), t1 = get_event(c);
     CK(cudaEventRecord(t0, c->gather));

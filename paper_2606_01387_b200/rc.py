@@ -39,7 +39,7 @@ class Config(C.Structure):
                 ("pool_dev", C.c_void_p), ("fill_dev", C.c_void_p),
                 ("stream_meta", C.c_void_p), ("stream_gather", C.c_void_p), ("stream_d2h", C.c_void_p),
                 ("stream_scatter", C.c_void_p), ("stream_h2d", C.c_void_p),
-                ("mover", C.c_uint32), ("grid_ctas", C.c_uint32), ("dedup", C.c_uint32), ("pad_", C.c_uint32)]
+                ("mover", C.c_uint32), ("grid_ctas", C.c_uint32), ("dedup", C.c_uint32), ("direct_offload", C.c_uint32)]
 
 
 class ClaimInfo(C.Structure):
@@ -106,7 +106,7 @@ class RC:
 
     def __init__(self, layers, kv_heads, head_dim, elem_bytes, block_size, pool_blocks, pool, fill,
                  host_store_bytes, staging_chunk_bytes=None, staging_chunks=2, max_claims=8192,
-                 max_table_entries=None, max_events=1 << 17, streams=None, mover=MOVER_AUTO, grid_ctas=0, dedup=False):
+                 max_table_entries=None, max_events=1 << 17, streams=None, mover=MOVER_AUTO, grid_ctas=0, dedup=False, direct_offload=False):
         self.L = lib()
         page = block_size * kv_heads * head_dim * elem_bytes
         self.page, self.blk, self.NB = page, 2 * layers * page, pool_blocks
@@ -118,7 +118,7 @@ class RC:
         cfg = Config(layers, kv_heads, head_dim, elem_bytes, block_size, pool_blocks, max_claims,
                      max_table_entries or max(4 * pool_blocks, 1 << 16), max_events, staging_chunks,
                      staging_chunk_bytes or min(1 << 30, max(self.blk, host_store_bytes)), host_store_bytes,
-                     pool.data_ptr(), fill.data_ptr(), s[0], s[1], s[2], s[3], s[4], mover, grid_ctas, int(dedup), 0)
+                     pool.data_ptr(), fill.data_ptr(), s[0], s[1], s[2], s[3], s[4], mover, grid_ctas, int(dedup), int(direct_offload))
         self.h = C.c_void_p()
         rc = self.L.rc_create(C.byref(cfg), C.byref(self.h))
         if rc != 0:

@@ -417,3 +417,13 @@ def test_requests_and_failure_policies_parity(dedup):
     rcode, _ = r.restore_request(0, ok, check=False)
     assert rcode == rc.ERR_INVALID
     p.close()
+
+
+@pytest.mark.parametrize("mover", [rc.MOVER_TMA, rc.MOVER_LDG])
+def test_direct_offload_into_mapped_pinned_store(mover):
+    """NEXT-4 (first half): the gather kernel's stores cross the link themselves; every observable unchanged."""
+    wl = W.make_workload(0)
+    p = Pair(wl, 1 << 30, chunk_blocks=9, mover=mover, direct_offload=True)
+    ev, st = p.run_wave(W.plan_waves(wl, 1 << 30)[0])
+    assert st[3] == rc.ST_RESTORE_FAILED and V.validate(ev)[0]
+    p.close()
