@@ -241,8 +241,8 @@ class OracleJob:
 
 
 def oracle_sample_shape(index):
-    # sized for roughly 10 s of single-thread work per pass
-    return {0: (8, 256), 1: (8, 640), 2: (3, 700), 3: (96, 2560), 4: (8, 640)}[index]
+    # sized for roughly 10-20 s of single-thread work per pass
+    return {0: (8, 256), 1: (16, 640), 2: (4, 800), 3: (256, 2560), 4: (16, 640)}[index]
 
 
 def run_oracle(index, steps, warmup):
