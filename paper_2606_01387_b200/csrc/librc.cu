@@ -633,7 +633,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
       op.copy_bytes += (u64)m * c->blk;
       k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, m, c->G, nullptr);
       CKL();
-      c->st.kernel_launches += 2;
+      c->st.kernel_launches++;
       continue;
     }
     if (c->slot_used[0][slot]) CK(cudaStreamWaitEvent(c->gather, c->ev_free[0][slot], 0));

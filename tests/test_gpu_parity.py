@@ -427,3 +427,46 @@ def test_direct_offload_into_mapped_pinned_store(mover):
     ev, st = p.run_wave(W.plan_waves(wl, 1 << 30)[0])
     assert st[3] == rc.ST_RESTORE_FAILED and V.validate(ev)[0]
     p.close()
+
+
+def test_large_batch_multi_tile_scans():
+    """3000 claims in one batch on a 98304-block pool: every single-CTA scan (offsets, restore plan, allocation,
+    event emission) runs over several tiles with carries; sub-batched restores hit NO_FREE_BLOCKS prefixes."""
+    wl = W.make_workload(0, n_claims=3000, pool_blocks=98304)
+    rng = np.random.default_rng(11)
+    for k in range(0, 3000, 97):
+        wl.claims[k].fault = (W.FK_XFER_ERROR, 0) if (k // 97) % 2 else (W.FK_BITFLIP, int(rng.integers(0, 1 << 31)))
+    for k in range(5, 3000, 211):
+        wl.claims[k].M = int(rng.integers(0, 448))          # under-materialized: PRED_FALSE
+        wl.claims[k].fault = None
+    host = 2 << 30
+    p = Pair(wl, host, chunk_blocks=4096, max_events=1 << 16)
+    waves = W.plan_waves(wl, host)
+    assert len(waves) == 1 and len(waves[0].claim_idx) == 3000
+    ids = [c.claim_id for c in wl.claims]
+    ev, st = p.run_wave(waves[0], restore_batches=[ids[:1500], ids[1500:]], check_bytes=False)
+    assert st.count(rc.ST_RESTORE_FAILED) == sum(1 for c in wl.claims if c.fault)
+    assert st.count(rc.ST_BAD_STATE) == sum(1 for c in wl.claims if c.M < c.N)
+    ok, why = V.validate(ev)
+    assert ok, why
+    # occupy most of the pool, then restore a batch that only partly fits: prefix grant across scan tiles
+    o, r = p.o, p.r
+    ok_ids = [c.claim_id for c in wl.claims if c.M >= c.N][:2000]
+    p.set_fill(waves[0].fill_ids, waves[0].fill_val)
+    for x in (o, r):
+        assert x.mark_used(waves[0].used_ids) == 0
+    args = (ids, [c.P for c in wl.claims], [c.N for c in wl.claims], waves[0].bt_off, waves[0].bt_ids)
+    assert np.array_equal(o.accept(*args), r.accept(*args))
+    assert np.array_equal(o.materialize(ids), r.materialize(ids))
+    assert np.array_equal(o.offload(ok_ids), r.offload(ok_ids))
+    used, _ = o.pool_state()
+    free = np.nonzero(used == 0)[0].astype(np.uint32)
+    for x in (o, r):
+        x.mark_used(free[40000:])                             # leave 40000 free blocks: about 1300 claims fit
+    sa, sb = o.restore(ok_ids), r.restore(ok_ids)
+    assert np.array_equal(sa, sb) and 0 in sa and 6 in sa
+    first6 = list(sa).index(6)
+    assert all(s == 6 for s in sa[first6:]) and first6 > 1024     # the grant boundary lies beyond the first scan tile
+    p.check_pool_state("partial grant", bytes_too=False)
+    p.check_events("partial grant")
+    p.close()
