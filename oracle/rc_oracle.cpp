@@ -34,14 +34,24 @@ typedef uint64_t u64;
 typedef uint32_t u32;
 typedef uint8_t u8;
 
-// ---- checksum (build-defined) -------------------------
-static const u64 K1 = 0x9E3779B97F4A7C15ull;  // 2^64/phi
+// ---- checksum (build-defined, reading R22) ---------------
+// All arithmetic mod 2^64 (products: the full 128 bits), memory read as little-endian u64.
+static const u64 K1 = 0x9E3779B97F4A7C15ull;  // floor(2^64/phi)
 static const u64 K2 = 0x6A09E667F3BCC909ull;  // frac(sqrt 2) | 1
 static const u64 KA = 0xBB67AE8584CAA73Bull;  // frac(sqrt 3), odd
 static const u64 K3 = 0x3C6EF372FE94F82Bull;  // frac(sqrt 5)
+static const u64 K4 = 0xA54FF53A5F1D36F1ull;  // frac(sqrt 7)
+static const u64 K5 = 0x510E527FADE682D1ull;  // frac(sqrt 11)
 
 static u64 mixL(u64 x) { u64 y = x ^ (x >> 32); y *= K2; return y ^ (y >> 29); }
 static u64 mixF(u64 x) { u64 y = mixL(x); y *= K1; return y ^ (y >> 32); }
+// mum(x, y): the 128-bit product x*y folded to 64 bits, low half XOR high half.  Unlike a
+// multiplication by an odd constant mod 2^64 it carries a difference in ANY input bit into
+// low and high output bits alike, and by an amount that depends on the other factor.
+static u64 mum(u64 x, u64 y) {
+  unsigned __int128 p = (unsigned __int128)x * y;
+  return (u64)p ^ (u64)(p >> 64);
+}
 
 static u64 load64le(const u8* p) {
   u64 v = 0;
@@ -49,27 +59,38 @@ static u64 load64le(const u8* p) {
   return v;
 }
 
-// One page = V = page_bytes/16 vectors of two little-endian u64 words.
-// 256 lanes; lane t folds vectors t, t+256, t+512, ... in increasing order.
-static u64 page_digest(const u8* pg, u64 page_bytes) {
-  u64 V = page_bytes / 16, p = 0;
+// One page = V = page_bytes/16 vectors (a, b) of two little-endian u64 words.
+// 256 lanes; lane t folds vectors t, t+256, t+512, ... in increasing order, in two
+// independent families: h (the checksum) and g (the content-key extension).
+struct Dig2 { u64 d, e; };
+static Dig2 page_digest2(const u8* pg, u64 page_bytes) {
+  u64 V = page_bytes / 16;
+  Dig2 out = {0, 0};
   for (u64 lane = 0; lane < 256; ++lane) {
-    u64 h = (lane + 1) * K1;
+    u64 h = (lane + 1) * K1, g = (lane + 1) * K4;
     for (u64 v = lane; v < V; v += 256) {
-      h = (h ^ load64le(pg + 16 * v)) * K2;
-      h = (h ^ load64le(pg + 16 * v + 8)) * K2;
+      u64 a = load64le(pg + 16 * v), b = load64le(pg + 16 * v + 8);
+      h = mum(a ^ K2, b ^ h);
+      g = mum(b ^ K5, a ^ g);
     }
-    p += mixL(h);
+    out.d += mixL(h);
+    out.e += mixL(g);
   }
-  return p;
+  return out;
 }
 
-// A block in offload order: 2L pages, page g = l*2 + kv.
-static u64 block_digest(const u8* blk, u32 n_pages, u64 page_bytes) {
-  u64 s = 0;
-  for (u32 g = 0; g < n_pages; ++g)
-    s += mixL(page_digest(blk + (u64)g * page_bytes, page_bytes) ^ ((u64)(g + 1) * K3));
-  return mixF(s);
+// A block in offload order: 2L pages, page g = l*2 + kv.  d = the 64-bit per-block checksum that is
+// chained and verified (BASELINE.json north_star (d)); e = a second, independent 64-bit digest of the
+// same bytes: (d, e) is the 128-bit content key of the dedup store, and verify compares it too.
+static Dig2 block_digest2(const u8* blk, u32 n_pages, u64 page_bytes) {
+  u64 s = 0, t = 0;
+  for (u32 g = 0; g < n_pages; ++g) {
+    Dig2 p = page_digest2(blk + (u64)g * page_bytes, page_bytes);
+    s += mixL(p.d ^ ((u64)(g + 1) * K3));
+    t += mixL(p.e ^ ((u64)(g + 1) * K5));
+  }
+  Dig2 out = {mixF(s), mixF(t)};
+  return out;
 }
 
 static u64 chain_seed(u64 claim_id) { return mixF(claim_id ^ K3); }
@@ -98,13 +119,16 @@ struct Event { u64 seq, claim_id; u32 code, aux; u64 arg; };   // 32 bytes
 struct Fault { u64 claim_id; u32 kind, param; };
 struct ClaimInfo { u64 claim_id, chain, host_bytes; u32 state, P, N, M, nb, n_table; };
 
+typedef std::pair<u64, u64> Key;   // 128-bit content key (d, e) of one block
+
 struct Claim {
   u32 state = 0, P = 0, N = 0, M = 0, nb = 0, policy = 0;
   std::vector<u32> bt;        // current block table
-  std::vector<u64> d;         // per-block digests recorded at offload
+  std::vector<u64> d;         // per-block checksums recorded at offload (chained)
+  std::vector<u64> e;         // per-block second digests recorded at offload ((d, e) = content key)
   u64 chain = 0;
   std::vector<u8> host;       // claim-scoped host copy (nb*blk bytes)
-  std::vector<u64> hkeys;     // dedup mode (NEXT-2): the claim's blocks as keys into the content-addressed store
+  std::vector<Key> hkeys;     // dedup mode (NEXT-2): the claim's blocks as keys into the content-addressed store
 };
 
 struct Ctx {
@@ -121,7 +145,7 @@ struct Ctx {
   // NEXT-2: content-addressed host store keyed by block digest, so blocks shared between claims
   // are held (and cross the link) once.  DESIGN.md "Dedup".
   bool dedup = false;
-  std::map<u64, std::pair<std::vector<u8>, u32>> store;   // digest -> (blk bytes, references)
+  std::map<Key, std::pair<std::vector<u8>, u32>> store;   // (d, e) -> (blk bytes, references)
   u64 link_d2h = 0, link_h2d = 0;                          // bytes that have to cross the host link, by definition
   void emit(u64 c, u32 code, u32 aux, u64 arg) {
     Event ev; ev.seq = events.size(); ev.claim_id = c; ev.code = code; ev.aux = aux; ev.arg = arg;
@@ -180,13 +204,13 @@ static void drop_refs(Ctx* c, Claim& cl) {
 static std::vector<u8> host_bytes_of(Ctx* c, const Claim& cl) {     // the claim-logical host copy
   if (!c->dedup) return cl.host;
   std::vector<u8> out;
-  for (u64 k : cl.hkeys) { const auto& b = c->store[k].first; out.insert(out.end(), b.begin(), b.end()); }
+  for (const Key& k : cl.hkeys) { const auto& b = c->store[k].first; out.insert(out.end(), b.begin(), b.end()); }
   return out;
 }
 static u64 host_size_of(Ctx* c, const Claim& cl) { return c->dedup ? (u64)cl.hkeys.size() * c->blk : (u64)cl.host.size(); }
 static void drop_host(Ctx* c, Claim& cl) {
   if (c->dedup) {
-    for (u64 k : cl.hkeys) { auto it = c->store.find(k); if (--it->second.second == 0) { c->store.erase(it); c->host_used -= c->blk; } }
+    for (const Key& k : cl.hkeys) { auto it = c->store.find(k); if (--it->second.second == 0) { c->store.erase(it); c->host_used -= c->blk; } }
     cl.hkeys.clear();
   } else {
     c->host_used -= cl.host.size();
@@ -202,18 +226,23 @@ static void do_offload_one(Ctx* c, u64 id, Claim& cl) {
   for (u32 i = 0; i < cl.nb; ++i)
     for (u32 g = 0; g < G; ++g)
       memcpy(cl.host.data() + (u64)i * c->blk + (u64)g * c->page, c->page_ptr(g, cl.bt[i]), c->page);
-  cl.d.resize(cl.nb);
-  for (u32 i = 0; i < cl.nb; ++i) cl.d[i] = block_digest(cl.host.data() + (u64)i * c->blk, G, c->page);
+  cl.d.resize(cl.nb); cl.e.resize(cl.nb);
+  for (u32 i = 0; i < cl.nb; ++i) {
+    Dig2 x = block_digest2(cl.host.data() + (u64)i * c->blk, G, c->page);
+    cl.d[i] = x.d; cl.e[i] = x.e;
+  }
   cl.chain = chain_of(id, cl.d.data(), cl.nb);
   if (c->dedup) {                                         // keep one copy per distinct block content
+    cl.hkeys.clear();
     for (u32 i = 0; i < cl.nb; ++i) {
-      auto it = c->store.find(cl.d[i]);
+      const Key key(cl.d[i], cl.e[i]);
+      cl.hkeys.push_back(key);
+      auto it = c->store.find(key);
       if (it != c->store.end()) { it->second.second++; continue; }
       const u8* b = cl.host.data() + (u64)i * c->blk;
-      c->store[cl.d[i]] = std::make_pair(std::vector<u8>(b, b + c->blk), 1u);
+      c->store[key] = std::make_pair(std::vector<u8>(b, b + c->blk), 1u);
       c->host_used += c->blk; c->link_d2h += c->blk;
     }
-    cl.hkeys = cl.d;
     std::vector<u8>().swap(cl.host);
   } else {
     c->host_used += cl.host.size(); c->link_d2h += cl.host.size();
@@ -279,7 +308,7 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_i
     }
   }
   bool any_served = false;
-  std::set<u64> call_keys;
+  std::set<Key> call_keys;
   std::vector<u64> blocking;
   for (u32 k = 0; k < n; ++k) {
     if (!served[k]) continue;
@@ -296,19 +325,20 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_i
     } else {
       std::vector<u8> staged = host_bytes_of(c, cl);    // host copy itself stays intact
       if (c->dedup && flt.kind != FK_BITFLIP) {           // one transfer per distinct block of the call; a corrupted
-        for (u64 k : cl.hkeys) if (call_keys.insert(k).second) c->link_h2d += c->blk;   // copy is private to its claim
+        for (const Key& k : cl.hkeys) if (call_keys.insert(k).second) c->link_h2d += c->blk;   // copy is private to its claim
       } else c->link_h2d += staged.size();
       if (flt.kind == FK_BITFLIP && !staged.empty()) staged[flt.param % staged.size()] ^= 0x01;
-      std::vector<u64> d2(cl.nb);
+      std::vector<u64> d2(cl.nb), e2(cl.nb);
       for (u32 i = 0; i < cl.nb; ++i) {
         for (u32 g = 0; g < G; ++g)
           memcpy(c->page_ptr(g, cl.bt[i]), staged.data() + (u64)i * c->blk + (u64)g * c->page, c->page);
         u32 rem = cl.M - i * c->BS;
         c->fill[cl.bt[i]] = (u8)(rem < c->BS ? rem : c->BS);
-        d2[i] = block_digest(staged.data() + (u64)i * c->blk, G, c->page);
+        Dig2 x = block_digest2(staged.data() + (u64)i * c->blk, G, c->page);
+        d2[i] = x.d; e2[i] = x.e;
       }
       bool found = false;
-      for (u32 i = 0; i < cl.nb && !found; ++i) if (d2[i] != cl.d[i]) { bad = i; found = true; }
+      for (u32 i = 0; i < cl.nb && !found; ++i) if (d2[i] != cl.d[i] || e2[i] != cl.e[i]) { bad = i; found = true; }
       ok = !found && chain_of(id, d2.data(), cl.nb) == cl.chain;
     }
     drop_host(c, cl);
@@ -324,7 +354,7 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_i
       else if (request_id == 0) c->emit(id, EV_ACTIVE_REQUEST_REFUSED, 1, id);    // blocking_claim_ids=[C]: aux = count, arg = C
       else blocking.push_back(id);
       for (u32 b : cl.bt) { c->used[b] = 0; c->ref[b] = 0; c->fill[b] = 0; }
-      cl.bt.clear(); cl.d.clear();
+      cl.bt.clear(); cl.d.clear(); cl.e.clear();
       cl.state = cl.policy == POL_DEMOTE ? CS_DEMOTED : (cl.policy == POL_EXPIRE ? CS_EXPIRED : CS_REFUSED);   // terminal
       st[k] = ST_RESTORE_FAILED;
     }
@@ -433,11 +463,11 @@ int rco_claim_blocks(void* h, u64 id, u32* ids, u32 cap, u32* n) {
   for (u32 i = 0; i < *n && i < cap; ++i) ids[i] = it->second.bt[i];
   return E_OK;
 }
-int rco_claim_digests(void* h, u64 id, u64* d, u32 cap, u32* n) {
+int rco_claim_digests(void* h, u64 id, u64* d, u64* e, u32 cap, u32* n) {   // e may be NULL
   Ctx* c = (Ctx*)h; auto it = c->claims.find(id);
   if (it == c->claims.end()) return E_INVALID;
   *n = (u32)it->second.d.size();
-  for (u32 i = 0; i < *n && i < cap; ++i) d[i] = it->second.d[i];
+  for (u32 i = 0; i < *n && i < cap; ++i) { d[i] = it->second.d[i]; if (e) e[i] = it->second.e[i]; }
   return E_OK;
 }
 int rco_host_read(void* h, u64 id, void* dst, u64 cap, u64* bytes) {
@@ -468,8 +498,12 @@ int rco_link_bytes(void* h, u64* out2) { Ctx* c = (Ctx*)h; out2[0] = c->link_d2h
 // checksum primitives, exported so the pins can reach each one directly
 u64 rco_mixL(u64 x) { return mixL(x); }
 u64 rco_mixF(u64 x) { return mixF(x); }
-u64 rco_page_digest(const void* p, u64 page_bytes) { return page_digest((const u8*)p, page_bytes); }
-u64 rco_block_digest(const void* p, u32 n_pages, u64 page_bytes) { return block_digest((const u8*)p, n_pages, page_bytes); }
+u64 rco_mum(u64 x, u64 y) { return mum(x, y); }
+// which: 0 = the checksum family (d), 1 = the key-extension family (e)
+u64 rco_page_digest(const void* p, u64 page_bytes, int which) { Dig2 x = page_digest2((const u8*)p, page_bytes); return which ? x.e : x.d; }
+u64 rco_block_digest(const void* p, u32 n_pages, u64 page_bytes, int which) {
+  Dig2 x = block_digest2((const u8*)p, n_pages, page_bytes); return which ? x.e : x.d;
+}
 u64 rco_chain_of(u64 id, const u64* d, u32 nb) { return chain_of(id, d, nb); }
 
 }  // extern "C"

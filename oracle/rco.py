@@ -46,12 +46,13 @@ def lib():
     global _lib
     if _lib is None:
         _lib = C.CDLL(build())
-        for name in ("rco_mixL", "rco_mixF", "rco_page_digest", "rco_block_digest", "rco_chain_of"):
+        for name in ("rco_mixL", "rco_mixF", "rco_mum", "rco_page_digest", "rco_block_digest", "rco_chain_of"):
             getattr(_lib, name).restype = C.c_uint64
         _lib.rco_mixL.argtypes = [C.c_uint64]
         _lib.rco_mixF.argtypes = [C.c_uint64]
-        _lib.rco_page_digest.argtypes = [C.c_void_p, C.c_uint64]
-        _lib.rco_block_digest.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64]
+        _lib.rco_mum.argtypes = [C.c_uint64, C.c_uint64]
+        _lib.rco_page_digest.argtypes = [C.c_void_p, C.c_uint64, C.c_int]
+        _lib.rco_block_digest.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_int]
         _lib.rco_chain_of.argtypes = [C.c_uint64, C.c_void_p, C.c_uint32]
     return _lib
 
@@ -76,14 +77,19 @@ def mixF(x):
     return int(lib().rco_mixF(C.c_uint64(x)))
 
 
-def page_digest(page: np.ndarray):
+def mum(x, y):
+    return int(lib().rco_mum(C.c_uint64(x), C.c_uint64(y)))
+
+
+def page_digest(page: np.ndarray, which=0):
+    """which: 0 = the checksum family (d), 1 = the key-extension family (e)."""
     page = np.ascontiguousarray(page).view(np.uint8)
-    return int(lib().rco_page_digest(_p(page), C.c_uint64(page.size)))
+    return int(lib().rco_page_digest(_p(page), C.c_uint64(page.size), which))
 
 
-def block_digest(blk: np.ndarray, n_pages: int):
+def block_digest(blk: np.ndarray, n_pages: int, which=0):
     blk = np.ascontiguousarray(blk).view(np.uint8)
-    return int(lib().rco_block_digest(_p(blk), n_pages, C.c_uint64(blk.size // n_pages)))
+    return int(lib().rco_block_digest(_p(blk), n_pages, C.c_uint64(blk.size // n_pages), which))
 
 
 def chain_of(claim_id, d):
@@ -192,12 +198,13 @@ class Oracle:
             self.L.rco_claim_blocks(self.h, C.c_uint64(cid), _p(buf), buf.size, C.byref(n))
         return buf[: n.value].copy()
 
-    def claim_digests(self, cid):
+    def claim_digests(self, cid, both=False):
+        """The claim's recorded per-block checksums d; both=True: (d, e) with e the key-extension digests."""
         n = C.c_uint32()
-        buf = np.zeros(1 << 16, np.uint64)
-        if self.L.rco_claim_digests(self.h, C.c_uint64(cid), _p(buf), buf.size, C.byref(n)) != 0:
+        buf, buf2 = np.zeros(1 << 16, np.uint64), np.zeros(1 << 16, np.uint64)
+        if self.L.rco_claim_digests(self.h, C.c_uint64(cid), _p(buf), _p(buf2), buf.size, C.byref(n)) != 0:
             return None
-        return buf[: n.value].copy()
+        return (buf[: n.value].copy(), buf2[: n.value].copy()) if both else buf[: n.value].copy()
 
     def host_read(self, cid):
         nbytes = C.c_uint64()
