@@ -93,7 +93,7 @@ typedef struct rc_config {
   void*    stream_h2d;      /* restore: pinned host -> staging copies                                */
   uint32_t mover;           /* RC_MOVER_*                                                            */
   uint32_t grid_ctas;       /* CTAs of a gather / scatter launch; 0 = library default                */
-  uint32_t dedup;           /* NEXT-2: 1 = content-addressed host store keyed by block digest: a block shared
+  uint32_t dedup;           /* NEXT-2: 1 = content-addressed host store keyed by the 128-bit (d, e) digests: a block shared
                                between claims is held and crosses the link once       */
   uint32_t direct_offload;  /* NEXT-4 (experimental): 1 = the gather kernel stores straight into the mapped pinned
                                store (no staging, no copy engine); ignored with dedup                          */
@@ -192,7 +192,9 @@ int rc_release(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* statu
 /* Introspection (tests, parity). */
 int rc_claim_info(rc_ctx* ctx, uint64_t claim_id, rc_claim_info_t* out);
 int rc_claim_blocks(rc_ctx* ctx, uint64_t claim_id, uint32_t* ids, uint32_t cap, uint32_t* n);
-int rc_claim_digests(rc_ctx* ctx, uint64_t claim_id, uint64_t* d, uint32_t cap, uint32_t* n);
+/* d: the recorded per-block checksums (chained into `chain`); e (may be NULL): the second digests -- (d[i], e[i]) is
+ * the 128-bit content key of block i (DESIGN.md "Checksum" R22). */
+int rc_claim_digests(rc_ctx* ctx, uint64_t claim_id, uint64_t* d, uint64_t* e, uint32_t cap, uint32_t* n);
 int rc_host_read(rc_ctx* ctx, uint64_t claim_id, void* dst, uint64_t cap, uint64_t* bytes);
 int rc_pool_state(rc_ctx* ctx, uint8_t* used /*NB*/, uint32_t* ref /*NB*/);
 int rc_stats_get(rc_ctx* ctx, rc_stats* out);
@@ -203,9 +205,10 @@ int rc_stats_reset(rc_ctx* ctx);
 int rc_measure_link(rc_ctx* ctx, uint64_t bytes, int direction, int reps, double* gbs);
 
 /* Standalone checksum of `n_blocks` contiguous blocks at DEVICE address src (offload order):
- * the read-only digest pass used to report the checksum against the HBM roofline.  digests is
- * a HOST array (may be NULL); ms (may be NULL) receives the device time of the digest kernel. */
-int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64_t* digests, float* ms);
+ * the read-only digest pass used to report the checksum against the HBM roofline.  digests / digests2
+ * are HOST arrays (d and e of each block; either may be NULL); ms (may be NULL) receives the device
+ * time of the digest kernel. */
+int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64_t* digests, uint64_t* digests2, float* ms);
 
 /* NEXT-1: the paper's artifact analyzer as a device pass.  Validates an event
  * array (HOST, n records in stream order; may contain the harness marker codes RC_EV_USE and

@@ -76,6 +76,9 @@ struct ExtAlloc {
   }
 };
 
+typedef std::pair<u64, u64> Key;          // 128-bit content key of a block: (checksum d, second digest e)
+struct KeyHash { size_t operator()(const Key& k) const { return (size_t)(k.first ^ (k.second * 0x9E3779B97F4A7C15ull)); } };
+
 struct Claim {
   u64 id = 0, chain = 0;
   u32 state = 0, P = 0, N = 0, M = 0, nb = 0, policy = 0;
@@ -83,7 +86,7 @@ struct Claim {
   u32 dg_off = 0, dg_len = 0;            // recorded digests
   std::vector<std::pair<u64, u64>> host; // host-store extents in blk units
   std::vector<u32> hslots;               // dedup mode: host-store slot of each block
-  std::vector<u64> hkeys;                // dedup mode: content key (digest) of each block
+  std::vector<Key> hkeys;                // dedup mode: 128-bit content key (d, e) of each block
   bool busy = false;
 };
 
@@ -109,13 +112,13 @@ struct rc_ctx {
   cudaStream_t meta = 0, gather = 0, d2h = 0, scatter = 0, h2d = 0, util = 0;
   bool own[5] = {false, false, false, false, false};
   u8* pool = nullptr; u8* fill = nullptr;
-  u8* d_used = nullptr; u32* d_ref = nullptr; u32* d_bt = nullptr; u64* d_dg = nullptr;
+  u8* d_used = nullptr; u32* d_ref = nullptr; u32* d_bt = nullptr; u64* d_dg = nullptr; u64* d_dg2 = nullptr;
   Event* d_ring = nullptr; u64* d_evcount = nullptr; u32* d_bitmaps = nullptr; u32* d_up = nullptr;
   u32* d_counters = nullptr; u32* d_alloc = nullptr; u64* d_flip = nullptr;
   Desc* d_desc[3] = {}; Res* d_res[3] = {}; u32* d_off[3] = {};
   Desc* h_desc[3] = {}; Res* h_res[3] = {};
   u32* h_up = nullptr; u64* h_flip = nullptr; u32* h_counters = nullptr;
-  u32* d_phys[2] = {}; u64* d_dtmp[2] = {};
+  u32* d_phys[2] = {}; u64* d_dtmp[2] = {}; u64* d_etmp[2] = {};
   std::vector<u8*> staging[2]; std::vector<u64*> part[2];
   std::vector<cudaEvent_t> ev_free[2], ev_ready[2];
   std::vector<bool> slot_used[2];
@@ -135,9 +138,9 @@ struct rc_ctx {
   // NEXT-2: content-addressed host store
   u64 request_id = 0;                                    // NEXT-3: the reuse request of the restore being begun (0: per-claim)
   bool dedup = false;
-  std::unordered_map<u64, std::pair<u32, u32>> store;    // digest -> (slot, references)
+  std::unordered_map<Key, std::pair<u32, u32>, KeyHash> store;   // (d, e) -> (slot, references)
   std::vector<u32> pending_free;                         // slots of an in-flight restore, recycled at its completion
-  u64* h_dig = nullptr; u32 *h_iw = nullptr, *h_ispos = nullptr, *d_iw = nullptr, *d_ispos = nullptr;
+  u64 *h_dig = nullptr, *h_dig2 = nullptr; u32 *h_iw = nullptr, *h_ispos = nullptr, *d_iw = nullptr, *d_ispos = nullptr;
   // NEXT-4 (first half): gather straight into the mapped pinned store, no staging, no copy engine
   bool direct = false; u8* h_store_dev = nullptr; u32 *h_hpos = nullptr, *d_hpos = nullptr;
 };
@@ -205,13 +208,13 @@ extern "C" int rc_destroy(rc_ctx* c) {
   cudaDeviceSynchronize();
   auto F = [](void* p) { if (p) cudaFree(p); };
   auto FH = [](void* p) { if (p) cudaFreeHost(p); };
-  F(c->d_used); F(c->d_ref); F(c->d_bt); F(c->d_dg); F(c->d_ring); F(c->d_evcount); F(c->d_bitmaps); F(c->d_up);
+  F(c->d_used); F(c->d_ref); F(c->d_bt); F(c->d_dg); F(c->d_dg2); F(c->d_ring); F(c->d_evcount); F(c->d_bitmaps); F(c->d_up);
   F(c->d_counters); F(c->d_alloc); F(c->d_flip);
   for (int i = 0; i < 3; ++i) { F(c->d_desc[i]); F(c->d_res[i]); F(c->d_off[i]); FH(c->h_desc[i]); FH(c->h_res[i]); }
-  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store); FH(c->h_dig); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
+  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
   F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
   for (int d = 0; d < 2; ++d) {
-    F(c->d_phys[d]); F(c->d_dtmp[d]);
+    F(c->d_phys[d]); F(c->d_dtmp[d]); F(c->d_etmp[d]);
     for (auto p : c->staging[d]) F(p);
     for (auto p : c->part[d]) F(p);
     for (auto e : c->ev_free[d]) cudaEventDestroy(e);
@@ -276,6 +279,7 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   CC(cudaMalloc(&c->d_ref, NB * 4), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_bt, cap * 4), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_dg, cap * 8), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_dg2, cap * 8), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_ring, (u64)cfg->max_events * sizeof(Event)), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_evcount, 8), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_bitmaps, (u64)c->accept_ctas * ((NB + 31) / 32) * 4), RC_ERR_NOMEM);
@@ -305,6 +309,7 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   }
   if (c->dedup) {
     CC(cudaHostAlloc(&c->h_dig, cap * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_dig2, cap * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
     CC(cudaHostAlloc(&c->h_iw, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
     CC(cudaHostAlloc(&c->h_ispos, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_iw, cap * 4), RC_ERR_NOMEM);
@@ -313,12 +318,13 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   for (int d = 0; d < 2; ++d) {
     CC(cudaMalloc(&c->d_phys[d], cap * 4), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_dtmp[d], cap * 8), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_etmp[d], cap * 8), RC_ERR_NOMEM);
     c->staging[d].assign(c->R, nullptr); c->part[d].assign(c->R, nullptr);
     c->ev_free[d].assign(c->R, nullptr); c->ev_ready[d].assign(c->R, nullptr);
     c->slot_used[d].assign(c->R, false);
     for (u32 r = 0; r < c->R; ++r) {
       CC(cudaMalloc(&c->staging[d][r], c->chunk_blocks * blk), RC_ERR_NOMEM);
-      CC(cudaMalloc(&c->part[d][r], c->chunk_blocks * c->G * WPC * 8), RC_ERR_NOMEM);
+      CC(cudaMalloc(&c->part[d][r], c->chunk_blocks * c->G * WPC * 16), RC_ERR_NOMEM);
       CC(cudaEventCreateWithFlags(&c->ev_free[d][r], cudaEventDisableTiming), RC_ERR_CUDA);
       CC(cudaEventCreateWithFlags(&c->ev_ready[d][r], cudaEventDisableTiming), RC_ERR_CUDA);
     }
@@ -631,7 +637,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
       CK(cudaEventRecord(t1, c->gather));
       op.t_copy.push_back({t0, t1});                       // the kernel IS the transfer
       op.copy_bytes += (u64)m * c->blk;
-      k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, m, c->G, nullptr);
+      k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, c->d_etmp[0] + w0, m, c->G, nullptr);
       CKL();
       c->st.kernel_launches++;
       continue;
@@ -644,7 +650,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     CK(cudaEventRecord(t1, c->gather));
     op.t_kernel.push_back({t0, t1});
     op.launches++;
-    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, m, c->G, nullptr);
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, c->d_etmp[0] + w0, m, c->G, nullptr);
     CKL();
     c->st.kernel_launches++;
     CK(cudaEventRecord(c->ev_ready[0][slot], c->gather));
@@ -657,7 +663,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     CK(cudaEventRecord(c->ev_free[0][slot], c->d2h));
     c->slot_used[0][slot] = true;
   }
-  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_dtmp[0], c->d_dg);
+  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_dtmp[0], c->d_etmp[0], c->d_dg, c->d_dg2);
   CKL();
   c->st.kernel_launches++;
   CK(cudaEventRecord(c->ev_body_a[0], c->gather));
@@ -823,7 +829,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     CK(cudaEventRecord(t1, c->scatter));
     op.t_kernel.push_back({t0, t1});
     op.launches++;
-    k_block_digest<<<warps_grid(m), 256, 0, c->scatter>>>(c->part[1][slot], c->d_phys[1] + w0, c->d_dtmp[1] + w0, m, c->G, nullptr);
+    k_block_digest<<<warps_grid(m), 256, 0, c->scatter>>>(c->part[1][slot], c->d_phys[1] + w0, c->d_dtmp[1] + w0, c->d_etmp[1] + w0, m, c->G, nullptr);
     CKL();
     c->st.kernel_launches++;
     CK(cudaEventRecord(c->ev_free[1][slot], c->scatter));
@@ -831,7 +837,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   }
   CK(cudaEventRecord(c->ev_body_a[1], c->scatter));
   CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[1], 0));
-  k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_dg, c->d_bt,
+  k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_etmp[1], c->d_dg, c->d_dg2, c->d_bt,
                                                c->d_used, c->d_ref, c->fill, c->cfg.block_size);
   CKL();
   c->st.kernel_launches++;
@@ -1001,7 +1007,7 @@ extern "C" int rc_claim_blocks(rc_ctx* c, uint64_t id, uint32_t* ids, uint32_t c
   }
   return RC_OK;
 }
-extern "C" int rc_claim_digests(rc_ctx* c, uint64_t id, uint64_t* d, uint32_t cap, uint32_t* n) {
+extern "C" int rc_claim_digests(rc_ctx* c, uint64_t id, uint64_t* d, uint64_t* e, uint32_t cap, uint32_t* n) {
   GUARD();
   auto it = c->claims.find(id);
   if (it == c->claims.end() || !n) return RC_ERR_INVALID;
@@ -1010,6 +1016,7 @@ extern "C" int rc_claim_digests(rc_ctx* c, uint64_t id, uint64_t* d, uint32_t ca
   const u32 m = std::min(cap, cl.dg_len);
   if (m && d) {
     CK(cudaMemcpyAsync(d, c->d_dg + cl.dg_off, (u64)m * 8, cudaMemcpyDeviceToHost, c->util));
+    if (e) CK(cudaMemcpyAsync(e, c->d_dg2 + cl.dg_off, (u64)m * 8, cudaMemcpyDeviceToHost, c->util));
     CK(cudaStreamSynchronize(c->util));
   }
   return RC_OK;
@@ -1089,7 +1096,8 @@ extern "C" int rc_measure_link(rc_ctx* c, uint64_t bytes, int direction, int rep
   return RC_OK;
 }
 
-extern "C" int rc_digest_blocks(rc_ctx* c, const void* src, uint32_t n_blocks, uint64_t* digests, float* ms_out) {
+extern "C" int rc_digest_blocks(rc_ctx* c, const void* src, uint32_t n_blocks, uint64_t* digests, uint64_t* digests2,
+                                float* ms_out) {
   GUARD();
   if (!src || ((uintptr_t)src & 15) || n_blocks > c->cap_entries) return RC_ERR_INVALID;
   if (c->ops[0].active) return RC_ERR_BUSY;
@@ -1101,15 +1109,16 @@ extern "C" int rc_digest_blocks(rc_ctx* c, const void* src, uint32_t n_blocks, u
     launch_move<MV_DIGEST>(c, c->gather, (u8*)src + w0 * c->blk, nullptr, c->part[0][0], m);
     CKL();
     CK(cudaEventRecord(t1, c->gather));
-    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][0], nullptr, c->d_dtmp[0] + w0, m, c->G, nullptr);
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][0], nullptr, c->d_dtmp[0] + w0, c->d_etmp[0] + w0, m, c->G, nullptr);
     CKL();
     CK(cudaStreamSynchronize(c->gather));
     float ms = 0;
     CK(cudaEventElapsedTime(&ms, t0, t1));
     total += ms;
   }
-  if (digests && n_blocks) {
-    CK(cudaMemcpyAsync(digests, c->d_dtmp[0], (u64)n_blocks * 8, cudaMemcpyDeviceToHost, c->gather));
+  if (n_blocks && (digests || digests2)) {
+    if (digests) CK(cudaMemcpyAsync(digests, c->d_dtmp[0], (u64)n_blocks * 8, cudaMemcpyDeviceToHost, c->gather));
+    if (digests2) CK(cudaMemcpyAsync(digests2, c->d_etmp[0], (u64)n_blocks * 8, cudaMemcpyDeviceToHost, c->gather));
     CK(cudaStreamSynchronize(c->gather));
   }
   c->ev_pool.push_back(t0); c->ev_pool.push_back(t1);

@@ -1,6 +1,6 @@
 // rc_dedup.inl -- NEXT-2: content-addressed host store.  Included by librc.cu.
 //
-// Blocks are keyed by their 64-bit digest (the one the fused gather computes anyway).  Offload: every block is
+// Blocks are keyed by the 128-bit pair (d, e) of their two digests (both computed by the fused gather anyway).  Offload: every block is
 // gathered and digested at HBM speed as before; per staging chunk the digests come back to the host (8 B per
 // block), and only blocks whose key is not in the store are copied over the link.  Restore: the distinct
 // blocks of the call are staged once (first appearance order) and the scatter kernel reads them through an
@@ -96,10 +96,11 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     CK(cudaEventRecord(t1, c->gather));
     op.t_kernel.push_back({t0, t1});
     op.launches++;
-    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, m, c->G, nullptr);
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, c->d_etmp[0] + w0, m, c->G, nullptr);
     CKL();
     c->st.kernel_launches++;
     CK(cudaMemcpyAsync(c->h_dig + w0, c->d_dtmp[0] + w0, (u64)m * 8, cudaMemcpyDeviceToHost, c->gather));
+    CK(cudaMemcpyAsync(c->h_dig2 + w0, c->d_etmp[0] + w0, (u64)m * 8, cudaMemcpyDeviceToHost, c->gather));
     CK(cudaEventRecord(c->ev_ready[0][slot], c->gather));
     CK(cudaStreamSynchronize(c->gather));                  // the keys decide which blocks cross the link
     CK(cudaStreamWaitEvent(c->d2h, c->ev_ready[0][slot], 0));
@@ -109,7 +110,7 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     for (u64 w = w0; w < w1; ++w) {
       while (ci_claim + 1 < served.size() && first_w[ci_claim + 1] <= w) ++ci_claim;
       Claim& cl = *op.cl[served[ci_claim]];
-      const u64 key = c->h_dig[w];
+      const Key key(c->h_dig[w], c->h_dig2[w]);
       auto it = c->store.find(key);
       u32 hs;
       if (it != c->store.end()) { it->second.second++; hs = it->second.first; }
@@ -133,7 +134,7 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     CK(cudaEventRecord(c->ev_free[0][slot], c->d2h));
     c->slot_used[0][slot] = true;
   }
-  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_dtmp[0], c->d_dg);
+  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_dtmp[0], c->d_etmp[0], c->d_dg, c->d_dg2);
   CKL();
   c->st.kernel_launches++;
   CK(cudaEventRecord(c->ev_body_a[0], c->gather));
@@ -292,7 +293,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
       CK(cudaEventRecord(t1, c->scatter));
       op.t_kernel.push_back({t0, t1});
       op.launches++;
-      k_block_digest<<<warps_grid(m), 256, 0, c->scatter>>>(c->part[1][slot], c->d_phys[1], c->d_dtmp[1], m, c->G, c->d_iw + j0);
+      k_block_digest<<<warps_grid(m), 256, 0, c->scatter>>>(c->part[1][slot], c->d_phys[1], c->d_dtmp[1], c->d_etmp[1], m, c->G, c->d_iw + j0);
       CKL();
       c->st.kernel_launches++;
     }
@@ -302,7 +303,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
   }
   CK(cudaEventRecord(c->ev_body_a[1], c->scatter));
   CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[1], 0));
-  k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_dg, c->d_bt,
+  k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_etmp[1], c->d_dg, c->d_dg2, c->d_bt,
                                                c->d_used, c->d_ref, c->fill, c->cfg.block_size);
   CKL();
   c->st.kernel_launches++;

@@ -29,6 +29,8 @@ constexpr u64 C1 = 0x9E3779B97F4A7C15ull;
 constexpr u64 C2 = 0x6A09E667F3BCC909ull;
 constexpr u64 CA = 0xBB67AE8584CAA73Bull;
 constexpr u64 C3 = 0x3C6EF372FE94F82Bull;
+constexpr u64 C4 = 0xA54FF53A5F1D36F1ull;
+constexpr u64 C5 = 0x510E527FADE682D1ull;
 constexpr u32 SKIP = 0xFFFFFFFFu;       // work item whose transfer was suppressed (XFER_ERROR)
 constexpr int LANES = 256;              // checksum lanes per page == threads per CTA of k_move_hash
 constexpr int WPC = LANES / 32;         // warps per CTA
@@ -88,18 +90,22 @@ __device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
   asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
                :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
-__device__ __forceinline__ u64 fold(u64 h, const uint4& v) {
-  h = (h ^ ((u64)v.x | ((u64)v.y << 32))) * C2;
-  h = (h ^ ((u64)v.z | ((u64)v.w << 32))) * C2;
-  return h;
+// DESIGN.md "Checksum" R22: one 16-byte vector (a, b) per step, two independent lane families.
+//   h = mum(a ^ C2, b ^ h)   (the checksum d)        g = mum(b ^ C5, a ^ g)   (the key extension e)
+// mum = 128-bit product folded low ^ high: mul.lo.u64 + mul.hi.u64 (4 IMAD.WIDE + carries each pair).
+__device__ __forceinline__ u64 mum(u64 x, u64 y) { return (x * y) ^ __umul64hi(x, y); }
+__device__ __forceinline__ void fold2(u64& h, u64& g, const uint4& v) {
+  const u64 a = (u64)v.x | ((u64)v.y << 32), b = (u64)v.z | ((u64)v.w << 32);
+  h = mum(a ^ C2, b ^ h);
+  g = mum(b ^ C5, a ^ g);
 }
 
 // ---------------------------------------------------------------------------------------------
 // K2 / K4: page mover with fused checksum.  One CTA (256 threads = the 256 checksum lanes) per
 // page at a time, grid-stride over the n_items*G pages of a staging chunk.  Thread t moves
 // vectors t, t+256, ... of the page (each warp access = 512 contiguous bytes) and folds them in
-// that order; each warp writes the sum of its 32 lane terms to part[page*8 + warp] -- no block
-// barrier and no atomics in the streaming loop.  MODE 0 gather (pool -> staging), 1 scatter
+// that order; each warp writes the sums of its 32 lane terms (both families) to part[(page*8 + warp)*2 + {0,1}]
+// -- no block barrier and no atomics in the streaming loop.  MODE 0 gather (pool -> staging), 1 scatter
 // (staging -> pool), 2 digest only (read staging).
 // ---------------------------------------------------------------------------------------------
 enum { MV_GATHER = 0, MV_SCATTER = 1, MV_DIGEST = 2 };
@@ -121,7 +127,7 @@ k_move_hash(uint4* __restrict__ pool, uint4* __restrict__ staging, const u32* __
     uint4* sp = staging + (ispos ? ((u64)__ldg(ispos + w) * G + g) : (u64)u) * vpp + t;
     const uint4* src = (MODE == MV_GATHER) ? pp : sp;
     uint4* dst = (MODE == MV_GATHER) ? sp : pp;
-    u64 h = (u64)(t + 1) * C1;
+    u64 h = (u64)(t + 1) * C1, gq = (u64)(t + 1) * C4;
     for (u32 j0 = 0; j0 < vpt; j0 += UNR) {
       uint4 v[UNR];
 #pragma unroll
@@ -131,11 +137,11 @@ k_move_hash(uint4* __restrict__ pool, uint4* __restrict__ staging, const u32* __
       for (int jj = 0; jj < UNR; ++jj)
         if (j0 + jj < vpt) {
           if (MODE != MV_DIGEST) st_stream(dst + (u64)(j0 + jj) * LANES, v[jj]);
-          h = fold(h, v[jj]);
+          fold2(h, gq, v[jj]);
         }
     }
-    const u64 s = warp_sum64(mixL(h));
-    if ((t & 31) == 0) part[(u64)u * WPC + (t >> 5)] = s;
+    const u64 s = warp_sum64(mixL(h)), s2 = warp_sum64(mixL(gq));
+    if ((t & 31) == 0) { u64* o = part + ((u64)u * WPC + (t >> 5)) * 2; o[0] = s; o[1] = s2; }
   }
 }
 
@@ -185,7 +191,7 @@ __device__ __forceinline__ void mbar_arrive(u64* bar) {
 constexpr int TMA_THREADS = LANES + 64;
 
 template <int MODE, int STAGES, int TILE>
-__global__ void __launch_bounds__(TMA_THREADS)
+__global__ void __launch_bounds__(TMA_THREADS, 1)
 k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __restrict__ phys,
                 u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 page_bytes,
                 const u32* __restrict__ iw, const u32* __restrict__ ispos) {
@@ -240,47 +246,48 @@ k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __re
       asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
   } else {                                                 // ---- consumers: lane t folds vectors t, t+256, ...
-    u64 h = 0;
+    u64 h = 0, gq = 0;
     for (u64 q = 0; q < n_tiles; ++q) {
       const u32 s = (u32)(q % STAGES);
       const u32 k = (u32)(q / tpp), tile = (u32)(q - (u64)k * tpp);
-      if (tile == 0) h = (u64)(t + 1) * C1;
+      if (tile == 0) { h = (u64)(t + 1) * C1; gq = (u64)(t + 1) * C4; }
       mbar_wait(&full[s], (u32)((q / STAGES) & 1));
       const uint4* sv = reinterpret_cast<const uint4*>(smem + s * TILE) + t;
 #pragma unroll
-      for (u32 j = 0; j < VT; ++j) h = fold(h, sv[j * LANES]);
-      asm volatile("" :: "l"(h) : "memory");               // the fold consumed the tile: its shared loads have completed
+      for (u32 j = 0; j < VT; ++j) fold2(h, gq, sv[j * LANES]);
+      asm volatile("" :: "l"(h), "l"(gq) : "memory");      // the fold consumed the tile: its shared loads have completed
       __syncwarp();
       if ((t & 31) == 0) mbar_arrive(&empty[s]);           // this warp releases the stage
       if (tile == tpp - 1) {
         bool skip = false;
         const u32 u = blockIdx.x + k * gridDim.x;
         if (MODE != MV_DIGEST) { const u32 w = u / G; skip = __ldg(phys + (iw ? __ldg(iw + w) : w)) == SKIP; }
-        const u64 sum = warp_sum64(mixL(h));
-        if ((t & 31) == 0 && !skip) part[(u64)u * WPC + warp] = sum;
+        const u64 sum = warp_sum64(mixL(h)), sum2 = warp_sum64(mixL(gq));
+        if ((t & 31) == 0 && !skip) { u64* o = part + ((u64)u * WPC + warp) * 2; o[0] = sum; o[1] = sum2; }
       }
     }
   }
 }
 
-// Per-block digest from the warp partial sums: page_digest(g) = sum of its 8 partials,
-// d = mixF( sum_g mixL(page_digest(g) ^ (g+1)*C3) ).  One warp per work item.
+// Per-block digests from the warp partial sums: page_digest(g) = (sum of its 8 partials, per family),
+// d = mixF( sum_g mixL(p_g ^ (g+1)*C3) ),  e = mixF( sum_g mixL(q_g ^ (g+1)*C5) ).  One warp per work item.
 __global__ void k_block_digest(const u64* __restrict__ part, const u32* __restrict__ phys, u64* __restrict__ d_out,
-                               u32 n_items, u32 G, const u32* __restrict__ iw) {
+                               u64* __restrict__ e_out, u32 n_items, u32 G, const u32* __restrict__ iw) {
   const u32 w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (w >= n_items) return;
   const u32 wo = iw ? __ldg(iw + w) : w;            // output (and phys) position of item w
-  if (phys && __ldg(phys + wo) == SKIP) { if (lane == 0) d_out[wo] = 0; return; }
-  u64 s = 0;
+  if (phys && __ldg(phys + wo) == SKIP) { if (lane == 0) { d_out[wo] = 0; e_out[wo] = 0; } return; }
+  u64 s = 0, t = 0;
   for (u32 g = lane; g < G; g += 32) {
-    const u64* p = part + ((u64)w * G + g) * WPC;
-    u64 pd = 0;
+    const u64* p = part + ((u64)w * G + g) * (WPC * 2);
+    u64 pd = 0, qd = 0;
 #pragma unroll
-    for (int i = 0; i < WPC; ++i) pd += p[i];
+    for (int i = 0; i < WPC; ++i) { pd += p[2 * i]; qd += p[2 * i + 1]; }
     s += mixL(pd ^ ((u64)(g + 1) * C3));
+    t += mixL(qd ^ ((u64)(g + 1) * C5));
   }
-  s = warp_sum64(s);
-  if (lane == 0) d_out[wo] = mixF(s);
+  s = warp_sum64(s); t = warp_sum64(t);
+  if (lane == 0) { d_out[wo] = mixF(s); e_out[wo] = mixF(t); }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -388,7 +395,8 @@ __device__ __forceinline__ u64 chain_tile(u64 h, u64 d, bool valid) {
 }
 
 __global__ void k_chain(const Desc* __restrict__ desc, Res* __restrict__ res, u32 n, const u32* __restrict__ off,
-                        const u64* __restrict__ d_tmp, u64* __restrict__ dg) {
+                        const u64* __restrict__ d_tmp, const u64* __restrict__ e_tmp, u64* __restrict__ dg,
+                        u64* __restrict__ dg2) {
   const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (k >= n) return;
   const Desc d = desc[k];
@@ -398,7 +406,7 @@ __global__ void k_chain(const Desc* __restrict__ desc, Res* __restrict__ res, u3
     const u32 i = base + lane;
     const bool valid = i < d.nb;
     const u64 x = valid ? d_tmp[off[k] + i] : 0;
-    if (valid) dg[d.dg_off + i] = x;
+    if (valid) { dg[d.dg_off + i] = x; dg2[d.dg_off + i] = e_tmp[off[k] + i]; }
     h = chain_tile(h, x, valid);
   }
   if (lane == 0) res[k] = Res{R_OK | R_SERVED, d.nb, h};
@@ -456,7 +464,8 @@ __global__ void k_restore_plan(const Desc* __restrict__ desc, Res* __restrict__ 
 // transfer was not suppressed, no block differs and the recomputed chain equals the recorded one.
 // ok: fill of the new blocks := leading tokens they hold.  not ok: the new blocks are freed.
 __global__ void k_verify(const Desc* __restrict__ desc, Res* __restrict__ res, u32 n, const u32* __restrict__ off,
-                         const u64* __restrict__ d_tmp, const u64* __restrict__ dg, const u32* __restrict__ bt,
+                         const u64* __restrict__ d_tmp, const u64* __restrict__ e_tmp, const u64* __restrict__ dg,
+                         const u64* __restrict__ dg2, const u32* __restrict__ bt,
                          u8* __restrict__ used, u32* __restrict__ ref, u8* __restrict__ fill, u32 BS) {
   const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (k >= n) return;
@@ -470,7 +479,7 @@ __global__ void k_verify(const Desc* __restrict__ desc, Res* __restrict__ res, u
       const u32 i = base + lane;
       const bool valid = i < d.nb;
       const u64 x = valid ? d_tmp[off[k] + i] : 0;
-      const u32 mm = __ballot_sync(0xFFFFFFFFu, valid && x != dg[d.dg_off + i]);
+      const u32 mm = __ballot_sync(0xFFFFFFFFu, valid && (x != dg[d.dg_off + i] || e_tmp[off[k] + i] != dg2[d.dg_off + i]));
       if (mm && bad == 0xFFFFFFFFu) bad = base + __ffs(mm) - 1;
       h = chain_tile(h, x, valid);
     }

@@ -242,13 +242,13 @@ class RC:
         self._ck(self.L.rc_claim_blocks(self.h, C.c_uint64(cid), _p(buf), buf.size, C.byref(n)), "rc_claim_blocks")
         return buf[: n.value].copy()
 
-    def claim_digests(self, cid):
+    def claim_digests(self, cid, both=False):
         n = C.c_uint32()
-        if self.L.rc_claim_digests(self.h, C.c_uint64(cid), None, 0, C.byref(n)) != 0:
+        if self.L.rc_claim_digests(self.h, C.c_uint64(cid), None, None, 0, C.byref(n)) != 0:
             return None
-        buf = np.zeros(max(1, n.value), np.uint64)
-        self._ck(self.L.rc_claim_digests(self.h, C.c_uint64(cid), _p(buf), buf.size, C.byref(n)), "rc_claim_digests")
-        return buf[: n.value].copy()
+        buf, buf2 = np.zeros(max(1, n.value), np.uint64), np.zeros(max(1, n.value), np.uint64)
+        self._ck(self.L.rc_claim_digests(self.h, C.c_uint64(cid), _p(buf), _p(buf2), buf.size, C.byref(n)), "rc_claim_digests")
+        return (buf[: n.value].copy(), buf2[: n.value].copy()) if both else buf[: n.value].copy()
 
     def host_read(self, cid):
         nbytes = C.c_uint64()
@@ -277,12 +277,12 @@ class RC:
         self._ck(self.L.rc_measure_link(self.h, C.c_uint64(nbytes), direction, reps, C.byref(g)), "rc_measure_link")
         return g.value
 
-    def digest_blocks(self, src_ptr, n_blocks, want=True):
-        d = np.zeros(n_blocks, np.uint64)
+    def digest_blocks(self, src_ptr, n_blocks, want=True, both=False):
+        d, e = np.zeros(n_blocks, np.uint64), np.zeros(n_blocks, np.uint64)
         ms = C.c_float()
-        self._ck(self.L.rc_digest_blocks(self.h, C.c_void_p(src_ptr), n_blocks, _p(d) if want else None, C.byref(ms)),
-                 "rc_digest_blocks")
-        return d, ms.value
+        self._ck(self.L.rc_digest_blocks(self.h, C.c_void_p(src_ptr), n_blocks, _p(d) if want else None,
+                                         _p(e) if want else None, C.byref(ms)), "rc_digest_blocks")
+        return ((d, e) if both else d), ms.value
 
 
 def validate_trace(events, want_claims=True):

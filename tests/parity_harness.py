@@ -73,7 +73,9 @@ class Pair:
                 continue
             assert np.array_equal(self.o.claim_blocks(cid), self.r.claim_blocks(cid)), "%s: table %x" % (what, cid)
             if digests:
-                assert np.array_equal(self.o.claim_digests(cid), self.r.claim_digests(cid)), "%s: digests %x" % (what, cid)
+                (da, ea), (db, eb) = self.o.claim_digests(cid, both=True), self.r.claim_digests(cid, both=True)
+                assert np.array_equal(da, db), "%s: digests d %x" % (what, cid)
+                assert np.array_equal(ea, eb), "%s: digests e %x" % (what, cid)
             if host:
                 ha, hb = self.o.host_read(cid), self.r.host_read(cid)
                 assert ha.size == hb.size and np.array_equal(ha, hb), "%s: host bytes %x" % (what, cid)

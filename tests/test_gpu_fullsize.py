@@ -48,9 +48,10 @@ def test_config1_full_size_bench_configuration():
             info = r.claim_info(c.claim_id)
             hb = r.host_read(c.claim_id)
             assert np.array_equal(hb, before[c.claim_id][: info["nb"]].cpu().numpy().reshape(-1))   # host bytes = gather
-            d = r.claim_digests(c.claim_id)
+            d, e = r.claim_digests(c.claim_id, both=True)
             for i in rng.choice(info["nb"], min(4, info["nb"]), replace=False):                    # oracle, block by block
-                assert int(d[i]) == rco.block_digest(hb[i * g.blk_bytes:(i + 1) * g.blk_bytes], 2 * g.layers)
+                assert int(d[i]) == rco.block_digest(hb[i * g.blk_bytes:(i + 1) * g.blk_bytes], 2 * g.layers, 0)
+                assert int(e[i]) == rco.block_digest(hb[i * g.blk_bytes:(i + 1) * g.blk_bytes], 2 * g.layers, 1)
             assert info["chain"] == rco.chain_of(c.claim_id, d)
 
     def check_restored(cl, st, before):

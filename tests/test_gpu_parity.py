@@ -214,10 +214,11 @@ def test_standalone_digest_matches_oracle():
     g = wl.geom
     p = Pair(wl, 1 << 30, chunk_blocks=6)
     x = torch.randint(0, 256, (20 * g.blk_bytes,), dtype=torch.uint8, device="cuda")
-    d, ms = p.r.digest_blocks(x.data_ptr(), 20)
+    (d, e), ms = p.r.digest_blocks(x.data_ptr(), 20, both=True)
     xh = x.cpu().numpy()
-    want = [rco.block_digest(xh[i * g.blk_bytes:(i + 1) * g.blk_bytes], 2 * g.layers) for i in range(20)]
-    assert [int(v) for v in d] == want
+    for which, got in ((0, d), (1, e)):
+        want = [rco.block_digest(xh[i * g.blk_bytes:(i + 1) * g.blk_bytes], 2 * g.layers, which) for i in range(20)]
+        assert [int(v) for v in got] == want
     p.close()
 
 
@@ -469,4 +470,63 @@ def test_large_batch_multi_tile_scans():
     assert all(s == 6 for s in sa[first6:]) and first6 > 1024     # the grant boundary lies beyond the first scan tile
     p.check_pool_state("partial grant", bytes_too=False)
     p.check_events("partial grant")
+    p.close()
+
+
+def test_predicate_on_random_non_monotone_fill():
+    """500 claims whose fill vectors are NOT 'full blocks, one partial, zeros': holes followed by full blocks, a zero
+    first block, fill above the token count of a short last block.  M is the LEADING run of materialized tokens
+    (P:L25 'leading-prefix-at-least-448'): k_pred must agree with the oracle, and both with the token-level definition
+    restated here; a predicate that summed fills would differ on most of these claims."""
+    wl = W.make_workload(0, n_claims=500, pool_blocks=16384)
+    g = wl.geom
+    BS = g.block_size
+    wave = W.plan_waves(wl, 1 << 40)[0]
+    rng = np.random.default_rng(23)
+    fill = np.zeros(g.pool_blocks, np.uint8)
+    want_M, differs = [], 0
+    for k, c in enumerate(wl.claims):
+        c.fault = None
+        tab = wave.bt_ids[wave.bt_off[k]:wave.bt_off[k + 1]]
+        nt = len(tab)
+        f = rng.integers(0, BS + 1, nt)                                    # arbitrary fills everywhere ...
+        kind = k % 5
+        lead = nt if kind == 0 else (0 if kind == 1 else int(rng.integers(max(0, nt - 6), nt + 1)))
+        f[:lead] = BS                                                      # ... behind `lead` complete blocks
+        if kind == 2 and lead < nt:
+            f[lead] = int(rng.integers(0, BS))                             # the hole
+            f[lead + 1:] = BS                                              # and full blocks after it
+        if kind == 3:
+            f[-1] = BS                                                     # fill above the tokens of the short last block
+        fill[tab] = f
+        M = next((t for t in range(c.P) if not (t % BS) < f[t // BS]), c.P)
+        want_M.append(M)
+        differs += int(sum(min(int(f[i]), min(BS, c.P - i * BS)) for i in range(nt)) != M)
+    assert differs > 200
+    p = Pair(wl, 1 << 32, chunk_blocks=512)
+    o, r = p.o, p.r
+    p.set_fill(np.arange(g.pool_blocks), fill)
+    ids = [c.claim_id for c in wl.claims]
+    for x in (o, r):
+        assert x.mark_used(wave.used_ids) == 0
+    args = (ids, [c.P for c in wl.claims], [c.N for c in wl.claims], wave.bt_off, wave.bt_ids)
+    assert np.array_equal(o.accept(*args), r.accept(*args))
+    sa, sb = o.materialize(ids), r.materialize(ids)
+    assert np.array_equal(sa, sb)
+    assert [int(s) for s in sa] == [0 if M >= c.N else 1 for M, c in zip(want_M, wl.claims)]
+    assert 100 < int((sa == 0).sum()) < 400
+    for c, M, s in zip(wl.claims, want_M, sa):
+        if s == 0:
+            assert r.claim_info(c.claim_id)["M"] == M == o.claim_info(c.claim_id)["M"]
+    p.check_claims(ids, "materialize", digests=False)
+    sa, sb = o.offload(ids), r.offload(ids)
+    assert np.array_equal(sa, sb)
+    p.check_claims(ids, "offload", host=True)
+    p.poison_free()
+    assert np.array_equal(o.restore(ids), r.restore(ids))
+    p.check_claims(ids, "restore")
+    p.check_pool_state("restore")                                          # fill of restored blocks = min(BS, M - i*BS)
+    ev = p.check_events("random fill")
+    assert [int(e["aux"]) for e in ev if int(e["code"]) == 2] == [M for M, s in zip(want_M, sa) if s != 3 and M >= 448]
+    assert V.validate(ev)[0]
     p.close()

@@ -92,10 +92,45 @@ def test_dedup_events_and_statuses_equal_the_plain_store():
 def test_dedup_host_space_is_granted_by_worst_case_then_charged_by_content():
     o, wl, wave, view, ids = build(True, host=70 * W.GEOMS[0].blk_bytes)
     st = o.offload(ids)
-    nbs = [o.claim_info(c)["nb"] for c in ids]
-    # the grant assumes every block is new: claim k is served iff host_used + nb_k*blk <= cap at its turn
+    # SURVEY 8(c).2 offload: claims are served in batch order while the running sum of nb*blk fits the host store
+    # that was free at call entry -- every block counted as new; the first claim that does not fit and all later ones
+    # get NO_HOST_SPACE
     assert list(st[:2]) == [0, 0] and 7 in list(st)
     first_refused = list(st).index(7)
     assert all(s == 7 for s in st[first_refused:])                              # prefix rule (R7) unchanged
     assert o.stats()["host_used"] <= 70 * wl.geom.blk_bytes
     assert o.set_dedup(False) != 0                                             # refused while bytes are held
+
+
+def _three_claims(host_blocks, dedup):
+    """Tiny geometry; claims 1 and 2 name the SAME 28 physical blocks (identical content), claim 3 names 28 others."""
+    g = W.GEOMS[0]
+    pool = W.pool_host(g)
+    fill = np.zeros(g.pool_blocks, np.uint8)
+    fill[:56] = g.block_size
+    o = rco.Oracle(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, pool, fill,
+                   host_blocks * g.blk_bytes)
+    assert o.set_dedup(dedup) == 0
+    o.mark_used(np.arange(56))
+    t = list(range(28))
+    assert not o.accept([1, 2, 3], [448] * 3, [448] * 3, [0, 28, 56, 84], t + t + list(range(28, 56))).any()
+    assert not o.materialize([1, 2, 3]).any()
+    return o, g
+
+
+def test_dedup_grant_rule_is_the_call_entry_prefix_sum_not_the_content_charge():
+    """The one input on which the two candidate grant rules differ.  Rule taken (DESIGN 11, from
+    SURVEY 8(c).2 "served while the running sum of nb*blk fits the free host store ... a pure prefix-sum rule"): the
+    sum counts every block as new, so with room for 83 blocks the third claim (28+28+28 = 84) is refused although the
+    store would hold only 56 blocks afterwards.  A content-charged grant (host_used as it stands at the claim's turn
+    + nb*blk: 28 + 28 = 56 <= 83) would serve it."""
+    o, g = _three_claims(83, True)
+    assert o.offload([1, 2, 3]).tolist() == [0, 0, 7]
+    assert o.stats()["host_used"] == 28 * g.blk_bytes and o.link_bytes()[0] == 28 * g.blk_bytes   # charged by content
+    assert o.offload([3]).tolist() == [0]                  # a later call sees what is really held: 28 + 28 <= 83
+    assert o.stats()["host_used"] == 56 * g.blk_bytes
+    o, g = _three_claims(84, True)
+    assert o.offload([1, 2, 3]).tolist() == [0, 0, 0]
+    o, g = _three_claims(83, False)                        # the plain store agrees on the statuses: same rule, R7
+    assert o.offload([1, 2, 3]).tolist() == [0, 0, 7]
+    assert o.stats()["host_used"] == 56 * g.blk_bytes
