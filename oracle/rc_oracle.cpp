@@ -104,11 +104,13 @@ static u64 chain_of(u64 claim_id, const u64* d, u32 nb) {
 enum { EV_ACCEPTED = 1, EV_MATERIALIZED = 2, EV_OFFLOADED = 3, EV_RESTORE_REQUIRED = 4,
        EV_LOAD_FAILED = 5, EV_RESTORED = 6, EV_RESTORATION_FAILED = 7,
        EV_ACTIVE_REQUEST_REFUSED = 8,
-       EV_DEMOTED = 9, EV_EXPIRED = 10 };   // NEXT-3: the other claim-scoped outcomes of a failed restoration (Table "offloadable")
+       EV_DEMOTED = 9, EV_EXPIRED = 10,     // NEXT-3: the other claim-scoped outcomes of a failed restoration (Table "offloadable")
+       EV_CONFLICT_REFUSED = 11 };          // NEXT-3: active_request_refused(blocking_claim_ids) under hard protection
 enum { POL_REFUSE = 0, POL_DEMOTE = 1, POL_EXPIRE = 2 };
 static const u32 REQ_FLAG = 0x80000000u;     // REFUSED.aux of a request-level refusal: flag | size of blocking_claim_ids
 enum { ST_OK = 0, ST_PRED_FALSE = 1, ST_UNKNOWN_CLAIM = 2, ST_BAD_STATE = 3, ST_DUPLICATE_ID = 4,
-       ST_BAD_TABLE = 5, ST_NO_FREE_BLOCKS = 6, ST_NO_HOST_SPACE = 7, ST_RESTORE_FAILED = 8 };
+       ST_BAD_TABLE = 5, ST_NO_FREE_BLOCKS = 6, ST_NO_HOST_SPACE = 7, ST_RESTORE_FAILED = 8,
+       ST_PROTECTED_CONFLICT = 9 };
 enum { CS_ACCEPTED = 1, CS_MATERIALIZED = 2, CS_OFFLOADED = 3, CS_RESIDENT_AGAIN = 4, CS_REFUSED = 5,
        CS_DEMOTED = 6, CS_EXPIRED = 7 };
 enum { FK_XFER_ERROR = 1, FK_BITFLIP = 2 };
@@ -123,6 +125,8 @@ typedef std::pair<u64, u64> Key;   // 128-bit content key (d, e) of one block
 
 struct Claim {
   u32 state = 0, P = 0, N = 0, M = 0, nb = 0, policy = 0;
+  u32 protect = 0;            // NEXT-3: hard_protected -- its table is never a victim
+  u64 order = 0;              // acceptance sequence number: the victim order
   std::vector<u32> bt;        // current block table
   std::vector<u64> d;         // per-block checksums recorded at offload (chained)
   std::vector<u64> e;         // per-block second digests recorded at offload ((d, e) = content key)
@@ -142,6 +146,7 @@ struct Ctx {
   std::vector<Fault> faults; u32 fault_flags = 0;
   std::vector<Event> events; u64 drained = 0;
   u64 generic_failures = 0;
+  u64 accept_seq = 0;
   // NEXT-2: content-addressed host store keyed by block digest, so blocks shared between claims
   // are held (and cross the link) once.  DESIGN.md "Dedup".
   bool dedup = false;
@@ -167,7 +172,7 @@ static int do_accept(Ctx* c, u64 id, u32 P, u32 N, const u32* bt, u32 nbt) {
     if (bt[i] >= c->NB || !c->used[bt[i]]) return ST_BAD_TABLE;
     for (u32 j = 0; j < i; ++j) if (bt[j] == bt[i]) return ST_BAD_TABLE;
   }
-  Claim cl; cl.state = CS_ACCEPTED; cl.P = P; cl.N = N; cl.bt.assign(bt, bt + nbt);
+  Claim cl; cl.state = CS_ACCEPTED; cl.P = P; cl.N = N; cl.bt.assign(bt, bt + nbt); cl.order = c->accept_seq++;
   for (u32 i = 0; i < nbt; ++i) c->ref[bt[i]]++;
   c->claims[id] = cl;
   c->emit(id, EV_ACCEPTED, N, P);
@@ -367,6 +372,70 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_i
   }
 }
 
+// ---- NEXT-3: allocator-side protection (reading R23) ------------------------------------------------
+// P:L85 victim_exclusion_before_violation ("without victim exclusion, hard protection collapses to soft priority
+// under pressure unless another explicit contract transition occurs first"), explicit_conflict_action,
+// blocking_claim_ids, claim_demoted_before_loss; P:L103 hard_protected bundle; P:L270 allocator_hook ("exposes the
+// victim candidate set, protected resident footprint, and ordered exclusion or release before predicate-breaking
+// loss").  make_room(R, need): an active request R needs `need` free blocks.
+//   1. F = free blocks.  F >= need: OK, nothing happens.
+//   2. Victim candidates = live claims that hold a table (ACCEPTED, MATERIALIZED, RESIDENT_AGAIN): the unprotected
+//      ones first, then the protected ones, each group in acceptance order.  Evicting a claim frees the blocks whose
+//      last reference it holds.  m = the shortest prefix of the list whose eviction brings the free count to `need`.
+//   3. m exists and lies inside the unprotected group: those m claims are demoted, in list order -- DEMOTED(C,
+//      aux = table blocks released, arg = R) is emitted BEFORE the claim's references are dropped (ordered release
+//      before loss); state DEMOTED (terminal).  Status OK; ids = the demoted claims.
+//   4. otherwise the need could only be met from a protected footprint: NOTHING is evicted, no block changes hands.
+//      If protected candidates exist, the request is refused: one CONFLICT_REFUSED record per blocking claim, in list
+//      order, claim_id = the blocking claim, aux = REQ_FLAG | k, arg = R; blocking_claim_ids = the k protected claims
+//      the walk had to enter (all of them if even that is not enough).  Status PROTECTED_CONFLICT; ids = those claims.
+//      With no protected candidate: NO_FREE_BLOCKS, no event.
+static int do_make_room(Ctx* c, u64 request_id, u32 need, u64* ids_out, u32 cap, u32* n_out) {
+  *n_out = 0;
+  u64 nfree = 0;
+  for (u32 b = 0; b < c->NB; ++b) nfree += !c->used[b];
+  if (nfree >= need) return ST_OK;
+  std::vector<std::pair<u64, u64>> cand[2];             // (acceptance order, id); [0] unprotected, [1] protected
+  for (auto& kv : c->claims) {
+    const Claim& cl = kv.second;
+    if (cl.state == CS_ACCEPTED || cl.state == CS_MATERIALIZED || cl.state == CS_RESIDENT_AGAIN)
+      cand[cl.protect ? 1 : 0].push_back({cl.order, kv.first});
+  }
+  std::sort(cand[0].begin(), cand[0].end()); std::sort(cand[1].begin(), cand[1].end());
+  std::vector<u64> list;
+  for (auto& x : cand[0]) list.push_back(x.second);
+  const size_t U = list.size();
+  for (auto& x : cand[1]) list.push_back(x.second);
+  std::vector<u32> ref = c->ref;                         // trial walk on a copy: nothing is evicted yet
+  size_t m = 0; bool met = false;
+  u64 f = nfree;
+  while (m < list.size()) {
+    for (u32 b : c->claims[list[m]].bt) if (--ref[b] == 0) ++f;
+    ++m;
+    if (f >= need) { met = true; break; }
+  }
+  if (met && m <= U) {
+    for (size_t k = 0; k < m; ++k) {
+      Claim& cl = c->claims[list[k]];
+      c->emit(list[k], EV_DEMOTED, (u32)cl.bt.size(), request_id);   // the boundary precedes the loss
+      drop_refs(c, cl);
+      cl.state = CS_DEMOTED;
+      if (*n_out < cap) ids_out[*n_out] = list[k];
+      ++*n_out;
+    }
+    return ST_OK;
+  }
+  if (list.size() == U) return ST_NO_FREE_BLOCKS;       // no protected footprint is in the way: plain exhaustion
+  const size_t hi = met ? m : list.size();
+  const u32 k = (u32)(hi - U);
+  for (size_t i = U; i < hi; ++i) {
+    c->emit(list[i], EV_CONFLICT_REFUSED, REQ_FLAG | k, request_id);
+    if (*n_out < cap) ids_out[*n_out] = list[i];
+    ++*n_out;
+  }
+  return ST_PROTECTED_CONFLICT;
+}
+
 // ---- C ABI (host pointers everywhere) ---------------------------------------
 struct rco_config { u32 layers, kv_heads, head_dim, elem_bytes, block_size, pool_blocks;
                     u64 host_store_bytes; void* pool; u8* fill; };
@@ -421,6 +490,26 @@ int rco_set_policy(void* h, u32 n, const u64* id, const u32* policy) {   // what
   Ctx* c = (Ctx*)h;
   for (u32 k = 0; k < n; ++k) if (!c->claims.count(id[k]) || policy[k] > POL_EXPIRE) return E_INVALID;
   for (u32 k = 0; k < n; ++k) c->claims[id[k]].policy = policy[k];
+  return E_OK;
+}
+int rco_protect(void* h, u32 n, const u64* id, const u32* on) {          // hard_protected on / off; any live claim
+  Ctx* c = (Ctx*)h;
+  for (u32 k = 0; k < n; ++k) {
+    auto it = c->claims.find(id[k]);
+    if (it == c->claims.end() || on[k] > 1 || it->second.state >= CS_REFUSED) return E_INVALID;
+  }
+  for (u32 k = 0; k < n; ++k) c->claims[id[k]].protect = on[k];
+  return E_OK;
+}
+int rco_make_room(void* h, u64 request_id, u32 need, int32_t* status, u64* ids, u32 cap, u32* n_ids) {
+  if (request_id == 0 || !status || !n_ids) return E_INVALID;
+  *status = do_make_room((Ctx*)h, request_id, need, ids, cap, n_ids);
+  return E_OK;
+}
+int rco_protected_map(void* h, u8* prot) {               // prot[NB]: 1 = block lies in a protected footprint
+  Ctx* c = (Ctx*)h;
+  memset(prot, 0, c->NB);
+  for (auto& kv : c->claims) if (kv.second.protect) for (u32 b : kv.second.bt) prot[b] = 1;
   return E_OK;
 }
 int rco_release(void* h, u32 n, const u64* id, int32_t* st) {

@@ -16,7 +16,8 @@ EVENT_DTYPE = np.dtype([("seq", "<u8"), ("claim_id", "<u8"), ("code", "<u4"), ("
 FAULT_DTYPE = np.dtype([("claim_id", "<u8"), ("kind", "<u4"), ("param", "<u4")])
 
 EV_NAMES = {1: "ACCEPTED", 2: "MATERIALIZED", 3: "OFFLOADED", 4: "RESTORE_REQUIRED", 5: "LOAD_FAILED",
-            6: "RESTORED", 7: "RESTORATION_FAILED", 8: "ACTIVE_REQUEST_REFUSED", 9: "DEMOTED", 10: "EXPIRED"}
+            6: "RESTORED", 7: "RESTORATION_FAILED", 8: "ACTIVE_REQUEST_REFUSED", 9: "DEMOTED", 10: "EXPIRED",
+            11: "CONFLICT_REFUSED"}
 REQ_FLAG = 0x80000000
 
 
@@ -169,6 +170,24 @@ class Oracle:
 
     def release(self, ids):
         return self._batch(self.L.rco_release, ids)
+
+    def protect(self, ids, on):
+        ids, on = _u64(ids), _u32(on)
+        return self.L.rco_protect(self.h, ids.size, _p(ids), _p(on))
+
+    def make_room(self, request_id, need, cap=4096):
+        """Returns (status, ids): OK -> the claims demoted to make room; PROTECTED_CONFLICT -> blocking_claim_ids."""
+        st, n = C.c_int32(-1), C.c_uint32()
+        ids = np.zeros(cap, np.uint64)
+        rc = self.L.rco_make_room(self.h, C.c_uint64(request_id), C.c_uint32(need), C.byref(st), _p(ids), cap, C.byref(n))
+        if rc != 0:
+            raise ValueError("rco_make_room: %d" % rc)
+        return st.value, [int(x) for x in ids[: min(cap, n.value)]]
+
+    def protected_map(self):
+        prot = np.zeros(self.NB, np.uint8)
+        self.L.rco_protected_map(self.h, _p(prot))
+        return prot
 
     def outcomes(self, cap=1 << 20):
         buf = np.zeros(cap, EVENT_DTYPE)

@@ -21,9 +21,16 @@ Rules and the passages that fix them:
     same cycle is invalid: generic, unclaimed or wrong-claim failure (P:L25, P:L48,
     P:L463, P:L493);
   * REFUSED.arg (blocking_claim_ids) must be [C], the refused claim itself.
+Allocator-side protection (NEXT-3, DESIGN.md 12 / R23):
+  * DEMOTED(C, arg = request id != 0) while C is resident (ACCEPTED / MATERIALIZED / RESTORED) is the ordered
+    demotion of a victim before its blocks are lost (claim_demoted_before_loss); terminal like the other outcomes;
+    DEMOTED after RESTORATION_FAILED keeps arg = 0;
+  * CONFLICT_REFUSED(C, aux = REQ_FLAG | k, arg = request id): a resident claim C blocks an active request under hard
+    protection; C stays as it is.  The k records of one refusal are consecutive and name k different claims.
 """
 ACCEPTED, MATERIALIZED, OFFLOADED, RESTORE_REQUIRED, LOAD_FAILED, RESTORED, RESTORATION_FAILED, REFUSED = range(1, 9)
 DEMOTED, EXPIRED = 9, 10          # NEXT-3: the other claim-scoped outcomes of a failed restoration (P:L105, P:L120)
+CONFLICT_REFUSED = 11             # NEXT-3: active_request_refused(blocking_claim_ids) under hard protection (P:L85)
 USE, REQUEST_FINISHED = 100, 101
 REQ_FLAG = 0x80000000             # REFUSED.aux of a request-level refusal: flag | size of blocking_claim_ids
 
@@ -50,6 +57,10 @@ _NEXT = {
     (_ACC, REQUEST_FINISHED): _FIN,
     (_MAT, REQUEST_FINISHED): _FIN,
     (_RES, REQUEST_FINISHED): _FIN,
+    # allocator-side protection: a resident victim is demoted before its blocks are lost; a protected resident claim
+    # that blocks an active request is named and stays
+    (_ACC, DEMOTED): _DEM, (_MAT, DEMOTED): _DEM, (_RES, DEMOTED): _DEM,
+    (_ACC, CONFLICT_REFUSED): _ACC, (_MAT, CONFLICT_REFUSED): _MAT, (_RES, CONFLICT_REFUSED): _RES,
 }
 
 
@@ -77,6 +88,7 @@ def _scan(events):
     last_seq = None
     pending = 0                     # claims in state RF: failed, outcome not yet emitted
     group = None                    # [arg, aux, records still to come]
+    cgroup = None                   # the same for a CONFLICT_REFUSED run, plus the claims it has named
     for i, (seq, cid, code, aux, arg) in enumerate(_rows(events)):
         if last_seq is not None and seq <= last_seq:
             return False, i, "seq not strictly increasing at %d" % seq
@@ -85,13 +97,30 @@ def _scan(events):
             return False, i, "event names no claim (unclaimed) at seq %d" % seq
         if group is not None and not (code == REFUSED and arg == group[0] and aux == group[1]):
             return False, i, "blocking_claim_ids run of request %#x interrupted (seq %d)" % (group[0], seq)
+        if cgroup is not None and not (code == CONFLICT_REFUSED and arg == cgroup[0] and aux == cgroup[1]):
+            return False, i, "blocking_claim_ids run of request %#x interrupted (seq %d)" % (cgroup[0], seq)
         s = state.get(cid, _S0)
         nxt = _NEXT.get((s, code))
+        if code == DEMOTED and nxt is not None and (arg == 0) != (s == _RF):
+            nxt = None                                  # arg = 0 after a failed restoration, = request id for a victim
+        if code == CONFLICT_REFUSED and nxt is not None:
+            k = aux & ~REQ_FLAG
+            if not (aux & REQ_FLAG) or k == 0 or arg == 0:
+                nxt = None
+            elif cgroup is None:
+                cgroup = [arg, aux, k, set()]
+            if nxt is not None:
+                if cid in cgroup[3]:
+                    return False, i, "request %#x: blocking claim %#x named twice (seq %d)" % (arg, cid, seq)
+                cgroup[3].add(cid)
+                cgroup[2] -= 1
+                if cgroup[2] == 0:
+                    cgroup = None
         if nxt is None:
             return False, i, "claim %#x: code %d not allowed in state %d (seq %d)" % (cid, code, s, seq)
         if code == RESTORATION_FAILED:
             pending += 1
-        elif code in (DEMOTED, EXPIRED):
+        elif code == EXPIRED or (code == DEMOTED and s == _RF):
             pending -= 1
         elif code == REFUSED:
             if aux & REQ_FLAG:

@@ -107,7 +107,8 @@ struct Op {
 
 struct rc_ctx {
   rc_config cfg;
-  u32 G = 0, vpp = 0, NB = 0, R = 0, sms = 0, grid = 0, tma_variant = 0, mover = 0;
+  u32 G = 0, vpp = 0, NB = 0, R = 0, sms = 0, grid = 0, mover = 0;
+  u32 tma_variant[3] = {0, 0, 0}, tma_grid[3] = {0, 0, 0};   // per mover mode (gather, scatter, digest)
   u64 page = 0, blk = 0, chunk_blocks = 0, host_blocks = 0, cap_entries = 0, desc_cap = 0;
   cudaStream_t meta = 0, gather = 0, d2h = 0, scatter = 0, h2d = 0, util = 0;
   bool own[5] = {false, false, false, false, false};
@@ -180,24 +181,31 @@ static void launch_ldg(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, 
     k_move_hash<MODE, 1><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos);
 }
 
-// (TILE, STAGES) variants of the TMA mover; RC_TMA_VARIANT=<index> overrides the default choice (tuning sweeps)
+// (TILE, STAGES per group, consumer groups, CTAs/SM) variants of the TMA mover; RC_TMA_VARIANT=<index> overrides the
+// default choice (tuning sweeps, profiles/r02_mover_sweep.md)
 typedef void (*tma_fn)(u8*, u8*, const u32*, u64*, u32, u32, u32, u32, const u32*, const u32*);
-struct TmaVariant { u32 tile, stages, ctas_per_sm; tma_fn fn[3]; };
-#define TMA_V(T, S, C) {T, S, C, {k_move_hash_tma<MV_GATHER, S, T>, k_move_hash_tma<MV_SCATTER, S, T>, k_move_hash_tma<MV_DIGEST, S, T>}}
-// Measured on B200 (profiles/r01_mover_sweep.md): about 96 KiB of bulk loads in flight per SM is the sweet
-// spot -- 32 KiB tiles x 3 stages x 1 CTA/SM (variant 7) or 16 KiB x 3 x 2 CTAs/SM (variant 3); more bytes in
-// flight lowers DRAM efficiency, fewer leaves the latency uncovered.
-static const TmaVariant kTma[] = {TMA_V(4096, 4, 2), TMA_V(8192, 4, 2), TMA_V(8192, 8, 1), TMA_V(16384, 3, 2), TMA_V(16384, 4, 1),
-                                  TMA_V(16384, 6, 1), TMA_V(32768, 2, 2), TMA_V(32768, 3, 1), TMA_V(16384, 12, 1), TMA_V(32768, 6, 1)};
+struct TmaVariant { u32 tile, stages, groups, ctas_per_sm; tma_fn fn[3]; };
+#define TMA_V(T, S, NG, C) {T, S, NG, C, {k_move_hash_tma<MV_GATHER, S, T, NG>, k_move_hash_tma<MV_SCATTER, S, T, NG>, k_move_hash_tma<MV_DIGEST, S, T, NG>}}
+static const TmaVariant kTma[] = {
+    TMA_V(4096, 4, 1, 2),  TMA_V(8192, 4, 1, 2),  TMA_V(8192, 8, 1, 1),   TMA_V(16384, 3, 1, 2),  TMA_V(16384, 4, 1, 1),
+    TMA_V(16384, 6, 1, 1), TMA_V(32768, 2, 1, 2), TMA_V(32768, 3, 1, 1),  TMA_V(16384, 12, 1, 1), TMA_V(32768, 6, 1, 1),
+    /* 10.. two consumer groups */
+    TMA_V(32768, 2, 2, 1), TMA_V(32768, 3, 2, 1), TMA_V(16384, 3, 2, 1),  TMA_V(16384, 4, 2, 1),  TMA_V(16384, 6, 2, 1),
+    TMA_V(16384, 2, 2, 2), TMA_V(16384, 3, 2, 2), TMA_V(8192, 4, 2, 2),   TMA_V(4096, 4, 2, 2),   TMA_V(32768, 4, 1, 1),
+    /* 20.. small tiles */
+    TMA_V(8192, 3, 1, 2),  TMA_V(8192, 6, 1, 1),  TMA_V(8192, 4, 1, 3),   TMA_V(16384, 2, 1, 2),  TMA_V(4096, 8, 1, 2),
+    TMA_V(8192, 2, 1, 4),  TMA_V(8192, 6, 1, 2),  TMA_V(4096, 6, 1, 3),   TMA_V(8192, 3, 2, 2),   TMA_V(8192, 2, 2, 2)};
 constexpr int kTmaN = sizeof(kTma) / sizeof(kTma[0]);
+static inline u32 tma_smem(const TmaVariant& v) { return v.tile * v.stages * v.groups; }
+static inline u32 tma_block(const TmaVariant& v) { return v.groups * LANES + 64; }
 
 template <int MODE>
 static void launch_move(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items,
                         const u32* iw = nullptr, const u32* ispos = nullptr) {
   if (c->mover == RC_MOVER_TMA) {
-    const TmaVariant& v = kTma[c->tma_variant];
-    const u32 grid = std::min(n_items * c->G, c->grid);
-    v.fn[MODE]<<<grid, TMA_THREADS, v.tile * v.stages, s>>>(c->pool, staging, phys, part, n_items, c->G, c->NB, (u32)c->page, iw, ispos);
+    const TmaVariant& v = kTma[c->tma_variant[MODE]];
+    const u32 grid = std::min(n_items * c->G, c->tma_grid[MODE]);
+    v.fn[MODE]<<<grid, tma_block(v), tma_smem(v), s>>>(c->pool, staging, phys, part, n_items, c->G, c->NB, (u32)c->page, iw, ispos);
   } else launch_ldg<MODE>(c, s, staging, phys, part, n_items, iw, ispos);
   c->st.kernel_launches++;
 }
@@ -337,26 +345,28 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   if (c->host_blocks && c->direct) CC(cudaHostGetDevicePointer((void**)&c->h_store_dev, c->h_store, 0), RC_ERR_CUDA);
   // launch geometry of the movers
   c->mover = cfg->mover == RC_MOVER_AUTO ? RC_MOVER_TMA : cfg->mover;
-  int occ = 0;
   if (c->mover == RC_MOVER_TMA) {
-    int want = page % 32768 == 0 ? 7 : (page % 16384 == 0 ? 3 : (page % 8192 == 0 ? 1 : 0));
-    if (const char* e = getenv("RC_TMA_VARIANT")) want = atoi(e);
-    if (want < 0 || want >= kTmaN || page % kTma[want].tile != 0) return fail(RC_ERR_INVALID, "RC_TMA_VARIANT", cudaSuccess);
-    c->tma_variant = want;
-    const TmaVariant& v = kTma[want];
-    occ = 1 << 30;
+    // Measured on B200 with the mum fold (profiles/r02_mover_sweep.md): the fused movers want about 64 KiB of bulk
+    // loads in flight per SM -- 8 KiB tiles x 4 stages x 2 CTAs/SM (variant 1) wins for 32 KiB and 16 KiB pages alike;
+    // the read-only digest pass runs at twice the byte rate and wants two folding groups (variants 10 / 15).
     for (int m = 0; m < 3; ++m) {
+      int want = page % 8192 == 0 ? 1 : 0;
+      if (m == MV_DIGEST) want = page % 32768 == 0 ? 10 : (page % 16384 == 0 ? 15 : want);
+      if (const char* e = getenv("RC_TMA_VARIANT")) want = atoi(e);
+      if (m == MV_DIGEST) if (const char* e = getenv("RC_TMA_VARIANT_DIGEST")) want = atoi(e);
+      if (want < 0 || want >= kTmaN || page % kTma[want].tile != 0) return fail(RC_ERR_INVALID, "RC_TMA_VARIANT", cudaSuccess);
+      c->tma_variant[m] = want;
+      const TmaVariant& v = kTma[want];
       int o = 0;
-      CC(cudaFuncSetAttribute(v.fn[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(v.tile * v.stages)), RC_ERR_CUDA);
-      CC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, v.fn[m], TMA_THREADS, v.tile * v.stages), RC_ERR_CUDA);
-      occ = std::min(occ, o);
+      CC(cudaFuncSetAttribute(v.fn[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem(v)), RC_ERR_CUDA);
+      CC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, v.fn[m], (int)tma_block(v), tma_smem(v)), RC_ERR_CUDA);
+      o = std::max(1, std::min<int>(o, v.ctas_per_sm));
+      c->tma_grid[m] = cfg->grid_ctas ? cfg->grid_ctas : c->sms * (u32)o;
     }
-  } else {
-    CC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hash<MV_GATHER, 8>, LANES, 0), RC_ERR_CUDA);
   }
-  if (occ < 1) occ = 1;
-  if (c->mover == RC_MOVER_TMA) occ = std::min<int>(occ, kTma[c->tma_variant].ctas_per_sm);
-  else occ = std::min(occ, 2);
+  int occ = 0;
+  CC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_move_hash<MV_GATHER, 8>, LANES, 0), RC_ERR_CUDA);
+  occ = std::max(1, std::min(occ, 2));
   c->grid = cfg->grid_ctas ? cfg->grid_ctas : c->sms * (u32)occ;
 #undef CC
   *out = c;

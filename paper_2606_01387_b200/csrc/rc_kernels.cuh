@@ -150,7 +150,7 @@ k_move_hash(uint4* __restrict__ pool, uint4* __restrict__ staging, const u32* __
 // (cp.async.bulk global->shared completing on an mbarrier; shared->global bulk store), so the
 // LSU only sees conflict-free 16-byte shared loads for the checksum.  One elected thread issues
 // the copies; a ring of STAGES tiles of TILE bytes keeps STAGES-1 loads in flight per CTA.
-// Tiles are consumed in page order, so thread t still folds vectors t, t+256, ... in increasing
+// Tiles of a page are consumed in order, so lane t still folds vectors t, t+256, ... in increasing
 // order.  Persistent grid: CTA c handles pages c, c+grid, ...
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
@@ -184,34 +184,41 @@ __device__ __forceinline__ void mbar_arrive(u64* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(bar)) : "memory");
 }
 
-// Warp roles: warps 0..7 = the 256 checksum lanes (consumers); warp 8 lane 0 = load producer; warp 9
-// lane 0 = store issuer.  full[s]: tile landed (tx bytes).  empty[s]: 8 consumer warps (+ the store
-// issuer once its bulk store has finished reading the stage) released the stage.  No block barrier in
-// the steady state: the producer runs STAGES tiles ahead, consumers and stores follow at their own pace.
-constexpr int TMA_THREADS = LANES + 64;
+// Warp roles: NG consumer groups of 8 warps (= the 256 checksum lanes of one page each; group g folds the CTA's pages
+// g, g+NG, ...), then one load-producer warp and one store-issuer warp (lane 0 of each).  Every group owns a ring of
+// STAGES tiles, so each mbarrier is waited on by the same warps in every phase.  full[s]: tile landed (tx bytes).
+// empty[s]: the group's 8 warps (+ the store issuer once its bulk store has finished reading the stage) released the
+// stage.  No block barrier in the steady state.  NG = 2 keeps four folding warps per scheduler: the mum fold (R22) is
+// a chain of dependent IMAD.WIDEs, and two warps per scheduler could not hide its latency.
+template <int NG> constexpr int tma_threads() { return NG * LANES + 64; }
 
-template <int MODE, int STAGES, int TILE>
-__global__ void __launch_bounds__(TMA_THREADS, 1)
+template <int MODE, int STAGES, int TILE, int NG>
+__global__ void __launch_bounds__(NG * LANES + 64, 1)
 k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __restrict__ phys,
                 u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 page_bytes,
                 const u32* __restrict__ iw, const u32* __restrict__ ispos) {
   extern __shared__ __align__(128) u8 smem[];
-  __shared__ __align__(8) u64 full[STAGES];
-  __shared__ __align__(8) u64 empty[STAGES];
+  __shared__ __align__(8) u64 full[NG * STAGES];
+  __shared__ __align__(8) u64 empty[NG * STAGES];
   const u32 t = threadIdx.x, warp = t >> 5;
+  constexpr u32 NCW = NG * WPC;                          // consumer warps
   const u32 n_pages = n_items * G;
   const u32 tpp = page_bytes / TILE;                     // tiles per page (page % TILE == 0)
   constexpr u32 VT = TILE / (16 * LANES);                // vectors per lane per tile
   if (t == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], WPC + (MODE != MV_DIGEST ? 1 : 0)); }
+    for (int s = 0; s < NG * STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], WPC + (MODE != MV_DIGEST ? 1 : 0)); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  // this CTA's tile sequence: pages blockIdx.x + k*grid, tiles 0..tpp-1 of each
+  // this CTA's pages: blockIdx.x + k*grid, k = 0..my_pages-1; page k belongs to group k % NG and is that group's
+  // (k / NG)-th page; its tile `tile` is the group's j-th tile, staged in ring slot j % STAGES in phase j / STAGES
   const u32 my_pages = (n_pages > blockIdx.x) ? (n_pages - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
   const u64 n_tiles = (u64)my_pages * tpp;
-  auto addr = [&](u64 q, u8*& gsrc, u8*& gdst, bool& skip) {
-    const u32 k = (u32)(q / tpp), tile = (u32)(q - (u64)k * tpp);
+  auto slot = [&](u32 k, u32 tile, u32& s, u64& j) {
+    j = (u64)(k / NG) * tpp + tile;
+    s = (k % NG) * STAGES + (u32)(j % STAGES);
+  };
+  auto addr = [&](u32 k, u32 tile, u8*& gsrc, u8*& gdst, bool& skip) {
     const u32 u = blockIdx.x + k * gridDim.x;
     const u32 w = u / G, g = u - w * G;
     u32 b = 0;
@@ -222,49 +229,52 @@ k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __re
     gsrc = (MODE == MV_GATHER) ? pp : sp;
     gdst = (MODE == MV_GATHER) ? sp : pp;
   };
-  if (warp == WPC) {                                       // ---- load producer
-    if (t == LANES) {
+  if (warp == NCW) {                                       // ---- load producer
+    if (t == NCW * 32) {
       for (u64 q = 0; q < n_tiles; ++q) {
-        const u32 s = (u32)(q % STAGES);
-        if (q >= STAGES) mbar_wait(&empty[s], (u32)(((q / STAGES) - 1) & 1));
-        u8 *gs, *gd; bool skip; addr(q, gs, gd, skip);
+        const u32 k = (u32)(q / tpp), tile = (u32)(q - (u64)k * tpp);
+        u32 s; u64 j; slot(k, tile, s, j);
+        if (j >= STAGES) mbar_wait(&empty[s], (u32)(((j / STAGES) - 1) & 1));
+        u8 *gs, *gd; bool skip; addr(k, tile, gs, gd, skip);
         mbar_expect_tx(&full[s], TILE);
         bulk_g2s(smem + s * TILE, gs, TILE, &full[s]);
       }
     }
-  } else if (warp == WPC + 1) {                            // ---- store issuer
-    if (MODE != MV_DIGEST && t == LANES + 32) {
+  } else if (warp == NCW + 1) {                            // ---- store issuer
+    if (MODE != MV_DIGEST && t == NCW * 32 + 32) {
+      u32 prev = 0;
       for (u64 q = 0; q < n_tiles; ++q) {
-        const u32 s = (u32)(q % STAGES);
-        mbar_wait(&full[s], (u32)((q / STAGES) & 1));
-        u8 *gs, *gd; bool skip; addr(q, gs, gd, skip);
+        const u32 k = (u32)(q / tpp), tile = (u32)(q - (u64)k * tpp);
+        u32 s; u64 j; slot(k, tile, s, j);
+        mbar_wait(&full[s], (u32)((j / STAGES) & 1));
+        u8 *gs, *gd; bool skip; addr(k, tile, gs, gd, skip);
         if (!skip) bulk_s2g(gd, smem + s * TILE, TILE);
         bulk_commit();
-        if (q > 0) { bulk_wait_read<1>(); mbar_arrive(&empty[(u32)((q - 1) % STAGES)]); }   // store q-1 drained its stage
+        if (q > 0) { bulk_wait_read<1>(); mbar_arrive(&empty[prev]); }   // the previous store drained its stage
+        prev = s;
       }
-      if (n_tiles) { bulk_wait_read<0>(); mbar_arrive(&empty[(u32)((n_tiles - 1) % STAGES)]); }
+      if (n_tiles) { bulk_wait_read<0>(); mbar_arrive(&empty[prev]); }
       asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
-  } else {                                                 // ---- consumers: lane t folds vectors t, t+256, ...
-    u64 h = 0, gq = 0;
-    for (u64 q = 0; q < n_tiles; ++q) {
-      const u32 s = (u32)(q % STAGES);
-      const u32 k = (u32)(q / tpp), tile = (u32)(q - (u64)k * tpp);
-      if (tile == 0) { h = (u64)(t + 1) * C1; gq = (u64)(t + 1) * C4; }
-      mbar_wait(&full[s], (u32)((q / STAGES) & 1));
-      const uint4* sv = reinterpret_cast<const uint4*>(smem + s * TILE) + t;
+  } else {                                                 // ---- consumers: lane tl of group grp folds vectors tl, tl+256, ...
+    const u32 grp = warp / WPC, tl = t - grp * LANES, wl = warp - grp * WPC;
+    for (u32 k = grp; k < my_pages; k += NG) {
+      u64 h = (u64)(tl + 1) * C1, gq = (u64)(tl + 1) * C4;
+      for (u32 tile = 0; tile < tpp; ++tile) {
+        u32 s; u64 j; slot(k, tile, s, j);
+        mbar_wait(&full[s], (u32)((j / STAGES) & 1));
+        const uint4* sv = reinterpret_cast<const uint4*>(smem + s * TILE) + tl;
 #pragma unroll
-      for (u32 j = 0; j < VT; ++j) fold2(h, gq, sv[j * LANES]);
-      asm volatile("" :: "l"(h), "l"(gq) : "memory");      // the fold consumed the tile: its shared loads have completed
-      __syncwarp();
-      if ((t & 31) == 0) mbar_arrive(&empty[s]);           // this warp releases the stage
-      if (tile == tpp - 1) {
-        bool skip = false;
-        const u32 u = blockIdx.x + k * gridDim.x;
-        if (MODE != MV_DIGEST) { const u32 w = u / G; skip = __ldg(phys + (iw ? __ldg(iw + w) : w)) == SKIP; }
-        const u64 sum = warp_sum64(mixL(h)), sum2 = warp_sum64(mixL(gq));
-        if ((t & 31) == 0 && !skip) { u64* o = part + ((u64)u * WPC + warp) * 2; o[0] = sum; o[1] = sum2; }
+        for (u32 v = 0; v < VT; ++v) fold2(h, gq, sv[v * LANES]);
+        asm volatile("" :: "l"(h), "l"(gq) : "memory");    // the fold consumed the tile: its shared loads have completed
+        __syncwarp();
+        if ((t & 31) == 0) mbar_arrive(&empty[s]);         // this warp releases the stage
       }
+      bool skip = false;
+      const u32 u = blockIdx.x + k * gridDim.x;
+      if (MODE != MV_DIGEST) { const u32 w = u / G; skip = __ldg(phys + (iw ? __ldg(iw + w) : w)) == SKIP; }
+      const u64 sum = warp_sum64(mixL(h)), sum2 = warp_sum64(mixL(gq));
+      if ((t & 31) == 0 && !skip) { u64* o = part + ((u64)u * WPC + wl) * 2; o[0] = sum; o[1] = sum2; }
     }
   }
 }
