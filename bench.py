@@ -427,7 +427,9 @@ def main():
                        "what": "same step through the C ABI with host arrays; fill[] sent from pinned host memory, "
                                "statuses and the event stream read back, inside the timed region"}
     if world == 1 and not a.no_cpu_baseline:   # NEXT-1: device trace validator on a 200k-claim synthetic stream (not part of `value`)
-        tr = W.make_trace(200000, 1)
+        sys.path.insert(0, os.path.join(ROOT, "tests"))
+        import trace_inputs                                  # input generator only (tests/trace_inputs.py)
+        tr = trace_inputs.make_trace(200000, 1)
         best = None
         for _ in range(3):
             rep, _c = rc.validate_trace(tr, want_claims=False)

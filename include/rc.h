@@ -44,7 +44,7 @@ enum { RC_OK = 0, RC_ERR_INVALID = -1, RC_ERR_CUDA = -2, RC_ERR_NOMEM = -3, RC_E
 /* per-claim status */
 enum { RC_ST_OK = 0, RC_ST_PRED_FALSE = 1, RC_ST_UNKNOWN_CLAIM = 2, RC_ST_BAD_STATE = 3,
        RC_ST_DUPLICATE_ID = 4, RC_ST_BAD_TABLE = 5, RC_ST_NO_FREE_BLOCKS = 6,
-       RC_ST_NO_HOST_SPACE = 7, RC_ST_RESTORE_FAILED = 8 };
+       RC_ST_NO_HOST_SPACE = 7, RC_ST_RESTORE_FAILED = 8, RC_ST_PROTECTED_CONFLICT = 9 };
 
 /* event codes (the ordered claim-scoped outcome stream) */
 enum { RC_EV_ACCEPTED = 1,          /* aux = N (predicate threshold), arg = P (prefix tokens)      */
@@ -55,7 +55,10 @@ enum { RC_EV_ACCEPTED = 1,          /* aux = N (predicate threshold), arg = P (p
        RC_EV_RESTORED = 6,          /* aux = nb, arg = chain checksum                              */
        RC_EV_RESTORATION_FAILED = 7,
        RC_EV_ACTIVE_REQUEST_REFUSED = 8, /* aux = 1 = |blocking_claim_ids|, arg = C; request form below */
-       RC_EV_DEMOTED = 9, RC_EV_EXPIRED = 10 /* NEXT-3: the other claim-scoped outcomes of a failed restoration */ };
+       RC_EV_DEMOTED = 9, RC_EV_EXPIRED = 10, /* NEXT-3: the other claim-scoped outcomes of a failed restoration (arg = 0);
+                                                 DEMOTED with arg = request id: a victim demoted by rc_make_room    */
+       RC_EV_CONFLICT_REFUSED = 11 /* NEXT-3: active_request_refused(blocking_claim_ids) under hard protection:
+                                      claim_id = a blocking claim, aux = RC_REFUSED_REQUEST | k, arg = request id */ };
 /* request-level refusal (rc_restore_request): aux = RC_REFUSED_REQUEST | size of blocking_claim_ids, arg = request id */
 #define RC_REFUSED_REQUEST 0x80000000u
 
@@ -177,6 +180,25 @@ int rc_set_policy(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, const uint3
 int rc_restore_request(rc_ctx* ctx, uint64_t request_id, uint32_t n, const uint64_t* claim_id, int32_t* status);
 int rc_restore_request_begin(rc_ctx* ctx, uint64_t request_id, uint32_t n, const uint64_t* claim_id, int32_t* status);
 
+/* NEXT-3, allocator-side protection (P:L85 victim_exclusion_before_violation, explicit_conflict_action,
+ * blocking_claim_ids, claim_demoted_before_loss; P:L103 hard_protected; P:L270 allocator_hook).
+ * rc_protect: marks live (non-terminal) claims hard_protected (on = 1) or not (0).  The protected resident footprint is
+ * the union of the block tables of protected claims (rc_protected_map copies it out as u8[NB]); it follows a claim
+ * through offload and restore.  Unknown / terminal id or on > 1 -> RC_ERR_INVALID, nothing changes.
+ * rc_make_room: an active request (request_id != 0) needs `need_blocks` free blocks.  If they are free already:
+ * status OK, nothing happens.  Otherwise the victim candidates are the live claims that hold a table, unprotected
+ * first, then protected, each group in acceptance order; evicting a claim frees the blocks whose last holder it is.
+ * If a prefix of the UNPROTECTED candidates suffices, exactly that prefix is demoted: DEMOTED(C, aux = table blocks
+ * released, arg = request_id) is emitted before the claim's references are dropped; the claims become terminal;
+ * status OK, ids = the demoted claims.  If the need could only be met from a protected footprint, nothing is evicted
+ * and no block changes hands: status RC_ST_PROTECTED_CONFLICT, ids = blocking_claim_ids = the protected claims the
+ * walk had to enter, one RC_EV_CONFLICT_REFUSED record each.  No protected claim in the way: RC_ST_NO_FREE_BLOCKS, no
+ * event.  n_ids receives the number of ids (may exceed cap).  RC_ERR_BUSY while an offload or restore is in flight. */
+int rc_protect(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, const uint32_t* on);
+int rc_make_room(rc_ctx* ctx, uint64_t request_id, uint32_t need_blocks, int32_t* status, uint64_t* ids, uint32_t cap,
+                 uint32_t* n_ids);
+int rc_protected_map(rc_ctx* ctx, uint8_t* prot /* HOST u8[NB] */);
+
 /* Drains up to cap not-yet-returned events of completed calls, in seq order. */
 int rc_outcomes(rc_ctx* ctx, rc_event* buf, uint64_t cap, uint64_t* n_out);
 
@@ -223,7 +245,11 @@ int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64
  * violation (UINT64_MAX if none).  claims (HOST, may be NULL) receives up to cap per-claim records in
  * unspecified order: final automaton state, gate bits (RC_GATE_FAILURE: the claim's subsequence ends with
  * the seven steps of P:L27; RC_GATE_OBSERVATION: path A; both 0 unless the stream is valid),
- * its first violating position.  Needs no context; allocates and frees its own device memory. */
+ * its first violating position.  NEXT-3 adds: DEMOTED with arg = request id from ACCEPTED / MATERIALIZED / RESTORED (a
+ * victim of rc_make_room; DEMOTED after RESTORATION_FAILED keeps arg 0), and RC_EV_CONFLICT_REFUSED (aux =
+ * RC_REFUSED_REQUEST | k, arg = request id) as a self-loop of a resident claim, k consecutive records naming k
+ * different claims.  n <= 2^30 events (RC_ERR_INVALID above).  Needs no context; allocates and frees its own
+ * device memory. */
 enum { RC_EV_USE = 100, RC_EV_REQUEST_FINISHED = 101 };
 enum { RC_GATE_FAILURE = 1, RC_GATE_OBSERVATION = 2 };
 typedef struct rc_trace_claim { uint64_t claim_id; uint64_t first_bad; uint32_t state; uint32_t gates; uint32_t n_events; uint32_t pad; } rc_trace_claim;

@@ -89,6 +89,7 @@ def _scan(events):
     pending = 0                     # claims in state RF: failed, outcome not yet emitted
     group = None                    # [arg, aux, records still to come]
     cgroup = None                   # the same for a CONFLICT_REFUSED run, plus the claims it has named
+    cdone = None                    # (arg, aux) of the CONFLICT_REFUSED run that ended with the previous record
     for i, (seq, cid, code, aux, arg) in enumerate(_rows(events)):
         if last_seq is not None and seq <= last_seq:
             return False, i, "seq not strictly increasing at %d" % seq
@@ -107,6 +108,8 @@ def _scan(events):
             k = aux & ~REQ_FLAG
             if not (aux & REQ_FLAG) or k == 0 or arg == 0:
                 nxt = None
+            elif cgroup is None and cdone == (arg, aux):
+                return False, i, "request %#x: more blocking_claim_ids records than announced (seq %d)" % (arg, seq)
             elif cgroup is None:
                 cgroup = [arg, aux, k, set()]
             if nxt is not None:
@@ -116,6 +119,10 @@ def _scan(events):
                 cgroup[2] -= 1
                 if cgroup[2] == 0:
                     cgroup = None
+                    cdone = (arg, aux)
+                    state[cid] = nxt
+                    continue
+        cdone = None
         if nxt is None:
             return False, i, "claim %#x: code %d not allowed in state %d (seq %d)" % (cid, code, s, seq)
         if code == RESTORATION_FAILED:

@@ -82,6 +82,8 @@ struct KeyHash { size_t operator()(const Key& k) const { return (size_t)(k.first
 struct Claim {
   u64 id = 0, chain = 0;
   u32 state = 0, P = 0, N = 0, M = 0, nb = 0, policy = 0;
+  u32 protect = 0;                       // NEXT-3: hard_protected -- never a victim of rc_make_room
+  u64 order = 0;                         // acceptance sequence number: the victim order
   u32 bt_off = 0, bt_len = 0;            // live table extent (bt_len == 0: no table)
   u32 dg_off = 0, dg_len = 0;            // recorded digests
   std::vector<std::pair<u64, u64>> host; // host-store extents in blk units
@@ -116,6 +118,7 @@ struct rc_ctx {
   u8* d_used = nullptr; u32* d_ref = nullptr; u32* d_bt = nullptr; u64* d_dg = nullptr; u64* d_dg2 = nullptr;
   Event* d_ring = nullptr; u64* d_evcount = nullptr; u32* d_bitmaps = nullptr; u32* d_up = nullptr;
   u32* d_counters = nullptr; u32* d_alloc = nullptr; u64* d_flip = nullptr;
+  u32 *d_posmax = nullptr, *d_gain = nullptr; u8* d_protmap = nullptr; u64 accept_seq = 0;   // NEXT-3 allocator-side protection
   Desc* d_desc[3] = {}; Res* d_res[3] = {}; u32* d_off[3] = {};
   Desc* h_desc[3] = {}; Res* h_res[3] = {};
   u32* h_up = nullptr; u64* h_flip = nullptr; u32* h_counters = nullptr;
@@ -217,7 +220,7 @@ extern "C" int rc_destroy(rc_ctx* c) {
   auto F = [](void* p) { if (p) cudaFree(p); };
   auto FH = [](void* p) { if (p) cudaFreeHost(p); };
   F(c->d_used); F(c->d_ref); F(c->d_bt); F(c->d_dg); F(c->d_dg2); F(c->d_ring); F(c->d_evcount); F(c->d_bitmaps); F(c->d_up);
-  F(c->d_counters); F(c->d_alloc); F(c->d_flip);
+  F(c->d_counters); F(c->d_alloc); F(c->d_flip); F(c->d_posmax); F(c->d_gain); F(c->d_protmap);
   for (int i = 0; i < 3; ++i) { F(c->d_desc[i]); F(c->d_res[i]); F(c->d_off[i]); FH(c->h_desc[i]); FH(c->h_res[i]); }
   FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
   F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
@@ -295,6 +298,9 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   CC(cudaMalloc(&c->d_counters, 16), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_alloc, cap * 4), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_flip, dc * 8), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_posmax, NB * 4), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_gain, dc * 4), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_protmap, NB), RC_ERR_NOMEM);
   CC(cudaMemset(c->d_used, 0, NB), RC_ERR_CUDA);
   CC(cudaMemset(c->d_ref, 0, NB * 4), RC_ERR_CUDA);
   CC(cudaMemset(c->d_evcount, 0, 8), RC_ERR_CUDA);
@@ -451,7 +457,7 @@ static int accept_run(rc_ctx* c, u32 n, const u64* id, const u32* P, const u32* 
   for (u32 k : cand) {
     if (c->h_res[2][k].flag & R_OK) {
       Claim cl;
-      cl.id = id[k]; cl.state = RC_CS_ACCEPTED; cl.P = P[k]; cl.N = N[k];
+      cl.id = id[k]; cl.state = RC_CS_ACCEPTED; cl.P = P[k]; cl.N = N[k]; cl.order = c->accept_seq++;
       cl.bt_off = hd[k].bt_off; cl.bt_len = hd[k].bt_len;
       c->claims.emplace(id[k], std::move(cl));
       c->ev_emitted++;
@@ -931,6 +937,121 @@ extern "C" int rc_set_policy(rc_ctx* c, uint32_t n, const uint64_t* id, const ui
   return RC_OK;
 }
 
+// ---- NEXT-3: allocator-side protection (rc.h, R23) -------------------------------------------------
+extern "C" int rc_protect(rc_ctx* c, uint32_t n, const uint64_t* id, const uint32_t* on) {
+  GUARD();
+  if (n && (!id || !on)) return RC_ERR_INVALID;
+  for (u32 k = 0; k < n; ++k) {
+    auto it = c->claims.find(id[k]);
+    if (it == c->claims.end() || on[k] > 1 || it->second.state >= RC_CS_REFUSED) return RC_ERR_INVALID;
+  }
+  for (u32 k = 0; k < n; ++k) c->claims[id[k]].protect = on[k];
+  return RC_OK;
+}
+
+// live claims that hold a table, in victim order: unprotected first, then protected, acceptance order inside each
+static void victim_list(rc_ctx* c, std::vector<Claim*>& list, u32& U) {
+  std::vector<Claim*> grp[2];
+  for (auto& kv : c->claims) {
+    Claim& cl = kv.second;
+    if (cl.bt_len && (cl.state == RC_CS_ACCEPTED || cl.state == RC_CS_MATERIALIZED || cl.state == RC_CS_RESIDENT_AGAIN))
+      grp[cl.protect ? 1 : 0].push_back(&cl);
+  }
+  for (auto& g : grp) std::sort(g.begin(), g.end(), [](const Claim* a, const Claim* b) { return a->order < b->order; });
+  list = grp[0];
+  U = (u32)list.size();
+  list.insert(list.end(), grp[1].begin(), grp[1].end());
+}
+static void fill_desc(Desc& d, const Claim& cl, u32 flags) {
+  memset(&d, 0, sizeof(Desc));
+  d.id = cl.id; d.P = cl.P; d.N = cl.N; d.M = cl.M; d.nb = cl.nb; d.bt_off = cl.bt_off; d.bt_len = cl.bt_len; d.flags = flags;
+}
+
+extern "C" int rc_make_room(rc_ctx* c, uint64_t request_id, uint32_t need, int32_t* status, uint64_t* ids, uint32_t cap,
+                            uint32_t* n_ids) {
+  GUARD();
+  if (request_id == 0 || !status || !n_ids || (cap && !ids)) return RC_ERR_INVALID;
+  if (c->ops[0].active || c->ops[1].active) return RC_ERR_BUSY;
+  *n_ids = 0;
+  std::vector<Claim*> list;
+  u32 U = 0;
+  victim_list(c, list, U);
+  const u32 n = (u32)list.size();
+  if (n > c->desc_cap || !ev_room(c, n)) return RC_ERR_CAPACITY;
+  Desc* hd = c->h_desc[2];
+  for (u32 k = 0; k < n; ++k) fill_desc(hd[k], *list[k], D_ELIG | (list[k]->protect ? (u32)D_PROT : 0u));
+  int rc;
+  if (n) {
+    if ((rc = upload_desc(c, 2, n))) return rc;
+    CK(cudaMemsetAsync(c->d_posmax, 0, (u64)c->NB * 4, c->meta));
+    k_vic_posmax<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[2], n, c->d_bt, c->d_posmax);
+    CKL();
+    k_vic_gain<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[2], n, c->d_bt, c->d_posmax, c->d_gain);
+    CKL();
+    c->st.kernel_launches += 2;
+  }
+  k_vic_decide<<<1, 1024, 0, c->meta>>>(c->d_gain, n, U, need, c->d_used, c->NB, c->d_counters);
+  CKL();
+  c->st.kernel_launches++;
+  CK(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->meta));
+  CK(cudaStreamSynchronize(c->meta));
+  const u32 oc = c->h_counters[0], lo = c->h_counters[1], hi = c->h_counters[2];
+  if (oc == VO_FITS) { *status = RC_ST_OK; return RC_OK; }
+  if (oc == VO_NOFREE) { *status = RC_ST_NO_FREE_BLOCKS; return RC_OK; }
+  const u32 m = hi - lo;
+  for (u32 k = 0; k < m; ++k) {
+    fill_desc(hd[k], *list[lo + k], D_ELIG);
+    if (*n_ids < cap) ids[*n_ids] = list[lo + k]->id;
+    ++*n_ids;
+  }
+  if ((rc = upload_desc(c, 2, m))) return rc;
+  if (oc == VO_EVICT) {
+    // ordered release: DEMOTED is on the stream before the references are dropped (claim_demoted_before_loss)
+    if ((rc = emit(c, 2, m, EM_DEMOTE, request_id))) return rc;
+    k_unref<<<warps_grid(m), 256, 0, c->meta>>>(c->d_desc[2], m, c->d_bt, c->d_used, c->d_ref);
+    CKL();
+    c->st.kernel_launches++;
+    CK(cudaStreamSynchronize(c->meta));
+    for (u32 k = 0; k < m; ++k) {
+      Claim& cl = *list[k];
+      c->bt_alloc.release(cl.bt_off, cl.bt_len);
+      cl.bt_len = 0;
+      cl.state = RC_CS_DEMOTED;
+    }
+    *status = RC_ST_OK;
+  } else {                                                 // nothing is evicted; the request is refused, naming the blockers
+    if ((rc = emit(c, 2, m, EM_CONFLICT, request_id))) return rc;
+    CK(cudaStreamSynchronize(c->meta));
+    *status = RC_ST_PROTECTED_CONFLICT;
+  }
+  c->ev_emitted += m;
+  return RC_OK;
+}
+
+extern "C" int rc_protected_map(rc_ctx* c, uint8_t* prot) {
+  GUARD();
+  if (!prot) return RC_ERR_INVALID;
+  if (c->ops[0].active || c->ops[1].active) return RC_ERR_BUSY;
+  std::vector<Claim*> list;
+  u32 U = 0;
+  victim_list(c, list, U);
+  const u32 n = (u32)list.size();
+  if (n > c->desc_cap) return RC_ERR_CAPACITY;
+  Desc* hd = c->h_desc[2];
+  for (u32 k = 0; k < n; ++k) fill_desc(hd[k], *list[k], D_ELIG | (list[k]->protect ? (u32)D_PROT : 0u));
+  CK(cudaMemsetAsync(c->d_protmap, 0, c->NB, c->meta));
+  if (n) {
+    int rc;
+    if ((rc = upload_desc(c, 2, n))) return rc;
+    k_prot_map<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[2], n, c->d_bt, c->d_protmap);
+    CKL();
+    c->st.kernel_launches++;
+  }
+  CK(cudaMemcpyAsync(prot, c->d_protmap, c->NB, cudaMemcpyDeviceToHost, c->meta));
+  CK(cudaStreamSynchronize(c->meta));
+  return RC_OK;
+}
+
 // ---- outcomes, faults, release -----------------------------------------------------------------------------
 extern "C" int rc_outcomes(rc_ctx* c, rc_event* buf, uint64_t cap, uint64_t* n_out) {
   GUARD();
@@ -1139,14 +1260,15 @@ extern "C" int rc_digest_blocks(rc_ctx* c, const void* src, uint32_t n_blocks, u
 // ---- NEXT-1: trace validator ----------------------------------------------------------------------------------------
 extern "C" int rc_validate_trace(const rc_event* events, uint64_t n, rc_trace_report* rep, rc_trace_claim* claims, uint64_t cap) {
   using namespace rct;
-  if (!rep || (n && !events) || n > 0xFFFFFFF0ull) return RC_ERR_INVALID;
+  if (!rep || (n && !events) || n > (1ull << 30)) return RC_ERR_INVALID;   // the claim table is 2n slots rounded up, in u32
   memset(rep, 0, sizeof(*rep));
   rep->first_bad_index = NO_BAD; rep->n_events = n; rep->ok = 1;
   if (n == 0) return RC_OK;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return RC_ERR_CUDA;
-  u32 slots = 1024;
-  while ((u64)slots < 2 * n) slots <<= 1;
+  u64 slots64 = 1024;
+  while (slots64 < 2 * n) slots64 <<= 1;
+  const u32 slots = (u32)slots64;                          // <= 2^31 by the bound on n
   Event* d_ev = nullptr; u64* d_keys = nullptr; u32 *d_count = nullptr, *d_base = nullptr, *d_dense = nullptr, *d_fill = nullptr;
   u32 *d_slot = nullptr, *d_bucket = nullptr, *d_cur = nullptr, *d_bsum = nullptr; unsigned long long* d_bad = nullptr; ClaimOut* d_out = nullptr;
   cudaStream_t st = nullptr; cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr, e3 = nullptr;

@@ -45,7 +45,7 @@ struct Desc {
   u32 src_off;            // accept: offset of the candidate table in the upload buffer
   u32 pad;                // restore: the claim's failure policy (POL_*)
 };
-enum { D_ELIG = 1, D_XFER = 2 };
+enum { D_ELIG = 1, D_XFER = 2, D_PROT = 4 };
 
 // per-claim result of a call (device fills, host reads)
 struct Res {
@@ -58,7 +58,9 @@ enum { R_OK = 1, R_SERVED = 2 };
 struct Event { u64 seq, claim_id; u32 code, aux; u64 arg; };
 enum { EV_ACCEPTED = 1, EV_MATERIALIZED = 2, EV_OFFLOADED = 3, EV_RESTORE_REQUIRED = 4, EV_LOAD_FAILED = 5,
        EV_RESTORED = 6, EV_RESTORATION_FAILED = 7, EV_ACTIVE_REQUEST_REFUSED = 8 };
-enum { EM_ACCEPT = 0, EM_MATERIALIZE = 1, EM_OFFLOAD = 2, EM_RESTORE = 3 };
+enum { EM_ACCEPT = 0, EM_MATERIALIZE = 1, EM_OFFLOAD = 2, EM_RESTORE = 3, EM_DEMOTE = 4, EM_CONFLICT = 5 };
+enum { EV_CONFLICT_REFUSED = 11 };                   // NEXT-3: active_request_refused(blocking_claim_ids) under hard protection
+enum { VO_FITS = 0, VO_EVICT = 1, VO_CONFLICT = 2, VO_NOFREE = 3 };   // outcome of k_vic_decide
 enum { EV_DEMOTED = 9, EV_EXPIRED = 10 };            // NEXT-3: other claim-scoped outcomes of a failed restoration
 enum { POL_REFUSE = 0, POL_DEMOTE = 1, POL_EXPIRE = 2 };   // Desc.pad carries the claim's failure policy
 constexpr u32 REQ_FLAG = 0x80000000u;                // REFUSED.aux of a request-level refusal: flag | subset size
@@ -571,6 +573,7 @@ __global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ re
     if (k < n) {
       d = desc[k]; r = res[k];
       if (mode == EM_RESTORE) c = (r.flag & R_SERVED) ? ((r.flag & R_OK) ? 2u : (blocks_request(d, r) ? 3u : 4u)) : 0u;
+      else if (mode == EM_DEMOTE || mode == EM_CONFLICT) c = (d.flags & D_ELIG) ? 1u : 0u;
       else c = (r.flag & R_OK) ? 1u : 0u;
     }
     u32 tot;
@@ -584,6 +587,8 @@ __global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ re
       if (mode == EM_ACCEPT) put(EV_ACCEPTED, d.N, d.P);
       else if (mode == EM_MATERIALIZE) put(EV_MATERIALIZED, r.val, 0);
       else if (mode == EM_OFFLOAD) put(EV_OFFLOADED, d.nb, r.chain);
+      else if (mode == EM_DEMOTE) put(EV_DEMOTED, d.bt_len, request_id);          // victim: the boundary precedes the loss
+      else if (mode == EM_CONFLICT) put(EV_CONFLICT_REFUSED, REQ_FLAG | n, request_id);   // all n descs are blocking claims
       else {
         put(EV_RESTORE_REQUIRED, d.M, 0);
         if (r.flag & R_OK) put(EV_RESTORED, d.nb, d.chain);
@@ -627,6 +632,71 @@ __global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ re
   }
   __syncthreads();
   if (threadIdx.x == 0) *ev_count = seq0 + carry + carry_b;
+}
+
+// ---------------------------------------------------------------------------------------------
+// K5, allocator-side protection (NEXT-3; P:L85 victim_exclusion_before_violation, P:L270 allocator_hook).
+// Candidates arrive in victim order (unprotected first, then protected; acceptance order inside each group).
+// Evicting the first m candidates frees the blocks whose every holder is among them: block b is freed by the
+// LAST of its holders in list order, so gain[k] = #{b in table k : posmax[b] == k+1} with posmax[b] = the largest
+// list position (+1) of a holder of b, and the free count after evicting m claims is F + sum_{k<m} gain[k].
+// ---------------------------------------------------------------------------------------------
+__global__ void k_vic_posmax(const Desc* __restrict__ desc, u32 n, const u32* __restrict__ bt, u32* __restrict__ posmax) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= n) return;
+  const Desc d = desc[k];
+  for (u32 i = lane; i < d.bt_len; i += 32) atomicMax(&posmax[bt[d.bt_off + i]], k + 1);
+}
+__global__ void k_vic_gain(const Desc* __restrict__ desc, u32 n, const u32* __restrict__ bt, const u32* __restrict__ posmax,
+                           u32* __restrict__ gain) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= n) return;
+  const Desc d = desc[k];
+  u32 g = 0;
+  for (u32 i = lane; i < d.bt_len; i += 32) g += posmax[bt[d.bt_off + i]] == k + 1;
+  g = warp_sum32(g);
+  if (lane == 0) gain[k] = g;
+}
+// One CTA.  F = free blocks; m = the shortest prefix with F + sum gain >= need.  U = number of unprotected candidates.
+// out[0] = outcome (VO_*), out[1] = first list position concerned, out[2] = one past the last, out[3] = F.
+__global__ void k_vic_decide(const u32* __restrict__ gain, u32 n, u32 U, u32 need, const u8* __restrict__ used, u32 NB,
+                             u32* __restrict__ out) {
+  __shared__ u32 wt[32];
+  __shared__ u32 s_m;
+  u32 cnt = 0;
+  for (u32 b = threadIdx.x; b < NB; b += blockDim.x) cnt += used[b] == 0;
+  u32 F;
+  block_scan_incl(cnt, wt, F);
+  if (threadIdx.x == 0) s_m = 0xFFFFFFFFu;
+  __syncthreads();
+  u32 carry = F;
+  for (u32 base = 0; base < n && F < need; base += blockDim.x) {
+    const u32 k = base + threadIdx.x;
+    u32 tot;
+    const u32 inc = carry + block_scan_incl(k < n ? gain[k] : 0u, wt, tot);
+    if (k < n && inc >= need) atomicMin(&s_m, k + 1);
+    carry += tot;
+    __syncthreads();
+    if (s_m != 0xFFFFFFFFu) break;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const u32 m = s_m;
+    u32 oc, lo = 0, hi = 0;
+    if (F >= need) oc = VO_FITS;
+    else if (m != 0xFFFFFFFFu && m <= U) { oc = VO_EVICT; lo = 0; hi = m; }
+    else if (U == n) oc = VO_NOFREE;
+    else { oc = VO_CONFLICT; lo = U; hi = m != 0xFFFFFFFFu ? m : n; }
+    out[0] = oc; out[1] = lo; out[2] = hi; out[3] = F;
+  }
+}
+// the protected resident footprint as a byte map (rc_protected_map)
+__global__ void k_prot_map(const Desc* __restrict__ desc, u32 n, const u32* __restrict__ bt, u8* __restrict__ map) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (k >= n) return;
+  const Desc d = desc[k];
+  if (!(d.flags & D_PROT)) return;
+  for (u32 i = lane; i < d.bt_len; i += 32) map[bt[d.bt_off + i]] = 1;
 }
 
 // fault injection (CPU->GPU transfers only): flip bit 0 of the listed staged bytes

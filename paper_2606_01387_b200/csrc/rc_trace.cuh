@@ -9,6 +9,10 @@
 //   REQUEST_FINISHED(C) between LOAD_FAILED and REFUSED is invalid: outcome precedes terminal handling;
 //   LOAD_FAILED / RESTORATION_FAILED / REFUSED without RESTORE_REQUIRED(C) in the same cycle is invalid;
 //   REFUSED must carry blocking_claim_ids = [C] (aux 1, arg C).
+// Allocator-side protection (NEXT-3): DEMOTED(C, arg = request id != 0) while C is resident is
+// the ordered demotion of a victim before its blocks are lost (after RESTORATION_FAILED, DEMOTED keeps arg = 0);
+// CONFLICT_REFUSED(C, aux = REQ_FLAG | k, arg = request id != 0) names a resident claim that blocks an active request;
+// the k records of one refusal are consecutive and name k different claims.
 #pragma once
 #include "rc_kernels.cuh"
 
@@ -23,17 +27,17 @@ constexpr u64 NO_BAD = ~0ull;
 struct ClaimOut { u64 claim_id; u64 first_bad; u32 state; u32 gates; u32 n_events; u32 pad; };
 
 __device__ __forceinline__ int col_of(u32 code) {
-  return code >= 1 && code <= 8 ? (int)code - 1 : (code == EV_USE ? 8 : (code == EV_FIN ? 9 : (code == EV_DEMOTED ? 10 : (code == EV_EXPIRED ? 11 : -1))));
+  return code >= 1 && code <= 8 ? (int)code - 1 : (code == EV_USE ? 8 : (code == EV_FIN ? 9 : (code == EV_DEMOTED ? 10 : (code == EV_EXPIRED ? 11 : (code == EV_CONFLICT_REFUSED ? 12 : -1)))));
 }
 
 // next-state table [state][column]; BAD = not in the accepted language
 __device__ __forceinline__ u32 next_state(u32 s, int col) {
   // columns: 0 ACCEPTED 1 MATERIALIZED 2 OFFLOADED 3 RESTORE_REQUIRED 4 LOAD_FAILED 5 RESTORED 6 RESTORATION_FAILED 7 REFUSED 8 USE 9 FIN
-  //          10 DEMOTED 11 EXPIRED (NEXT-3)
+  //          10 DEMOTED 11 EXPIRED 12 CONFLICT_REFUSED (NEXT-3)
   switch (s) {
     case S0:   return col == 0 ? ACC : BAD;
-    case ACC:  return col == 1 ? MAT : (col == 9 ? FIN : BAD);
-    case MAT:  return col == 2 ? OFF : (col == 8 ? MAT : (col == 9 ? FIN : BAD));
+    case ACC:  return col == 1 ? MAT : (col == 9 ? FIN : (col == 10 ? DEM : (col == 12 ? ACC : BAD)));
+    case MAT:  return col == 2 ? OFF : (col == 8 ? MAT : (col == 9 ? FIN : (col == 10 ? DEM : (col == 12 ? MAT : BAD))));
     case OFF:  return col == 3 ? RREQ : BAD;
     case RREQ: return col == 5 ? RES : (col == 4 ? LF : BAD);
     case LF:   return col == 6 ? RF : BAD;
@@ -41,7 +45,7 @@ __device__ __forceinline__ u32 next_state(u32 s, int col) {
     case REF:  return col == 9 ? FIN : BAD;
     case DEM:  return col == 9 ? FIN : BAD;
     case EXP:  return col == 9 ? FIN : BAD;
-    case RES:  return col == 2 ? OFF : (col == 8 ? RES : (col == 9 ? FIN : BAD));
+    case RES:  return col == 2 ? OFF : (col == 8 ? RES : (col == 9 ? FIN : (col == 10 ? DEM : (col == 12 ? RES : BAD))));
     default:   return BAD;
   }
 }
@@ -98,25 +102,49 @@ __global__ void tv_walk(const Event* __restrict__ ev, const u64* __restrict__ ke
   const u32 c = count[s];
   if (c == 0) return;
   u32* b = bucket + base[s];
-  for (u32 i = 1; i < c; ++i) {                 // insertion sort: a claim has a handful of events
-    const u32 x = b[i];
-    u32 j = i;
-    while (j > 0 && b[j - 1] > x) { b[j] = b[j - 1]; --j; }
-    b[j] = x;
+  if (c <= 16) {                                // a claim has a handful of events: insertion sort
+    for (u32 i = 1; i < c; ++i) {
+      const u32 x = b[i];
+      u32 j = i;
+      while (j > 0 && b[j - 1] > x) { b[j] = b[j - 1]; --j; }
+      b[j] = x;
+    }
+  } else {                                      // a claim with many events (long USE runs, many cycles): heap sort, O(c log c)
+    auto sift = [&](u32 root, u32 end) {
+      for (;;) {
+        u32 ch = 2 * root + 1;
+        if (ch >= end) break;
+        if (ch + 1 < end && b[ch + 1] > b[ch]) ++ch;
+        if (b[root] >= b[ch]) break;
+        const u32 t = b[root]; b[root] = b[ch]; b[ch] = t;
+        root = ch;
+      }
+    };
+    for (u32 i = c / 2; i-- > 0;) sift(i, c);
+    for (u32 end = c - 1; end > 0; --end) { const u32 t = b[0]; b[0] = b[end]; b[end] = t; sift(0, end); }
   }
   const u64 cid = keys[s];
   u32 st = S0, n_codes = 0, c0 = 0, c1 = 0, tail = 0;   // tail: last five lifecycle codes, 4 bits each
   bool saw_fail = false;
   u64 bad = NO_BAD;
+  u64 cr_arg = 0; u32 cr_aux = 0, cr_pos = 0; bool cr_any = false;   // the claim's last CONFLICT_REFUSED record
   for (u32 i = 0; i < c; ++i) {
     const Event e = ev[b[i]];
     const int col = col_of(e.code);
     u32 nx = col < 0 ? (u32)BAD : next_state(st, col);
+    // DEMOTED: arg = 0 after a failed restoration, = the request id for a victim of rc_make_room
+    if (nx != BAD && col == 10 && ((e.arg == 0) != (st == RF))) nx = BAD;
+    if (nx != BAD && col == 12) {
+      const u32 k = e.aux & ~REQ_FLAG;
+      if (!(e.aux & REQ_FLAG) || k == 0 || e.arg == 0) nx = BAD;
+      else if (cr_any && cr_arg == e.arg && cr_aux == e.aux && b[i] - cr_pos < k) nx = BAD;   // named twice in one run
+      cr_any = true; cr_arg = e.arg; cr_aux = e.aux; cr_pos = b[i];
+    }
     // per-claim refusal carries [C] itself; the request form (REQ_FLAG) is checked across claims by tv_groups
     if (nx != BAD && e.code == EV_ACTIVE_REQUEST_REFUSED && !(e.aux & REQ_FLAG) && (e.arg != cid || e.aux != 1)) nx = BAD;
     if (nx == BAD) { bad = b[i]; st = BAD; break; }
     st = nx;
-    if (col < 8 || col >= 10) {
+    if (col < 8 || col == 10 || col == 11) {
       if (n_codes == 0) c0 = e.code; else if (n_codes == 1) c1 = e.code;
       tail = ((tail << 4) | e.code) & 0xFFFFFu;
       ++n_codes;
@@ -137,14 +165,15 @@ __global__ void tv_walk(const Event* __restrict__ ev, const u64* __restrict__ ke
 // ---- request-level refusal runs (NEXT-3) -----------------------------------------------------
 // pending(i) = claims whose restoration failed and is unanswered before stream position i
 //            = #RESTORATION_FAILED - #(REFUSED | DEMOTED | EXPIRED) among events [0, i)   (valid up to the first violation).
-__device__ __forceinline__ u32 pend_delta(u32 code) {
-  return code == EV_RESTORATION_FAILED ? 1u : ((code == EV_ACTIVE_REQUEST_REFUSED || code == EV_DEMOTED || code == EV_EXPIRED) ? 0xFFFFFFFFu : 0u);
+__device__ __forceinline__ u32 pend_delta(const Event& e) {
+  return e.code == EV_RESTORATION_FAILED ? 1u
+       : ((e.code == EV_ACTIVE_REQUEST_REFUSED || (e.code == EV_DEMOTED && e.arg == 0) || e.code == EV_EXPIRED) ? 0xFFFFFFFFu : 0u);
 }
 __global__ void tv_delta_sum(const Event* __restrict__ ev, u64 n, u32* __restrict__ bsum) {
   __shared__ u32 wt[32];
   const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
   u32 tot;
-  block_scan_incl(i < n ? pend_delta(ev[i].code) : 0u, wt, tot);
+  block_scan_incl(i < n ? pend_delta(ev[i]) : 0u, wt, tot);
   if (threadIdx.x == 0) bsum[blockIdx.x] = tot;
 }
 __global__ void tv_scan_bsum(u32* __restrict__ bsum, u32 nb) {          // exclusive scan in place, one CTA
@@ -160,8 +189,8 @@ __global__ void tv_scan_bsum(u32* __restrict__ bsum, u32 nb) {          // exclu
     __syncthreads();
   }
 }
-__device__ __forceinline__ bool same_run(const Event& a, u64 arg, u32 aux) {
-  return a.code == EV_ACTIVE_REQUEST_REFUSED && a.arg == arg && a.aux == aux;
+__device__ __forceinline__ bool same_run(const Event& a, u32 code, u64 arg, u32 aux) {
+  return a.code == code && a.arg == arg && a.aux == aux;
 }
 // A run of REFUSED records with the same (arg = request id, aux = REQ_FLAG | k) starts where the previous record does
 // not match.  The start checks: k >= 1 and k == pending (the run names exactly the failed, unanswered claims: neither
@@ -172,16 +201,17 @@ __global__ void tv_groups(const Event* __restrict__ ev, u64 n, const u32* __rest
   const u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
   Event e; e.code = 0; e.aux = 0; e.arg = 0;
   if (i < n) e = ev[i];
-  const u32 d = i < n ? pend_delta(e.code) : 0u;
+  const u32 d = i < n ? pend_delta(e) : 0u;
   u32 tot;
   const u32 pending = boff[blockIdx.x] + block_scan_incl(d, wt, tot) - d;
-  if (i >= n || e.code != EV_ACTIVE_REQUEST_REFUSED || !(e.aux & REQ_FLAG)) return;
-  if (i > 0 && same_run(ev[i - 1], e.arg, e.aux)) return;                // not a run start
+  const bool conflict = e.code == EV_CONFLICT_REFUSED;                   // same run shape, no pending rule
+  if (i >= n || !(e.code == EV_ACTIVE_REQUEST_REFUSED || conflict) || !(e.aux & REQ_FLAG)) return;
+  if (i > 0 && same_run(ev[i - 1], e.code, e.arg, e.aux)) return;        // not a run start
   const u32 k = e.aux & ~REQ_FLAG;
-  if (k == 0 || k != pending) { atomicMin(first_bad, (unsigned long long)i); return; }
+  if (k == 0 || (!conflict && k != pending)) { atomicMin(first_bad, (unsigned long long)i); return; }
   for (u32 j = 1; j < k && i + j < n; ++j)
-    if (!same_run(ev[i + j], e.arg, e.aux)) { atomicMin(first_bad, (unsigned long long)(i + j)); return; }
-  if (i + k < n && same_run(ev[i + k], e.arg, e.aux)) atomicMin(first_bad, (unsigned long long)(i + k));
+    if (!same_run(ev[i + j], e.code, e.arg, e.aux)) { atomicMin(first_bad, (unsigned long long)(i + j)); return; }
+  if (i + k < n && same_run(ev[i + k], e.code, e.arg, e.aux)) atomicMin(first_bad, (unsigned long long)(i + k));
 }
 
 }  // namespace rct

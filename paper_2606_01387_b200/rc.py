@@ -17,7 +17,7 @@ FAULT_DTYPE = np.dtype([("claim_id", "<u8"), ("kind", "<u4"), ("param", "<u4")])
 
 OK, ERR_INVALID, ERR_CUDA, ERR_NOMEM, ERR_CAPACITY, ERR_BUSY = 0, -1, -2, -3, -4, -5
 ST_OK, ST_PRED_FALSE, ST_UNKNOWN_CLAIM, ST_BAD_STATE, ST_DUPLICATE_ID, ST_BAD_TABLE = 0, 1, 2, 3, 4, 5
-ST_NO_FREE_BLOCKS, ST_NO_HOST_SPACE, ST_RESTORE_FAILED = 6, 7, 8
+ST_NO_FREE_BLOCKS, ST_NO_HOST_SPACE, ST_RESTORE_FAILED, ST_PROTECTED_CONFLICT = 6, 7, 8, 9
 FAULT_XFER_ERROR, FAULT_BITFLIP, FAULT_ALLOW_UNCLAIMED = 1, 2, 1
 MOVER_AUTO, MOVER_LDG, MOVER_TMA = 0, 1, 2
 REQ_FLAG = 0x80000000
@@ -25,7 +25,7 @@ POLICY_REFUSE, POLICY_DEMOTE, POLICY_EXPIRE = 0, 1, 2
 
 EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_accept", "rc_materialize", "rc_offload",
            "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_set_policy", "rc_restore_request",
-           "rc_restore_request_begin", "rc_outcomes", "rc_set_faults",
+           "rc_restore_request_begin", "rc_protect", "rc_make_room", "rc_protected_map", "rc_outcomes", "rc_set_faults",
            "rc_release", "rc_claim_info", "rc_claim_blocks", "rc_claim_digests", "rc_host_read", "rc_pool_state",
            "rc_stats_get", "rc_stats_reset", "rc_measure_link", "rc_digest_blocks", "rc_validate_trace", "rc_strerror",
            "rc_last_cuda_error"]
@@ -210,6 +210,23 @@ class RC:
     def set_policy(self, ids, policy):
         ids, policy = _u64(ids), _u32(policy)
         return self.L.rc_set_policy(self.h, ids.size, _p(ids), _p(policy))
+
+    def protect(self, ids, on):
+        ids, on = _u64(ids), _u32(on)
+        return self.L.rc_protect(self.h, ids.size, _p(ids), _p(on))
+
+    def make_room(self, request_id, need, cap=4096):
+        """Returns (status, ids): OK -> the claims demoted to make room; PROTECTED_CONFLICT -> blocking_claim_ids."""
+        st, n = C.c_int32(-1), C.c_uint32()
+        ids = np.zeros(cap, np.uint64)
+        self._ck(self.L.rc_make_room(self.h, C.c_uint64(request_id), C.c_uint32(need), C.byref(st), _p(ids), cap,
+                                     C.byref(n)), "rc_make_room")
+        return st.value, [int(x) for x in ids[: min(cap, n.value)]]
+
+    def protected_map(self):
+        prot = np.zeros(self.NB, np.uint8)
+        self._ck(self.L.rc_protected_map(self.h, _p(prot)), "rc_protected_map")
+        return prot
 
     def wait(self, which):
         self._ck(self.L.rc_wait(self.h, which), "rc_wait")

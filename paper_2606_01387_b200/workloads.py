@@ -253,251 +253,3 @@ def pool_torch(geom, device, seed=None):
 
 
 POISON = 0xA5   # byte written over freed blocks between offload and restore (DESIGN R5)
-
-
-# ---- synthetic event traces (inputs of the trace validator, NEXT-1) -----------------------------------
-TRACE_DTYPE = np.dtype([("seq", "<u8"), ("claim_id", "<u8"), ("code", "<u4"), ("aux", "<u4"), ("arg", "<u8")])
-T_USE, T_FIN = 100, 101
-TRACE_MUTATIONS = ["wrong_claim", "unclaimed", "restore_after_use", "finish_before_refused", "drop_restore_required",
-                   "swap_adjacent", "bad_blocking_ids", "seq_not_increasing", "generic_failure", "fallback_recompute"]
-
-
-def make_trace(n_claims, seed=0, fail_frac=0.1, cycles=(1, 3), markers=True):
-    """A valid interleaved stream: each claim runs ACCEPTED, MATERIALIZED, then 1..3 offload/restore cycles;
-    a fraction end in the failure path (the seven steps of P:L27); optional USE / REQUEST_FINISHED markers.
-    Events of different claims are interleaved at random, per-claim order kept.  Vectorised (10^6 claims ok)."""
-    rng = np.random.default_rng(SEED0 + 5000 + seed)
-    ids = rng.integers(1, 1 << 62, n_claims, dtype=np.uint64) * np.uint64(2) + np.uint64(1)
-    ids = np.unique(ids)
-    rng.shuffle(ids)
-    n = ids.size
-    ncyc = rng.integers(cycles[0], cycles[1] + 1, n)
-    fail = rng.random(n) < fail_frac
-    use = (rng.random(n) < 0.3) & ~fail & markers
-    fin = (rng.random(n) < 0.3) & markers
-    cols = []                                              # per-claim code sequences as padded columns
-    L = 2 + 3 * cycles[1] + 2 + 2
-    seqs = np.zeros((n, L), np.uint32)
-    ln = np.zeros(n, np.int64)
-
-    def push(mask, code):
-        idx = np.nonzero(mask)[0]
-        seqs[idx, ln[idx]] = code
-        ln[idx] += 1
-    allm = np.ones(n, bool)
-    push(allm, 1); push(allm, 2)
-    for cyc in range(cycles[1]):
-        act = ncyc > cyc
-        last = ncyc == cyc + 1
-        push(act, 3); push(act, 4)
-        push(act & ~(last & fail), 6)
-        push(act & last & fail, 5); push(act & last & fail, 7); push(act & last & fail, 8)
-    push(use, T_USE)
-    push(fin, T_FIN)
-    total = int(ln.sum())
-    owner = np.repeat(np.arange(n), ln)
-    within = np.arange(total) - np.repeat(np.cumsum(ln) - ln, ln)
-    t = rng.random(total)
-    # per-claim sorted times keep the claim's own order
-    order_in = np.lexsort((t, owner))
-    t_sorted = np.empty(total)
-    t_sorted[np.arange(total)] = t[order_in]
-    glob = np.argsort(t_sorted, kind="stable")
-    ev = np.zeros(total, TRACE_DTYPE)
-    code = seqs[owner, within]
-    ev["claim_id"] = ids[owner][glob]
-    ev["code"] = code[glob]
-    ev["seq"] = np.arange(total, dtype=np.uint64) * np.uint64(3) + np.uint64(7)
-    ref = ev["code"] == 8
-    ev["aux"][ref] = 1
-    ev["arg"][ref] = ev["claim_id"][ref]
-    return ev
-
-
-def mutate_trace(ev, kind, seed=0):
-    """One control-class mutation applied to a valid stream; returns a new array."""
-    rng = np.random.default_rng(SEED0 + 6000 + seed)
-    ev = ev.copy()
-    code, cid = ev["code"], ev["claim_id"]
-
-    def pick(mask):
-        idx = np.nonzero(mask)[0]
-        return int(idx[rng.integers(0, idx.size)]) if idx.size else None
-
-    def insert(pos, c, code_):
-        rec = np.zeros(1, TRACE_DTYPE)
-        rec["claim_id"], rec["code"] = c, code_
-        out = np.concatenate([ev[:pos], rec, ev[pos:]])
-        out["seq"] = np.arange(out.size, dtype=np.uint64) + np.uint64(1)
-        return out
-    if kind == "wrong_claim":                    # a failure record attributed to another claim
-        i = pick(code == 5)
-        other = cid[pick(cid != cid[i])]
-        ev["claim_id"][i] = other
-    elif kind == "unclaimed":
-        ev["claim_id"][pick(code == 5)] = 0
-    elif kind == "restore_after_use":            # USE(C) while C is offloaded
-        i = pick(code == 3)
-        return insert(i + 1, cid[i], T_USE)
-    elif kind == "finish_before_refused":        # terminal handling before the outcome (P:L380)
-        i = pick(code == 5)
-        return insert(i + 1, cid[i], T_FIN)
-    elif kind == "drop_restore_required":
-        i = pick(code == 4)
-        return np.delete(ev, i)
-    elif kind == "swap_adjacent":                # two consecutive events of one claim exchanged
-        i = pick(code == 3)
-        j = i + 1 + int(np.nonzero(cid[i + 1:] == cid[i])[0][0])
-        tmp = ev[["code", "aux", "arg"]][i].copy()
-        for f in ("code", "aux", "arg"):
-            a, b = ev[f][i], ev[f][j]
-            ev[f][i], ev[f][j] = b, a
-    elif kind == "bad_blocking_ids":             # blocking_claim_ids smeared onto another claim (P:L269)
-        i = pick(code == 8)
-        ev["arg"][i] = cid[pick(cid != cid[i])]
-    elif kind == "seq_not_increasing":
-        i = int(rng.integers(1, ev.size))
-        ev["seq"][i] = ev["seq"][i - 1]
-    elif kind == "generic_failure":              # failure records for a claim that was never restore-required
-        i = pick(code == 2)
-        return insert(i + 1, cid[i], 5)
-    elif kind == "fallback_recompute":           # RESTORED after a failed load (P:L492)
-        i = pick(code == 7)
-        ev["code"][i] = 6
-    else:
-        raise ValueError(kind)
-    return ev
-
-
-def make_shared_tiny(n_claims=6, seed=0, pool_blocks=256):
-    """Tiny geometry with prefix sharing (NEXT-2 inputs): claims share their leading blocks physically in
-    two groups, and `copies` lists (src, dst) block pairs whose bytes the harness makes identical, so that
-    different physical blocks carry the same content.  Returns (Workload, Wave, copies)."""
-    g0 = GEOMS[0]
-    g = Geometry(**{**g0.__dict__, "pool_blocks": pool_blocks})
-    rng = np.random.default_rng(SEED0 + 7000 + seed)
-    ids = _ids(rng, n_claims)
-    perm = [int(b) for b in rng.permutation(pool_blocks)]
-    cur = 0
-    groups = {}
-    for gi in range(2):
-        groups[gi] = perm[cur:cur + 24]
-        cur += 24
-    claims, offs, tab_all, fill = [], [0], [], {}
-    for k in range(n_claims):
-        P = int(rng.integers(448, 513))
-        nt = (P + g.block_size - 1) // g.block_size
-        shared = int(rng.integers(8, 25))
-        c = ClaimSpec(ids[k], P, N_PRED, P, k % 2, shared)
-        tab = groups[k % 2][:shared] + perm[cur:cur + nt - shared]
-        cur += nt - shared
-        for i, b in enumerate(tab):
-            fill[b] = max(fill.get(b, 0), g.block_size if i < shared else min(g.block_size, P - i * g.block_size))
-        claims.append(c)
-        tab_all.extend(tab)
-        offs.append(len(tab_all))
-    copies = [(tab_all[offs[0] + 26], tab_all[offs[1] + 27]), (tab_all[offs[2] + 25], tab_all[offs[2] + 26])]
-    fb = np.array(sorted(fill), dtype=np.uint32)
-    wave = Wave(list(range(n_claims)), np.array(offs, np.uint32), np.array(tab_all, np.uint32),
-                np.unique(np.array(tab_all, np.uint32)), fb, np.array([fill[int(b)] for b in fb], np.uint8), [], 0)
-    return Workload(0, g, claims), wave, copies
-
-
-REQ_FLAG = 0x80000000
-REQUEST_MUTATIONS = ["smeared_ids", "short_subset", "dropped_record", "extra_record", "other_request_id", "interrupted_run",
-                     "zero_subset", "early_finish"]
-
-
-def make_request_trace(n_requests, seed=0):
-    """Valid streams with multi-claim reuse requests (NEXT-3): every request names 2..5 offloaded claims; some fail
-    and are refused (request-level run), demoted or expired.  Returns (events, runs) where runs lists, per refused
-    request, the stream positions of its REFUSED records."""
-    rng = np.random.default_rng(SEED0 + 8000 + seed)
-    rows, hist, runs = [], [], []
-    next_id = 1
-    for r in range(n_requests):
-        m = int(rng.integers(2, 6))
-        cids = [int(next_id + 2 * j + 1) * 1000003 for j in range(m)]
-        next_id += 2 * m
-        for c in cids:
-            hist.append([(c, 1, 0, 0), (c, 2, 0, 0), (c, 3, 0, 0)])
-        req = 10 ** 12 + r
-        blocking = []
-        block = []
-        for c in cids:
-            block.append((c, 4, 0, 0))
-            u = rng.random()
-            if u < 0.55:
-                block.append((c, 6, 0, 0))
-            else:
-                block += [(c, 5, 0, 0), (c, 7, 0, 0)]
-                if u < 0.65:
-                    block.append((c, 9, 0, 0))
-                elif u < 0.75:
-                    block.append((c, 10, 0, 0))
-                else:
-                    blocking.append(c)
-        grp = [(c, 8, REQ_FLAG | len(blocking), req) for c in blocking]
-        rows.append((block, grp))
-    # histories interleaved at random (per-claim order kept), then the request blocks one after another
-    order = np.repeat(np.arange(len(hist)), 3)
-    rng.shuffle(order)
-    it = [iter(h) for h in hist]
-    flat = [next(it[k]) for k in order]
-    for block, grp in rows:
-        flat += block
-        if grp:
-            runs.append(list(range(len(flat), len(flat) + len(grp))))
-        flat += grp
-    ev = np.zeros(len(flat), TRACE_DTYPE)
-    for i, (c, code, aux, arg) in enumerate(flat):
-        ev[i] = (2 * i + 1, c, code, aux, arg)
-    return ev, runs
-
-
-def mutate_request_trace(ev, runs, kind, seed=0):
-    rng = np.random.default_rng(SEED0 + 9000 + seed)
-    ev = ev.copy()
-    big = [r for r in runs if len(r) >= 2] or runs
-    run = big[int(rng.integers(0, len(big)))]
-    req = ev["arg"][run[0]]
-
-    def reseq(a):
-        a["seq"] = np.arange(a.size, dtype=np.uint64) + np.uint64(1)
-        return a
-    if kind == "smeared_ids":                    # names a claim of the request that restored fine (P:L269)
-        start = run[0]
-        i = start - 1
-        while i >= 0 and ev["code"][i] != 6:
-            i -= 1
-        ev["claim_id"][run[-1]] = ev["claim_id"][i]
-    elif kind == "short_subset":                 # fewer ids than claims that failed
-        if len(run) >= 2:
-            ev["aux"][run] = REQ_FLAG | (len(run) - 1)
-            return reseq(np.delete(ev, run[-1]))
-        ev["aux"][run] = REQ_FLAG | 2
-    elif kind == "dropped_record":
-        return reseq(np.delete(ev, run[0])) if len(run) >= 2 else reseq(np.delete(ev, run[0] - 1))
-    elif kind == "extra_record":
-        return reseq(np.concatenate([ev[:run[-1] + 1], ev[run[-1]:run[-1] + 1], ev[run[-1] + 1:]]))
-    elif kind == "other_request_id":
-        ev["arg"][run[-1]] = req + np.uint64(12345)
-    elif kind == "interrupted_run":              # something else between the records of one run
-        if len(run) < 2:
-            ev["aux"][run] = REQ_FLAG | 2
-        else:
-            i = run[0] - 1
-            while ev["code"][i] not in (6, 9, 10, 3):
-                i -= 1
-            rec = np.zeros(1, TRACE_DTYPE)
-            rec["claim_id"], rec["code"] = ev["claim_id"][i], T_FIN
-            return reseq(np.concatenate([ev[:run[1]], rec, ev[run[1]:]]))
-    elif kind == "zero_subset":
-        ev["aux"][run] = REQ_FLAG
-    elif kind == "early_finish":                 # terminal handling before the request's outcome (P:L267, P:L380)
-        rec = np.zeros(1, TRACE_DTYPE)
-        rec["claim_id"], rec["code"] = ev["claim_id"][run[0]], T_FIN
-        return reseq(np.concatenate([ev[:run[0]], rec, ev[run[0]:]]))
-    else:
-        raise ValueError(kind)
-    return ev

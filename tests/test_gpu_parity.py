@@ -11,6 +11,7 @@ pytestmark = pytest.mark.gpu
 from oracle import rco, validator as V
 from paper_2606_01387_b200 import rc, workloads as W
 from parity_harness import Pair
+from shared_tiny import make_shared_tiny
 
 GOLD = [l.split("#")[0].strip() for l in open(__file__.rsplit("/", 1)[0] + "/golden/event_orders.txt")]
 GOLD = {l.split(":")[0].strip(): [x.strip() for x in l.split(":")[1].split(",")] for l in GOLD if l}
@@ -309,7 +310,7 @@ def test_bitflip_positions_across_chunk_boundaries():
 def test_dedup_shared_tiny_full_parity(mover, chunk_blocks):
     """Shared prefixes + identical content in different blocks: one held copy and one link transfer per
     distinct block, everything else (bytes, digests, chains, events, allocation) as without dedup."""
-    wl, wave, copies = W.make_shared_tiny()
+    wl, wave, copies = make_shared_tiny()
     ids = [c.claim_id for c in wl.claims]
     p = Pair(wl, 1 << 30, chunk_blocks=chunk_blocks, mover=mover, dedup=True, copies=copies)
     g = wl.geom
@@ -339,7 +340,7 @@ def test_dedup_config2_shared_prefixes_reduced():
 def test_dedup_overlapped_begin_wait_matches_synchronous_order():
     """restore(k) in flight while offload(k+1) dedups against the store: the restore's reference drops
     take effect at _begin, so the overlapped run equals the oracle's synchronous order."""
-    wl, wave, copies = W.make_shared_tiny()
+    wl, wave, copies = make_shared_tiny()
     ids = [c.claim_id for c in wl.claims]
     p = Pair(wl, 1 << 30, chunk_blocks=11, dedup=True, copies=copies)
     o, r = p.o, p.r

@@ -8,10 +8,11 @@ import numpy as np
 
 from oracle import rco, validator as V
 from paper_2606_01387_b200 import workloads as W
+from shared_tiny import make_shared_tiny
 
 
 def build(dedup, host=1 << 40):
-    wl, wave, copies = W.make_shared_tiny()
+    wl, wave, copies = make_shared_tiny()
     g = wl.geom
     pool = W.pool_host(g)
     view = pool.reshape(2 * g.layers, g.pool_blocks, g.page_bytes)
