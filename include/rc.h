@@ -218,6 +218,14 @@ int rc_claim_blocks(rc_ctx* ctx, uint64_t claim_id, uint32_t* ids, uint32_t cap,
  * the 128-bit content key of block i (DESIGN.md "Checksum" R22). */
 int rc_claim_digests(rc_ctx* ctx, uint64_t claim_id, uint64_t* d, uint64_t* e, uint32_t cap, uint32_t* n);
 int rc_host_read(rc_ctx* ctx, uint64_t claim_id, void* dst, uint64_t cap, uint64_t* bytes);
+/* Borrowed, READ-ONLY view of the claim's host copy: *p = the pinned-store address of the claim's block `block` (offload
+ * order: block-major, then page g = layer*2 + kv), *contiguous_bytes = how many bytes from there belong to the claim and
+ * are contiguous (a claim's bytes may be split over several extents of the store).  Valid until the claim is restored,
+ * released or offloaded again; RC_ERR_BUSY while the claim's offload is in flight; RC_ERR_INVALID if the claim holds no
+ * such host block.  (rc_host_read is the copying form.) */
+int rc_host_store(rc_ctx* ctx, uint64_t claim_id, uint32_t block, const void** p, uint64_t* contiguous_bytes);
+/* Completes every in-flight operation (as rc_wait(0), rc_wait(1)) and drains the library's streams. */
+int rc_sync(rc_ctx* ctx);
 int rc_pool_state(rc_ctx* ctx, uint8_t* used /*NB*/, uint32_t* ref /*NB*/);
 int rc_stats_get(rc_ctx* ctx, rc_stats* out);
 int rc_stats_reset(rc_ctx* ctx);

@@ -1165,6 +1165,39 @@ extern "C" int rc_host_read(rc_ctx* c, uint64_t id, void* dst, uint64_t cap, uin
   }
   return RC_OK;
 }
+extern "C" int rc_host_store(rc_ctx* c, uint64_t id, uint32_t block, const void** p, uint64_t* contiguous_bytes) {
+  GUARD();
+  auto it = c->claims.find(id);
+  if (it == c->claims.end() || !p || !contiguous_bytes) return RC_ERR_INVALID;
+  const Claim& cl = it->second;
+  if (cl.busy) return RC_ERR_BUSY;                         // an in-flight offload is still writing it
+  *p = nullptr; *contiguous_bytes = 0;
+  if (!cl.hslots.empty()) {                                // dedup store: one slot per block
+    if (block >= cl.hslots.size()) return RC_ERR_INVALID;
+    u64 run = 1;
+    while (block + run < cl.hslots.size() && cl.hslots[block + run] == cl.hslots[block] + run) ++run;
+    *p = c->h_store + (u64)cl.hslots[block] * c->blk; *contiguous_bytes = run * c->blk;
+    return RC_OK;
+  }
+  u64 at = 0;
+  for (auto& e : cl.host) {
+    if (block < at + e.second) {
+      *p = c->h_store + (e.first + (block - at)) * c->blk; *contiguous_bytes = (at + e.second - block) * c->blk;
+      return RC_OK;
+    }
+    at += e.second;
+  }
+  return RC_ERR_INVALID;                                   // the claim holds no host bytes, or fewer blocks
+}
+extern "C" int rc_sync(rc_ctx* c) {
+  GUARD();
+  int rc = wait_offload(c);
+  if (rc) return rc;
+  if ((rc = wait_restore(c))) return rc;
+  cudaStream_t ss[6] = {c->meta, c->gather, c->d2h, c->scatter, c->h2d, c->util};
+  for (cudaStream_t s : ss) CK(cudaStreamSynchronize(s));
+  return RC_OK;
+}
 extern "C" int rc_pool_state(rc_ctx* c, uint8_t* used, uint32_t* ref) {
   GUARD();
   if (used) CK(cudaMemcpyAsync(used, c->d_used, c->NB, cudaMemcpyDeviceToHost, c->util));

@@ -26,7 +26,7 @@ POLICY_REFUSE, POLICY_DEMOTE, POLICY_EXPIRE = 0, 1, 2
 EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_accept", "rc_materialize", "rc_offload",
            "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_set_policy", "rc_restore_request",
            "rc_restore_request_begin", "rc_protect", "rc_make_room", "rc_protected_map", "rc_outcomes", "rc_set_faults",
-           "rc_release", "rc_claim_info", "rc_claim_blocks", "rc_claim_digests", "rc_host_read", "rc_pool_state",
+           "rc_release", "rc_claim_info", "rc_claim_blocks", "rc_claim_digests", "rc_host_read", "rc_host_store", "rc_sync", "rc_pool_state",
            "rc_stats_get", "rc_stats_reset", "rc_measure_link", "rc_digest_blocks", "rc_validate_trace", "rc_strerror",
            "rc_last_cuda_error"]
 
@@ -130,6 +130,7 @@ class RC:
         if getattr(self, "h", None):
             self.L.rc_destroy(self.h)
             self.h = None
+        self.pool = self.fill = None                           # the caller's tensors are no longer needed
 
     def __del__(self):
         self.close()
@@ -274,6 +275,24 @@ class RC:
         out = np.zeros(nbytes.value, np.uint8)
         self.L.rc_host_read(self.h, C.c_uint64(cid), _p(out), C.c_uint64(out.size), C.byref(nbytes))
         return out
+
+    def host_store(self, cid, block=0, n_blocks=1):
+        """Borrowed read-only numpy view (no copy) of `n_blocks` host blocks of the claim starting at `block`;
+        None if they are not contiguous in the pinned store or the claim holds no host bytes."""
+        p, nbytes = C.c_void_p(), C.c_uint64()
+        if self.L.rc_host_store(self.h, C.c_uint64(cid), block, C.byref(p), C.byref(nbytes)) != 0:
+            return None
+        if nbytes.value < n_blocks * self.blk:
+            return None
+        buf = (C.c_uint8 * (n_blocks * self.blk)).from_address(p.value)
+        a = np.frombuffer(buf, np.uint8)
+        a.flags.writeable = False
+        return a
+
+    def sync(self):
+        self._ck(self.L.rc_sync(self.h), "rc_sync")
+        for which in (0, 1):
+            self._pending.pop(which, None)
 
     def pool_state(self):
         used = np.zeros(self.NB, np.uint8)
