@@ -22,7 +22,8 @@
  * DEVICE.  Calls without a _begin suffix are synchronous: on return the device work
  * is complete.  One caller thread per context.  A CUDA error poisons the context:
  * every later call returns RC_ERR_CUDA.  A call-level error (negative return) emits
- * no event and changes no claim.  There is no CPU fallback anywhere behind this
+ * no event and changes no claim (RC_ERR_CUDA excepted: the context is poisoned and claim state is then undefined).
+ * There is no CPU fallback anywhere behind this
  * interface: every step of the path runs in the library's sm_100a kernels and its
  * copy-engine transfers.  Stream order: the library's streams are not ordered against
  * the caller's; writes the caller makes to pool_dev / fill_dev must have completed
@@ -231,7 +232,9 @@ int rc_stats_get(rc_ctx* ctx, rc_stats* out);
 int rc_stats_reset(rc_ctx* ctx);
 
 /* Host-link ceiling: best-of-`reps` cudaMemcpyAsync of `bytes` between the context's pinned
- * store and its staging ring; direction 0 = D2H, 1 = H2D, 2 = both at once (sum).  GB/s. */
+ * store and its staging ring; direction 0 = D2H, 1 = H2D, 2 = both at once (sum).  GB/s.  The copies write over the
+ * pinned store and the staging ring, so the call is refused with RC_ERR_BUSY while an operation is in flight or
+ * any claim holds host bytes. */
 int rc_measure_link(rc_ctx* ctx, uint64_t bytes, int direction, int reps, double* gbs);
 
 /* Standalone checksum of `n_blocks` contiguous blocks at DEVICE address src (offload order):

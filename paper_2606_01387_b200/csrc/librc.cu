@@ -420,22 +420,26 @@ extern "C" int rc_mark_used(rc_ctx* c, uint32_t n, const uint32_t* ids) { return
 extern "C" int rc_mark_free(rc_ctx* c, uint32_t n, const uint32_t* ids) { return mark(c, n, ids, 0); }
 
 // ---- a0 accept -----------------------------------------------------------------------------------
+constexpr u64 NO_EXT = ~0ull;
+static bool accept_shape_ok(rc_ctx* c, u64 id, u32 P, u32 N, u32 o0, u32 o1) {
+  return id != 0 && P != 0 && N != 0 && N <= P && o1 >= o0 && o1 - o0 == ceil_div(P, c->cfg.block_size);
+}
+// One run of a batch (no id twice inside a run).  ext[k] = the table extent rc_accept reserved for entry k before the
+// first run (NO_EXT for entries whose shape is invalid); an extent that ends up unused is given back here.
 static int accept_run(rc_ctx* c, u32 n, const u64* id, const u32* P, const u32* N, const u32* bt_off, const u32* bt_ids,
-                      int32_t* st) {
+                      int32_t* st, u64* ext) {
   Desc* hd = c->h_desc[2];
   std::vector<u32> cand;
   u64 up = 0;
-  auto rollback = [&]() { for (u32 k : cand) c->bt_alloc.release(hd[k].bt_off, hd[k].bt_len); };
+  auto give_back = [&](u32 k) { if (ext[k] != NO_EXT) { c->bt_alloc.release(ext[k], bt_off[k + 1] - bt_off[k]); ext[k] = NO_EXT; } };
   for (u32 k = 0; k < n; ++k) {
     memset(&hd[k], 0, sizeof(Desc));
     hd[k].id = id[k];
-    if (id[k] == 0) { st[k] = RC_ST_UNKNOWN_CLAIM; continue; }          // 0 is "no claim"
-    if (c->claims.count(id[k])) { st[k] = RC_ST_DUPLICATE_ID; continue; } // duplicate ownership
-    if (P[k] == 0 || N[k] == 0 || N[k] > P[k] || bt_off[k + 1] < bt_off[k] ||
-        bt_off[k + 1] - bt_off[k] != ceil_div(P[k], c->cfg.block_size)) { st[k] = RC_ST_BAD_TABLE; continue; }
+    if (id[k] == 0) { st[k] = RC_ST_UNKNOWN_CLAIM; give_back(k); continue; }          // 0 is "no claim"
+    if (c->claims.count(id[k])) { st[k] = RC_ST_DUPLICATE_ID; give_back(k); continue; } // duplicate ownership
+    if (!accept_shape_ok(c, id[k], P[k], N[k], bt_off[k], bt_off[k + 1])) { st[k] = RC_ST_BAD_TABLE; give_back(k); continue; }
     const u32 nt = bt_off[k + 1] - bt_off[k];
-    u64 o;
-    if (up + nt > c->cap_entries || !c->bt_alloc.alloc(nt, o)) { rollback(); return RC_ERR_CAPACITY; }
+    const u64 o = ext[k];
     hd[k].P = P[k]; hd[k].N = N[k]; hd[k].bt_off = (u32)o; hd[k].bt_len = nt; hd[k].flags = D_ELIG;
     hd[k].src_off = (u32)up;
     memcpy(c->h_up + up, bt_ids + bt_off[k], (u64)nt * 4);
@@ -466,6 +470,7 @@ static int accept_run(rc_ctx* c, u32 n, const u64* id, const u32* P, const u32* 
       c->bt_alloc.release(hd[k].bt_off, hd[k].bt_len);
       st[k] = RC_ST_BAD_TABLE;
     }
+    ext[k] = NO_EXT;
   }
   return RC_OK;
 }
@@ -476,17 +481,34 @@ extern "C" int rc_accept(rc_ctx* c, uint32_t n, const uint64_t* id, const uint32
   if (n == 0) return RC_OK;
   if (!id || !P || !N || !bt_off || !st || (bt_off[n] && !bt_ids)) return RC_ERR_INVALID;
   if (c->claims.size() + n > c->cfg.max_claims || !ev_room(c, n)) return RC_ERR_CAPACITY;
+  // every table extent of the batch is reserved before the first run mutates anything, so RC_ERR_CAPACITY leaves no
+  // claim accepted and no event emitted (rc.h: a negative return changes nothing)
+  std::vector<u64> ext(n, NO_EXT);
+  u64 per_run = 0;
+  bool fits = true;
+  for (u32 k = 0; k < n && fits; ++k) {
+    if (!accept_shape_ok(c, id[k], P[k], N[k], bt_off[k], bt_off[k + 1])) continue;
+    const u32 nt = bt_off[k + 1] - bt_off[k];
+    per_run += nt;
+    fits = per_run <= c->cap_entries && c->bt_alloc.alloc(nt, ext[k]);       // the upload buffer holds one run; a run <= the batch
+    if (!fits) ext[k] = NO_EXT;
+  }
+  if (!fits) {
+    for (u32 k = 0; k < n; ++k) if (ext[k] != NO_EXT) c->bt_alloc.release(ext[k], bt_off[k + 1] - bt_off[k]);
+    return RC_ERR_CAPACITY;
+  }
   // a run never holds the same id twice, so the runs reproduce one-by-one acceptance
   u32 s = 0;
-  while (s < n) {
+  int rc = RC_OK;
+  while (s < n && rc == RC_OK) {
     std::unordered_set<u64> seen;
     u32 e = s;
     while (e < n && e - s < c->desc_cap && (id[e] == 0 || seen.insert(id[e]).second)) ++e;
-    const int rc = accept_run(c, e - s, id + s, P + s, N + s, bt_off + s, bt_ids, st + s);
-    if (rc) return rc;
+    rc = accept_run(c, e - s, id + s, P + s, N + s, bt_off + s, bt_ids, st + s, ext.data() + s);
     s = e;
   }
-  return RC_OK;
+  for (u32 k = 0; k < n; ++k) if (ext[k] != NO_EXT) c->bt_alloc.release(ext[k], bt_off[k + 1] - bt_off[k]);   // CUDA error path
+  return rc;
 }
 
 // ---- a1 materialize --------------------------------------------------------------------------------
@@ -582,13 +604,15 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   std::vector<u32> served;
   bool full = false;
   u64 T = 0;
-  auto rollback = [&]() {
-    for (u32 k : served) {
-      Claim& cl = *op.cl[k];
+  std::vector<std::pair<u32, u32>> old_dg;                 // per served claim: the digest extent recorded by an earlier cycle
+  auto rollback = [&]() {                                  // a negative return changes no claim (rc.h)
+    for (size_t j = 0; j < served.size(); ++j) {
+      Claim& cl = *op.cl[served[j]];
       for (auto& e : cl.host) c->host_alloc.release(e.first, e.second);
       cl.host.clear();
       c->host_used -= (u64)cl.nb * c->blk;
-      if (cl.dg_len) { c->dg_alloc.release(cl.dg_off, cl.dg_len); cl.dg_len = 0; }
+      c->dg_alloc.release(cl.dg_off, cl.dg_len);
+      cl.dg_off = old_dg[j].first; cl.dg_len = old_dg[j].second;
       cl.busy = false;
     }
   };
@@ -601,9 +625,9 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     // no claim-less entry point exists: "ordinary offload without claim" cannot produce an outcome
     if (cl.busy || (cl.state != RC_CS_MATERIALIZED && cl.state != RC_CS_RESIDENT_AGAIN)) { st[k] = RC_ST_BAD_STATE; continue; }
     if (full || c->host_used + (u64)cl.nb * c->blk > c->cfg.host_store_bytes) { full = true; st[k] = RC_ST_NO_HOST_SPACE; continue; }
-    if (cl.dg_len) { c->dg_alloc.release(cl.dg_off, cl.dg_len); cl.dg_len = 0; }
-    u64 dgo;
+    u64 dgo;                                               // new extent first; the old one goes once the batch is admitted
     if (T + cl.nb > c->cap_entries || !c->dg_alloc.alloc(cl.nb, dgo)) { rollback(); return RC_ERR_CAPACITY; }
+    old_dg.push_back({cl.dg_off, cl.dg_len});
     cl.dg_off = (u32)dgo; cl.dg_len = cl.nb;
     cl.host.clear();
     // host space is granted by count in _begin order; the extents of a restore still in flight are
@@ -622,6 +646,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     st[k] = -1;
   }
   if (served.empty()) return RC_OK;
+  for (auto& od : old_dg) if (od.second) c->dg_alloc.release(od.first, od.second);
   op.n = n; op.status = st; op.blocks = T; op.copy_bytes = 0; op.launches = 0;
   int rc;
   // The head (offsets, compaction) only reads tables that completed calls wrote, so it runs on the gather
@@ -1230,6 +1255,7 @@ extern "C" int rc_measure_link(rc_ctx* c, uint64_t bytes, int direction, int rep
   GUARD();
   if (!gbs || direction < 0 || direction > 2 || reps < 1) return RC_ERR_INVALID;
   if (c->ops[0].active || c->ops[1].active) return RC_ERR_BUSY;
+  if (c->host_used != 0 || !c->store.empty()) return RC_ERR_BUSY;   // the measurement writes over the pinned store: only while it holds no claim bytes
   const u64 hs = c->host_blocks * c->blk, cs = c->chunk_blocks * c->blk;
   const u64 hmax = direction == 2 ? hs / 2 : hs;
   bytes = std::min(bytes, std::min(hmax, cs));

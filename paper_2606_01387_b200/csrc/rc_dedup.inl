@@ -44,10 +44,12 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
   std::vector<u64> first_w;
   bool full = false;
   u64 T = 0, worst = c->host_used;
-  auto rollback = [&]() {
-    for (u32 k : served) {
-      Claim& cl = *op.cl[k];
-      if (cl.dg_len) { c->dg_alloc.release(cl.dg_off, cl.dg_len); cl.dg_len = 0; }
+  std::vector<std::pair<u32, u32>> old_dg;
+  auto rollback = [&]() {                                  // a negative return changes no claim (rc.h)
+    for (size_t j = 0; j < served.size(); ++j) {
+      Claim& cl = *op.cl[served[j]];
+      c->dg_alloc.release(cl.dg_off, cl.dg_len);
+      cl.dg_off = old_dg[j].first; cl.dg_len = old_dg[j].second;
       cl.busy = false;
     }
   };
@@ -60,9 +62,9 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     if (cl.busy || (cl.state != RC_CS_MATERIALIZED && cl.state != RC_CS_RESIDENT_AGAIN)) { st[k] = RC_ST_BAD_STATE; continue; }
     if (full || worst + (u64)cl.nb * c->blk > c->cfg.host_store_bytes) { full = true; st[k] = RC_ST_NO_HOST_SPACE; continue; }
     worst += (u64)cl.nb * c->blk;
-    if (cl.dg_len) { c->dg_alloc.release(cl.dg_off, cl.dg_len); cl.dg_len = 0; }
     u64 dgo;
     if (T + cl.nb > c->cap_entries || !c->dg_alloc.alloc(cl.nb, dgo)) { rollback(); return RC_ERR_CAPACITY; }
+    old_dg.push_back({cl.dg_off, cl.dg_len});
     cl.dg_off = (u32)dgo; cl.dg_len = cl.nb;
     cl.hslots.clear(); cl.hkeys.clear();
     cl.busy = true;
@@ -75,6 +77,7 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     st[k] = -1;
   }
   if (served.empty()) return RC_OK;
+  for (auto& od : old_dg) if (od.second) c->dg_alloc.release(od.first, od.second);
   op.n = n; op.status = st; op.blocks = T; op.copy_bytes = 0; op.launches = 0;
   int rc;
   CK(cudaMemcpyAsync(c->d_desc[0], c->h_desc[0], (u64)n * sizeof(Desc), cudaMemcpyHostToDevice, c->gather));
@@ -115,7 +118,10 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
       u32 hs;
       if (it != c->store.end()) { it->second.second++; hs = it->second.first; }
       else {
-        if (!dedup_alloc_slot(c, hs, rc)) return rc ? rc : RC_ERR_CAPACITY;
+        if (!dedup_alloc_slot(c, hs, rc)) {               // cannot happen: space was granted by count at the top
+          if (!rc) { c->poisoned = true; c->cuda_err = "internal: dedup host-store accounting"; rc = RC_ERR_CUDA; }
+          return rc;                                       // sticky, like every error past the first enqueued copy
+        }
         c->store.emplace(key, std::make_pair(hs, 1u));
         c->host_used += c->blk;
         u8* h = c->h_store + (u64)hs * c->blk;

@@ -531,3 +531,49 @@ def test_predicate_on_random_non_monotone_fill():
     assert [int(e["aux"]) for e in ev if int(e["code"]) == 2] == [M for M, s in zip(want_M, sa) if s != 3 and M >= 448]
     assert V.validate(ev)[0]
     p.close()
+
+
+def test_call_level_errors_change_nothing():
+    """rc.h: a negative return emits no event and changes no claim: RC_ERR_CAPACITY of rc_accept in a later
+    run of a batch with a duplicate id, RC_ERR_CAPACITY of rc_offload after digests were recorded by an earlier cycle,
+    RC_ERR_BUSY of rc_measure_link while the pinned store holds claim bytes."""
+    import torch
+    wl = W.make_workload(0)
+    g = wl.geom
+    wave = W.plan_waves(wl, 1 << 30)[0]
+    cl = wl.claims
+    pool = W.pool_torch(g, torch.device("cuda:0"))
+    fill = torch.zeros(g.pool_blocks, dtype=torch.uint8, device="cuda:0")
+    fill[torch.from_numpy(wave.fill_ids.astype(np.int64)).cuda()] = torch.from_numpy(wave.fill_val).cuda()
+    torch.cuda.synchronize()
+    r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, pool, fill, 1 << 30,
+              staging_chunk_bytes=16 * g.blk_bytes, max_table_entries=100)
+    assert r.mark_used(wave.used_ids) == 0
+    tabs = [wave.bt_ids[wave.bt_off[k]:wave.bt_off[k + 1]] for k in range(4)]
+    ids = [c.claim_id for c in cl[:4]]
+
+    def batch(ks):
+        off = np.cumsum([0] + [len(tabs[k]) for k in ks]).astype(np.uint32)
+        return ([ids[k] for k in ks], [cl[k].P for k in ks], [448] * len(ks), off, np.concatenate([tabs[k] for k in ks]))
+    # claims 0, 0 (duplicate id: second run), 1, 2: 4 x ~30 table entries do not fit 100 -> nothing is accepted
+    rcode, st = r.accept(*batch([0, 0, 1, 2]), check=False)
+    assert rcode == rc.ERR_CAPACITY and len(r.outcomes()) == 0 and all(r.claim_info(c) is None for c in ids)
+    _, ref = r.pool_state()
+    assert not ref.any()
+    assert list(r.accept(*batch([0, 0, 1]))) == [0, 4, 0]                 # the same duplicate, now within capacity
+    assert not r.materialize(ids[:2]).any() and not r.offload(ids[:2]).any()
+    with pytest.raises(rc.RcError) as ei:
+        r.measure_link(1 << 20, 0, reps=1)                                 # would write over the claims' host copies
+    assert ei.value.code == rc.ERR_BUSY
+    hb = r.host_read(ids[0]).copy()
+    assert not r.restore(ids[:2]).any()
+    d0 = r.claim_digests(ids[0]).copy()
+    info0 = r.claim_info(ids[0])
+    # second cycle: the new digest extent is taken before the old one is given back; 2 x ~30 held + ~30 + ~30 new > 100
+    rcode, st = r.offload(ids[:2], check=False)
+    assert rcode == rc.ERR_CAPACITY
+    assert r.claim_info(ids[0]) == info0 and np.array_equal(r.claim_digests(ids[0]), d0)     # state and digests intact
+    assert r.stats()["host_used_bytes"] == 0 and len(r.outcomes()) == 10                    # 2 x (A, M, O, RR, R): no new event
+    assert list(r.offload(ids[:1])) == [0]                                                  # one claim still fits
+    assert np.array_equal(r.host_read(ids[0]), hb)
+    r.close()
