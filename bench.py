@@ -90,7 +90,7 @@ class Job:
         g = self.g = self.wl.geom
         dev = torch.device("cuda", torch.cuda.current_device())
         budget = int(0.5 * host_ram_bytes() / max(1, n_gpus))
-        self.host_store = min(g.pool_bytes, budget, host_cap or (1 << 62)) // g.blk_bytes * g.blk_bytes
+        self.host_store = min(g.pool_bytes, budget, host_cap or (64 << 30)) // g.blk_bytes * g.blk_bytes
         # pipelined: restore of wave k overlaps the offload of wave k+1 (full-duplex host link); waves of 1/wave_frac
         # of the pool (>= 2 so that two waves fit) keep the un-overlapped first offload and last restore short;
         # serial: one wave owns the pool and the host store
@@ -113,7 +113,7 @@ class Job:
         n_max = max(len(w.claim_idx) for w in self.waves)
         self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, self.pool, self.fill,
                        self.host_store, staging_chunk_bytes=min(chunk_bytes, self.host_store), staging_chunks=2,
-                       max_claims=max(1024, 2 * n_max), max_table_entries=max(4 * g.pool_blocks, 1 << 16),
+                       max_claims=max(1024, 4 * n_max), max_table_entries=max(4 * g.pool_blocks, 1 << 16),
                        max_events=max(1 << 16, 16 * n_max), mover=mover, grid_ctas=grid_ctas, dedup=dedup, direct_offload=direct)
         self.prep = []
         region = g.pool_blocks // wave_frac if pipelined else 0
@@ -138,6 +138,15 @@ class Job:
         self.fill_h2d = sum(p["fid_h"].numel() * 8 + p["fval_h"].numel() for p in self.prep)
         self.events = 0
 
+    def close(self):
+        import gc
+        self.r.close()
+        self.pool = self.fill = None
+        for p in self.prep:
+            p.clear()
+        gc.collect()
+        self.torch.cuda.empty_cache()
+
     def _admit(self, p, e2e):
         if e2e:     # fill[] arrives from pinned host memory inside the timed region
             self.fill.index_copy_(0, p["fid_h"].to(self.fill.device, non_blocking=True),
@@ -149,41 +158,54 @@ class Job:
         self.r.accept(p["ids"], p["P"], p["N"], p["bt_off"], p["bt_ids"])
         self.r.materialize(p["ids"])
 
-    def step(self, e2e):
+    def run(self, n_steps, e2e):
+        """n_steps passes over the workload's waves.  Pipelined schedule: the waves of all passes form one sequence;
+        wave j is restored while wave j+1 is offloaded (across pass boundaries too), and wave j+2 is admitted while
+        both are in flight.  Metadata steps run in call order, so every observable equals the synchronous calls."""
         r = self.r
         n_ev = 0
         if not self.pipelined:
-            for p in self.prep:
-                self._admit(p, e2e)
-                r.offload(p["ids"])
-                r.set_faults(p["faults"])
-                r.restore(p["ids"])
-                n_ev += len(r.outcomes(cap=8 * p["n"]))
-                r.release(p["ids"])
+            for _ in range(n_steps):
+                for p in self.prep:
+                    self._admit(p, e2e)
+                    r.offload(p["ids"])
+                    r.set_faults(p["faults"])
+                    r.restore(p["ids"])
+                    n_ev += len(r.outcomes(cap=8 * p["n"]))
+                    r.release(p["ids"])
         else:
-            # wave k is restored while wave k+1 is offloaded; metadata steps run in _begin order
-            self._admit(self.prep[0], e2e)
-            r.offload(self.prep[0]["ids"])
-            for k, p in enumerate(self.prep):
-                nxt = self.prep[k + 1] if k + 1 < len(self.prep) else None
-                if nxt is not None:
-                    self._admit(nxt, e2e)
+            seq = self.prep * n_steps
+            nmax = max(p["n"] for p in self.prep)
+            self._admit(seq[0], e2e)
+            r.offload(seq[0]["ids"])
+            if len(seq) > 1:
+                self._admit(seq[1], e2e)
+            for j, p in enumerate(seq):
+                nxt = seq[j + 1] if j + 1 < len(seq) else None
                 r.set_faults(p["faults"])
                 r.restore_begin(p["ids"])
                 if nxt is not None:
                     r.offload_begin(nxt["ids"])
+                if j + 2 < len(seq) and len(self.prep) > 2:
+                    # wave j+2 reuses the pool region wave j left at its offload; its ids were released at j+2-len(prep)
+                    self._admit(seq[j + 2], e2e)
+                if nxt is not None:
                     r.wait(0)
                 r.wait(1)
-                n_ev += len(r.outcomes(cap=16 * max(p["n"], nxt["n"] if nxt else 0)))
+                n_ev += len(r.outcomes(cap=32 * nmax))
                 r.release(p["ids"])
-        self.events = n_ev
+                if j + 2 < len(seq) and len(self.prep) <= 2:
+                    self._admit(seq[j + 2], e2e)
+        self.events = n_ev // max(1, n_steps)
         return n_ev
+
+    def step(self, e2e):
+        return self.run(1, e2e)
 
 
 def time_steps(job, steps, warmup, e2e, dist):
     torch = job.torch
-    for _ in range(warmup):
-        job.step(e2e)
+    job.run(warmup, e2e)
     job.r.stats_reset()
     if dist is not None:
         dist.barrier()
@@ -191,8 +213,7 @@ def time_steps(job, steps, warmup, e2e, dist):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = time.perf_counter()
     e0.record()
-    for _ in range(steps):
-        job.step(e2e)
+    job.run(steps, e2e)
     e1.record()
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
@@ -205,11 +226,18 @@ def time_steps(job, steps, warmup, e2e, dist):
 
 class OracleJob:
     """The oracle (oracle/, plain single-threaded C++) on a bounded sample of the same workload:
-    the first `n_claims` claims of the config on a reduced pool, same recipe, same calls."""
+    the first `n_claims` claims of the config on a reduced pool, same recipe, same calls.
+    shard = (p, P): this process takes claims p, p+P, ... of a P times larger sample (claims are independent)."""
 
-    def __init__(self, index, n_claims, pool_blocks):
+    def __init__(self, index, n_claims, pool_blocks, shard=None):
         from oracle import rco
-        self.wl = W.make_workload(index, n_claims=n_claims, pool_blocks=pool_blocks)
+        if shard is None:
+            self.wl = W.make_workload(index, n_claims=n_claims, pool_blocks=pool_blocks)
+        else:
+            self.wl = W.make_workload(index, n_claims=n_claims * shard[1], pool_blocks=pool_blocks)
+            self.wl.claims = self.wl.claims[shard[0]::shard[1]]
+            for c in self.wl.claims:                       # prefix groups do not survive sharding: private blocks
+                c.group, c.shared = -1, 0
         g = self.g = self.wl.geom
         self.pool = W.pool_host(g)
         self.fill = np.zeros(g.pool_blocks, np.uint8)
@@ -245,6 +273,36 @@ def oracle_sample_shape(index):
     return {0: (8, 256), 1: (16, 640), 2: (4, 800), 3: (256, 2560), 4: (16, 640)}[index]
 
 
+def _oracle_shard(args):
+    index, p, P = args
+    n_claims, pool_blocks = oracle_sample_shape(index)
+    job = OracleJob(index, n_claims, pool_blocks, shard=(p, P))
+    t0 = time.perf_counter()
+    moved = job.step()
+    return moved, time.perf_counter() - t0, sum(len(w.claim_idx) for w in job.waves)
+
+
+def run_oracle_all_cores(index):
+    """P = nproc independent oracle processes, claims sharded round-robin; aggregate bytes over the
+    slowest process's time.  The oracle itself stays single-threaded."""
+    import multiprocessing as mp
+    P = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    n_claims, pool_blocks = oracle_sample_shape(index)
+    need = P * (W.GEOMS[index].blk_bytes * pool_blocks) * 3                    # pool + host copies per process
+    while P > 1 and need > 0.5 * host_ram_bytes():
+        P //= 2
+        need //= 2
+    t0 = time.perf_counter()
+    with mp.get_context("spawn").Pool(P) as pool:
+        res = pool.map(_oracle_shard, [(index, p, P) for p in range(P)])
+    wall = time.perf_counter() - t0
+    moved, slowest, claims = sum(r[0] for r in res), max(r[1] for r in res), sum(r[2] for r in res)
+    return {"value": moved / slowest / 1e9, "unit": UNIT, "cores": P, "kind": "oracle",
+            "sample": "%d processes, each %d claims of configs[%d] (round-robin shard of the first %d) on a %d-block pool" % (
+                P, n_claims, index, n_claims * P, pool_blocks),
+            "claims_per_s": claims / slowest, "seconds": slowest, "wall_seconds_with_setup": wall}
+
+
 def run_oracle(index, steps, warmup):
     n_claims, pool_blocks = oracle_sample_shape(index)
     job = OracleJob(index, n_claims, pool_blocks)
@@ -270,11 +328,6 @@ def reduce_scalar(dist, x, op, device="cuda"):
     return float(t.item())
 
 
-def shard_claims(items, rank, world):
-    """Claim sharding for one shared workload: claims are independent, rank r takes items r, r+world, ..."""
-    return list(items[rank::world])
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -291,6 +344,8 @@ def main():
     ap.add_argument("--direct-offload", action="store_true", help="NEXT-4 experiment: gather straight into the mapped pinned store")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--per-config-budget-s", type=float, default=330.0,
+                    help="wall-clock budget for the per_config block (the other four configs, 3 steps each); 0 = off")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per gather launch (profiles/), if known")
     a = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -326,13 +381,20 @@ def main():
     job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac), dedup=a.dedup, direct=a.direct_offload)
     g = job.g
     link = {}
-    if world == 1:
+
+    def measure_ceilings():
+        # pinned-copy ceilings of this process (the store holds no claim bytes between steps); the best of the
+        # measurements taken before and after the timed region counts: the first copies on a fresh box run slow
         for name, d in (("d2h", 0), ("h2d", 1), ("both", 2)):
-            link[name] = job.r.measure_link(1 << 30, d, reps=5)
+            link[name] = max(link.get(name, 0.0), job.r.measure_link(1 << 30, d, reps=6))
+    if world == 1:
+        measure_ceilings()
 
     sampler = ClockSampler(local) if rank == 0 else None
     ms, wall_ms, st = time_steps(job, a.steps, a.warmup, False, dist)
     clocks = sampler.stop() if sampler else None
+    if world == 1:
+        measure_ceilings()
     payload = st["bytes_d2h"] + st["bytes_h2d"]
     link_bytes = payload
     if a.dedup:                # claim-logical bytes moved (what the claims hold), not the smaller number that crossed the link
@@ -366,16 +428,19 @@ def main():
                 "traffic": a.traffic, "peak_source": peak_src, "launches": launches,
                 "avg_launch_ms": ms_k / launches, "algorithmic_bytes_per_launch": per_launch}
 
+    traffic_source = "--traffic" if a.traffic is not None else None
     if a.traffic is None:      # dram__bytes_read+write of the gather kernel from the committed ncu capture, scaled per block
         try:
-            with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+            with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as f:
                 tj = json.load(f)
             a.traffic = (tj["dram_bytes_read"] + tj["dram_bytes_write"]) / tj["launch_blocks"] * st["gather_blocks"] / max(1, st["gather_launches"])
+            traffic_source = "profiles/r02_traffic.json: " + tj["source"] + "; scaled by blocks per launch (not measured in this run: ncu is needed)"
         except Exception:
             a.traffic = None
     roofline = roof(st["ms_gather"], st["gather_launches"], st["gather_blocks"])
     if roofline:
         roofline["kernel"] = "k_move_hash%s<GATHER> (K2 gather+checksum)" % ("_tma" if mover != rc.MOVER_LDG else "")
+        roofline["traffic_source"] = traffic_source
     roof_sc = roof(st["ms_scatter"], st["scatter_launches"], st["scatter_blocks"])
     if roof_sc:
         roof_sc["kernel"] = "k_move_hash%s<SCATTER> (K4 scatter+checksum)" % ("_tma" if mover != rc.MOVER_LDG else "")
@@ -401,7 +466,7 @@ def main():
         h2d = st["bytes_h2d"] / (st["ms_h2d"] * 1e6) if st["ms_h2d"] > 0 else None
         links = {"ceiling_gbs": link, "d2h_gbs": d2h, "h2d_gbs": h2d,
                  "d2h_frac": d2h / link["d2h"] if d2h else None, "h2d_frac": h2d / link["h2d"] if h2d else None,
-                 "ceiling_how": "best of 5 cudaMemcpyAsync of 1 GiB, pinned store <-> staging, same process; "
+                 "ceiling_how": "best of 2 x 6 cudaMemcpyAsync of 1 GiB (before and after the timed region), pinned store <-> staging, same process; "
                                 "'both' = D2H and H2D at once (sum); fractions are per direction over that "
                                 "direction's copy-stream busy time against its one-way ceiling"}
     line = {"metric": METRIC, "value": payload_all / (ms_max * 1e6), "unit": UNIT, "n_gpus": world, "steps": a.steps,
@@ -409,7 +474,7 @@ def main():
             "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": wname, "claims": len(job.wl.claims), "pool_blocks": g.pool_blocks, "blk_bytes": blk,
                        "waves": len(job.waves), "host_store_bytes": job.host_store, "staging_chunk_bytes": a.chunk_mib << 20,
-                       "mover": a.mover, "schedule": "serial" if a.serial else "restore(k) overlapped with offload(k+1)", "l2": "inputs larger than L2 (pool %d GiB, staging chunks %d MiB, L2 126 MB)" % (g.pool_bytes >> 30, a.chunk_mib),
+                       "mover": a.mover, "schedule": "serial" if a.serial else "restore(k) overlapped with offload(k+1), wave k+2 admitted meanwhile; waves of consecutive steps form one sequence", "l2": "inputs larger than L2 (pool %d GiB, staging chunks %d MiB, L2 126 MB)" % (g.pool_bytes >> 30, a.chunk_mib),
                        "parallelism": "claims independent: one replica of the workload per GPU, no collective"},
             "claims_per_s": claims_all / (ms_max / 1e3), "payload_bytes_per_step": payload_all / a.steps,
             "wall_ms_per_step": wall_ms / a.steps, "clocks": clocks, "gpu_launches": int(launches_all),
@@ -440,6 +505,49 @@ def main():
     if world == 1 and not a.no_cpu_baseline:
         line["cpu_baseline"] = {k: v for k, v in run_oracle(a.config, 1, 0).items() if k in
                                 ("value", "unit", "cores", "kind", "sample", "claims_per_s", "seconds")}
+        line["cpu_baseline"]["all_cores"] = run_oracle_all_cores(a.config)
+    if world == 1 and a.per_config_budget_s > 0:
+        # the other BASELINE.json configs at full size, same schedule, >= 3 steps each, device-timed like `value`;
+        # a config whose estimated cost does not fit the remaining budget is skipped and says so
+        job.close()
+        t_start = time.perf_counter()
+        per = {"configs[%d]" % a.config: {"value": line["value"], "claims_per_s": line["claims_per_s"], "steps": a.steps,
+                                          "ms_per_step": line["ms_per_step"], "gather_frac": roofline and roofline["frac"],
+                                          "scatter_frac": roof_sc and roof_sc["frac"],
+                                          "value_over_duplex_ceiling": links and links.get("value_over_duplex_ceiling")}}
+        for idx in (3, 0, 4, 2):
+            if idx == a.config:
+                continue
+            wl_i = W.make_workload(idx)
+            est_bytes = 2.0 * sum(((c.M + wl_i.geom.block_size - 1) // wl_i.geom.block_size) * wl_i.geom.blk_bytes
+                                  for c in wl_i.claims if c.M >= c.N)
+            est = 4 * est_bytes / 85e9 + 15 + wl_i.geom.pool_bytes / 4e9       # 1 warm-up + 3 steps, setup, pool generation
+            left = a.per_config_budget_s - (time.perf_counter() - t_start)
+            key = "configs[%d] %s" % (idx, W.GEOMS[idx].name)
+            if est > left:
+                per[key] = {"skipped": "estimated %.0f s, %.0f s of the budget left (run: python bench.py --config %d)" % (est, left, idx)}
+                continue
+            try:
+                j2 = Job(idx, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac))
+                ms_i, _, st_i = time_steps(j2, 3, 1, False, None)
+                pay = st_i["bytes_d2h"] + st_i["bytes_h2d"]
+                blk_i = j2.g.blk_bytes
+
+                def fr(ms_k, launches, blocks):
+                    return (2.0 * blk_i * blocks / (ms_k * 1e6)) / peak if launches and ms_k > 0 else None
+                per[key] = {"value": pay / (ms_i * 1e6), "claims_per_s": sum(p["n"] for p in j2.prep) * 3 / (ms_i / 1e3),
+                            "steps": 3, "warmup": 1, "ms_per_step": ms_i / 3, "waves": len(j2.waves),
+                            "payload_bytes_per_step": pay / 3, "pool_blocks": j2.g.pool_blocks,
+                            "gather_frac": fr(st_i["ms_gather"], st_i["gather_launches"], st_i["gather_blocks"]),
+                            "scatter_frac": fr(st_i["ms_scatter"], st_i["scatter_launches"], st_i["scatter_blocks"]),
+                            "d2h_gbs": st_i["bytes_d2h"] / (st_i["ms_d2h"] * 1e6) if st_i["ms_d2h"] > 0 else None,
+                            "h2d_gbs": st_i["bytes_h2d"] / (st_i["ms_h2d"] * 1e6) if st_i["ms_h2d"] > 0 else None,
+                            "value_over_duplex_ceiling": pay / (ms_i * 1e6) / link["both"] if link else None,
+                            "gpu_launches": int(st_i["kernel_launches"])}
+                j2.close()
+            except Exception as e:                                             # a side measurement must not lose the main line
+                per[key] = {"error": repr(e)[:200]}
+        line["per_config"] = per
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
