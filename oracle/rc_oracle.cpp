@@ -147,6 +147,9 @@ struct Ctx {
   std::vector<Event> events; u64 drained = 0;
   u64 generic_failures = 0;
   u64 accept_seq = 0;
+  // NEXT-4: TP mode and the restore that waits between its two phases for the merged verdict
+  u32 tp_ranks = 0;
+  bool tp_pending = false; std::vector<u64> tp_ids; std::vector<void*> tp_served;
   // NEXT-2: content-addressed host store keyed by block digest, so blocks shared between claims
   // are held (and cross the link) once.  DESIGN.md "Dedup".
   bool dedup = false;
@@ -254,7 +257,7 @@ static void do_offload_one(Ctx* c, u64 id, Claim& cl) {
   }
   drop_refs(c, cl);
   cl.state = CS_OFFLOADED;
-  c->emit(id, EV_OFFLOADED, cl.nb, cl.chain);
+  c->emit(id, EV_OFFLOADED, cl.nb, c->tp_ranks > 1 ? 0 : cl.chain);
 }
 
 static void do_offload(Ctx* c, u32 n, const u64* ids, int32_t* st) {
@@ -286,9 +289,16 @@ static void do_offload(Ctx* c, u32 n, const u64* ids, int32_t* st) {
 // batch is ONE reuse request naming several claims; its refusal is emitted once, after the per-claim records, as
 // one REFUSED record per failed claim (claim_id = the blocking claim, aux = REQ_FLAG | size of the failed subset,
 // arg = request id) -- blocking_claim_ids is exactly the failed subset ("smeared" ids fail closed).
-static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_id = 0) {
+// The call is written in two phases so that a TP-sharded deployment (NEXT-4; below) can put the
+// cross-rank verdict merge between them; rco_restore runs them back to back with the local verdicts.
+struct Verdict { u32 flags, bad; };                     // flags: 1 = served, 2 = locally ok; bad = first bad block / 0xFFFFFFFF
+enum { V_SERVED = 1, V_OK = 2 };
+
+// phase 1: steps 1-3 and, of step 4, everything but the events: fault decision, write, re-digest, LOCAL verdict
+static void restore_verify(Ctx* c, u32 n, const u64* ids, int32_t* st, std::vector<Claim*>& served, std::vector<Verdict>& v) {
   u32 G = 2 * c->L;
-  std::vector<Claim*> served(n, nullptr);
+  served.assign(n, nullptr);
+  v.assign(n, Verdict{0, 0xFFFFFFFFu});
   u64 nfree = 0;
   for (u32 b = 0; b < c->NB; ++b) nfree += !c->used[b];
   u64 need = 0; bool full = false;
@@ -312,14 +322,10 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_i
       c->used[cursor] = 1; c->ref[cursor] = 1; cl.bt.push_back(cursor);
     }
   }
-  bool any_served = false;
   std::set<Key> call_keys;
-  std::vector<u64> blocking;
   for (u32 k = 0; k < n; ++k) {
     if (!served[k]) continue;
-    any_served = true;
     Claim& cl = *served[k]; u64 id = ids[k];
-    c->emit(id, EV_RESTORE_REQUIRED, cl.M, 0);          // lookup "hit" (P:L364)
     int fi = -1;
     for (size_t f = 0; f < c->faults.size(); ++f) if (c->faults[f].claim_id == id) { fi = (int)f; break; }
     Fault flt{0, 0, 0};
@@ -330,7 +336,7 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_i
     } else {
       std::vector<u8> staged = host_bytes_of(c, cl);    // host copy itself stays intact
       if (c->dedup && flt.kind != FK_BITFLIP) {           // one transfer per distinct block of the call; a corrupted
-        for (const Key& k : cl.hkeys) if (call_keys.insert(k).second) c->link_h2d += c->blk;   // copy is private to its claim
+        for (const Key& kk : cl.hkeys) if (call_keys.insert(kk).second) c->link_h2d += c->blk;   // copy is private to its claim
       } else c->link_h2d += staged.size();
       if (flt.kind == FK_BITFLIP && !staged.empty()) staged[flt.param % staged.size()] ^= 0x01;
       std::vector<u64> d2(cl.nb), e2(cl.nb);
@@ -346,13 +352,33 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_i
       for (u32 i = 0; i < cl.nb && !found; ++i) if (d2[i] != cl.d[i] || e2[i] != cl.e[i]) { bad = i; found = true; }
       ok = !found && chain_of(id, d2.data(), cl.nb) == cl.chain;
     }
+    v[k].flags = V_SERVED | (ok ? V_OK : 0);
+    v[k].bad = bad;
+  }
+}
+
+// phase 2: per served claim, batch order: RESTORE_REQUIRED, then the outcome of the (merged) verdict; blocks of failed
+// claims are freed.  request_id == 0: every claim is its own reuse request (blocking_claim_ids=[C]).  request_id
+// != 0 (NEXT-3): the batch is ONE reuse request naming several claims; its refusal is emitted once, after the per-claim
+// records, as one REFUSED record per failed claim (claim_id = the blocking claim, aux = REQ_FLAG | size of the failed
+// subset, arg = request id) -- blocking_claim_ids is exactly the failed subset ("smeared" ids fail closed,
+// P:L384).
+static void restore_commit(Ctx* c, u32 n, const u64* ids, int32_t* st, const std::vector<Claim*>& served,
+                           const std::vector<Verdict>& v, u64 request_id) {
+  bool any_served = false;
+  std::vector<u64> blocking;
+  for (u32 k = 0; k < n; ++k) {
+    if (!served[k]) continue;
+    any_served = true;
+    Claim& cl = *served[k]; u64 id = ids[k];
+    c->emit(id, EV_RESTORE_REQUIRED, cl.M, 0);          // lookup "hit" (P:L364)
     drop_host(c, cl);
-    if (ok) {
+    if (v[k].flags & V_OK) {
       cl.state = CS_RESIDENT_AGAIN;
-      c->emit(id, EV_RESTORED, cl.nb, cl.chain);
+      c->emit(id, EV_RESTORED, cl.nb, c->tp_ranks > 1 ? 0 : cl.chain);
       st[k] = ST_OK;
     } else {
-      c->emit(id, EV_LOAD_FAILED, bad, 0);
+      c->emit(id, EV_LOAD_FAILED, v[k].bad, 0);
       c->emit(id, EV_RESTORATION_FAILED, 0, 0);
       if (cl.policy == POL_DEMOTE) c->emit(id, EV_DEMOTED, 0, 0);        // ordered responsibility boundary
       else if (cl.policy == POL_EXPIRE) c->emit(id, EV_EXPIRED, 0, 0);
@@ -370,6 +396,36 @@ static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_i
       if (c->faults[f].claim_id == 0) { c->generic_failures++; c->faults.erase(c->faults.begin() + f); }
       else ++f;
   }
+}
+
+static void do_restore(Ctx* c, u32 n, const u64* ids, int32_t* st, u64 request_id = 0) {
+  std::vector<Claim*> served;
+  std::vector<Verdict> v;
+  restore_verify(c, n, ids, st, served, v);
+  restore_commit(c, n, ids, st, served, v, request_id);
+}
+
+// ---- NEXT-4: TP-sharded KV, one common verdict (DESIGN.md 8 / R24) ----------------------------------
+// The pool is split by kv_head over G ranks; every rank makes the same calls on its own shard, with its own digests and
+// chain.  The verdict must be common (attribution must survive; it must not smear): between phase 1 and
+// phase 2 the ranks exchange their local verdicts, and every rank applies the SAME merged verdict per claim:
+//   served  -- must agree on every rank (same calls, same allocator state); a disagreement is a call-level error;
+//   ok      = AND over ranks;      bad = min over the ranks that failed (a transfer error, 0xFFFFFFFF, loses to a block index).
+// In TP mode OFFLOADED / RESTORED carry arg = 0 (chains are rank-local facts; rco_claim_info still returns them), so the
+// emitted streams are byte-identical on every rank.
+static int tp_merge(u32 n, u32 G, const Verdict* gathered /*[G][n]*/, std::vector<Verdict>& out) {
+  out.assign(n, Verdict{0, 0xFFFFFFFFu});
+  for (u32 k = 0; k < n; ++k) {
+    u32 served = gathered[k].flags & V_SERVED, ok = V_OK, bad = 0xFFFFFFFFu;
+    for (u32 r = 0; r < G; ++r) {
+      const Verdict& x = gathered[(u64)r * n + k];
+      if ((x.flags & V_SERVED) != served) return E_INVALID;     // the ranks did not make the same call
+      if (!(x.flags & V_OK)) { ok = 0; if (x.bad < bad) bad = x.bad; }
+    }
+    out[k].flags = served | (served ? ok : 0);
+    out[k].bad = ok ? 0xFFFFFFFFu : bad;
+  }
+  return E_OK;
 }
 
 // ---- NEXT-3: allocator-side protection (reading R23) ------------------------------------------------
@@ -490,6 +546,32 @@ int rco_set_policy(void* h, u32 n, const u64* id, const u32* policy) {   // what
   Ctx* c = (Ctx*)h;
   for (u32 k = 0; k < n; ++k) if (!c->claims.count(id[k]) || policy[k] > POL_EXPIRE) return E_INVALID;
   for (u32 k = 0; k < n; ++k) c->claims[id[k]].policy = policy[k];
+  return E_OK;
+}
+int rco_set_tp(void* h, u32 ranks) { ((Ctx*)h)->tp_ranks = ranks; return E_OK; }
+int rco_tp_restore_verify(void* h, u32 n, const u64* id, int32_t* st, Verdict* local) {
+  Ctx* c = (Ctx*)h;
+  if (c->tp_pending || c->dedup) return E_INVALID;
+  std::vector<Claim*> served; std::vector<Verdict> v;
+  restore_verify(c, n, id, st, served, v);
+  for (u32 k = 0; k < n; ++k) { local[k] = v[k]; if (served[k]) st[k] = -1; }   // pending: decided by the commit
+  c->tp_ids.assign(id, id + n);
+  c->tp_served.assign(served.begin(), served.end());
+  c->tp_pending = true;
+  return E_OK;
+}
+int rco_tp_restore_commit(void* h, u32 n, u32 G, const Verdict* gathered, int32_t* st) {
+  Ctx* c = (Ctx*)h;
+  if (!c->tp_pending || n != c->tp_ids.size() || G == 0) return E_INVALID;
+  std::vector<Verdict> merged;
+  if (tp_merge(n, G, gathered, merged) != E_OK) return E_INVALID;
+  std::vector<Claim*> served(n);
+  for (u32 k = 0; k < n; ++k) {
+    served[k] = (Claim*)c->tp_served[k];
+    if (((merged[k].flags & V_SERVED) != 0) != (served[k] != nullptr)) return E_INVALID;
+  }
+  restore_commit(c, n, c->tp_ids.data(), st, served, merged, 0);
+  c->tp_pending = false;
   return E_OK;
 }
 int rco_protect(void* h, u32 n, const u64* id, const u32* on) {          // hard_protected on / off; any live claim

@@ -14,6 +14,7 @@ _SO = os.path.join(_HERE, "librc_oracle.so")
 
 EVENT_DTYPE = np.dtype([("seq", "<u8"), ("claim_id", "<u8"), ("code", "<u4"), ("aux", "<u4"), ("arg", "<u8")])
 FAULT_DTYPE = np.dtype([("claim_id", "<u8"), ("kind", "<u4"), ("param", "<u4")])
+TP_VERDICT_DTYPE = np.dtype([("flags", "<u4"), ("bad", "<u4")])      # flags: 1 served, 2 locally ok
 
 EV_NAMES = {1: "ACCEPTED", 2: "MATERIALIZED", 3: "OFFLOADED", 4: "RESTORE_REQUIRED", 5: "LOAD_FAILED",
             6: "RESTORED", 7: "RESTORATION_FAILED", 8: "ACTIVE_REQUEST_REFUSED", 9: "DEMOTED", 10: "EXPIRED",
@@ -170,6 +171,27 @@ class Oracle:
 
     def release(self, ids):
         return self._batch(self.L.rco_release, ids)
+
+    def set_tp(self, ranks):
+        return self.L.rco_set_tp(self.h, ranks)
+
+    def tp_restore_verify(self, ids):
+        """Phase 1 of a TP-sharded restore: returns (statuses, local verdict records)."""
+        ids = _u64(ids)
+        st = np.zeros(ids.size, np.int32)
+        v = np.zeros(ids.size, TP_VERDICT_DTYPE)
+        rc = self.L.rco_tp_restore_verify(self.h, ids.size, _p(ids), _p(st), _p(v))
+        if rc != 0:
+            raise ValueError("rco_tp_restore_verify: %d" % rc)
+        return st, v
+
+    def tp_restore_commit(self, gathered, st):
+        """Phase 2: gathered = verdict records of all ranks, shape [G, n]; completes the statuses of phase 1 in place."""
+        g = np.ascontiguousarray(gathered, dtype=TP_VERDICT_DTYPE)
+        rc = self.L.rco_tp_restore_commit(self.h, g.shape[1], g.shape[0], _p(g), _p(st))
+        if rc != 0:
+            raise ValueError("rco_tp_restore_commit: %d" % rc)
+        return st
 
     def protect(self, ids, on):
         ids, on = _u64(ids), _u32(on)
