@@ -376,7 +376,8 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    from paper_2606_01387_b200 import rc
+    from paper_2606_01387_b200 import rc, tp
+    numa = tp.bind_to_gpu_numa_node(local)      # before rc_create: the pinned store is first touched on the GPU's node
     mover = {"auto": rc.MOVER_AUTO, "ldg": rc.MOVER_LDG, "tma": rc.MOVER_TMA}[a.mover]
     job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac), dedup=a.dedup, direct=a.direct_offload)
     g = job.g
@@ -475,7 +476,8 @@ def main():
             "config": {"workload": wname, "claims": len(job.wl.claims), "pool_blocks": g.pool_blocks, "blk_bytes": blk,
                        "waves": len(job.waves), "host_store_bytes": job.host_store, "staging_chunk_bytes": a.chunk_mib << 20,
                        "mover": a.mover, "schedule": "serial" if a.serial else "restore(k) overlapped with offload(k+1), wave k+2 admitted meanwhile; waves of consecutive steps form one sequence", "l2": "inputs larger than L2 (pool %d GiB, staging chunks %d MiB, L2 126 MB)" % (g.pool_bytes >> 30, a.chunk_mib),
-                       "parallelism": "claims independent: one replica of the workload per GPU, no collective"},
+                       "parallelism": "claims independent: one replica of the workload per GPU, no collective",
+                       "numa_node": numa},
             "claims_per_s": claims_all / (ms_max / 1e3), "payload_bytes_per_step": payload_all / a.steps,
             "wall_ms_per_step": wall_ms / a.steps, "clocks": clocks, "gpu_launches": int(launches_all),
             "dedup": ({"link_bytes_per_step": link_bytes / a.steps, "logical_bytes_per_step": payload / a.steps,

@@ -101,6 +101,10 @@ typedef struct rc_config {
                                between claims is held and crosses the link once       */
   uint32_t direct_offload;  /* NEXT-4 (experimental): 1 = the gather kernel stores straight into the mapped pinned
                                store (no staging, no copy engine); ignored with dedup                          */
+  uint32_t tp_ranks, tp_rank; /* NEXT-4: TP-sharded KV: this context holds the kv_heads of rank
+                               tp_rank of tp_ranks (<= 16); kv_heads above is the PER-RANK head count.  0 / 1 = off.
+                               With tp_ranks > 1 OFFLOADED / RESTORED carry arg = 0 (chains are rank-local) so that
+                               every rank emits the byte-identical stream; not combinable with dedup.          */
 } rc_config;
 
 typedef struct rc_claim_info_t {
@@ -180,6 +184,32 @@ int rc_wait(rc_ctx* ctx, int which);
 int rc_set_policy(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, const uint32_t* policy);
 int rc_restore_request(rc_ctx* ctx, uint64_t request_id, uint32_t n, const uint64_t* claim_id, int32_t* status);
 int rc_restore_request_begin(rc_ctx* ctx, uint64_t request_id, uint32_t n, const uint64_t* claim_id, int32_t* status);
+
+/* NEXT-4 (DESIGN.md 8 / R24): TP-sharded KV.  The pool is split by kv_head over tp_ranks ranks;
+ * every rank makes the same calls with the same arguments on its shard (own digests, own chain, same block ids).  The
+ * restoration verdict must be common, so a restore runs in two calls with the exchange in between:
+ *   rc_tp_restore_verify  a5-a7 on this rank: plan, allocation, H2D, scatter, digests, LOCAL verdict.  Nothing is
+ *       emitted and no block is released.  local[k] = { flags: RC_TP_SERVED | RC_TP_OK, bad }; status[k] is final for
+ *       entries that were not served (as rc_restore) and -1 for served ones.  The records are also stored into every
+ *       open peer mailbox (below).
+ *   rc_tp_restore_commit  a8 on the merged verdict: ok = AND over ranks, bad = min over the failing ranks (k_tp_merge);
+ *       fill / release of the new blocks, RESTORE_REQUIRED and the outcome records, statuses.  gathered = HOST
+ *       [ranks][n] records of all ranks in rank order (e.g. one all-gather), or NULL to read this rank's mailbox: then
+ *       every rank must have completed its verify (one barrier); RC_ERR_BUSY if a peer has not published yet -- the
+ *       library never waits inside a kernel for another rank.  RC_ERR_INVALID if the ranks disagree on which entries
+ *       were served (they did not make the same call); nothing is applied then and the commit may be repeated.
+ * Between the two calls rc_wait(1), rc_restore*, rc_make_room return RC_ERR_BUSY / RC_ERR_INVALID.
+ * Mailboxes (NVLink / NVSwitch path): rc_tp_mailbox returns this rank's mailbox (DEVICE); a peer rank is attached with
+ * rc_tp_set_peer (a device pointer valid in this process) or rc_tp_ipc_handle / rc_tp_open_peer (64-byte CUDA IPC
+ * handle, for one process per GPU). */
+enum { RC_TP_SERVED = 1, RC_TP_OK = 2 };
+typedef struct rc_tp_verdict { uint32_t flags, bad; } rc_tp_verdict;
+int rc_tp_restore_verify(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status, rc_tp_verdict* local);
+int rc_tp_restore_commit(rc_ctx* ctx, uint32_t n, uint32_t ranks, const rc_tp_verdict* gathered, int32_t* status);
+int rc_tp_mailbox(rc_ctx* ctx, void** mailbox_dev, uint64_t* bytes);
+int rc_tp_set_peer(rc_ctx* ctx, uint32_t rank, void* mailbox_dev /* DEVICE */);
+int rc_tp_ipc_handle(rc_ctx* ctx, void* handle64 /* HOST, 64 bytes out */);
+int rc_tp_open_peer(rc_ctx* ctx, uint32_t rank, const void* handle64 /* HOST, 64 bytes */);
 
 /* NEXT-3, allocator-side protection (P:L85 victim_exclusion_before_violation, explicit_conflict_action,
  * blocking_claim_ids, claim_demoted_before_loss; P:L103 hard_protected; P:L270 allocator_hook).

@@ -119,6 +119,10 @@ struct rc_ctx {
   Event* d_ring = nullptr; u64* d_evcount = nullptr; u32* d_bitmaps = nullptr; u32* d_up = nullptr;
   u32* d_counters = nullptr; u32* d_alloc = nullptr; u64* d_flip = nullptr;
   u32 *d_posmax = nullptr, *d_gain = nullptr; u8* d_protmap = nullptr; u64 accept_seq = 0;   // NEXT-3 allocator-side protection
+  // NEXT-4: TP-sharded KV.  Mailbox = [TP_MAX_RANKS epoch flags][G x desc_cap verdict records], peer-writable.
+  u32 tp_ranks = 0, tp_rank = 0, tp_n = 0; bool tp_split = false, tp_pending = false; u64 tp_epoch = 0;
+  u8* d_mailbox = nullptr; u64 mailbox_bytes = 0; TpVerdict *d_verd = nullptr, *d_gath = nullptr, *h_verd = nullptr;
+  u8* peer_mb[TP_MAX_RANKS] = {}; bool peer_ipc[TP_MAX_RANKS] = {};
   Desc* d_desc[3] = {}; Res* d_res[3] = {}; u32* d_off[3] = {};
   Desc* h_desc[3] = {}; Res* h_res[3] = {};
   u32* h_up = nullptr; u64* h_flip = nullptr; u32* h_counters = nullptr;
@@ -221,6 +225,8 @@ extern "C" int rc_destroy(rc_ctx* c) {
   auto FH = [](void* p) { if (p) cudaFreeHost(p); };
   F(c->d_used); F(c->d_ref); F(c->d_bt); F(c->d_dg); F(c->d_dg2); F(c->d_ring); F(c->d_evcount); F(c->d_bitmaps); F(c->d_up);
   F(c->d_counters); F(c->d_alloc); F(c->d_flip); F(c->d_posmax); F(c->d_gain); F(c->d_protmap);
+  for (u32 r = 0; r < TP_MAX_RANKS; ++r) if (c->peer_ipc[r] && c->peer_mb[r]) cudaIpcCloseMemHandle(c->peer_mb[r]);
+  F(c->d_mailbox); F(c->d_verd); F(c->d_gath); FH(c->h_verd);
   for (int i = 0; i < 3; ++i) { F(c->d_desc[i]); F(c->d_res[i]); F(c->d_off[i]); FH(c->h_desc[i]); FH(c->h_res[i]); }
   FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
   F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
@@ -253,6 +259,8 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   if (!cfg->max_claims || !cfg->max_table_entries || !cfg->max_events || cfg->staging_chunks < 2) return RC_ERR_INVALID;
   const u64 blk = 2ull * cfg->layers * page;
   if (cfg->staging_chunk_bytes < blk || cfg->mover > RC_MOVER_TMA) return RC_ERR_INVALID;
+  if (cfg->tp_ranks > TP_MAX_RANKS || (cfg->tp_ranks ? cfg->tp_rank >= cfg->tp_ranks : cfg->tp_rank != 0)) return RC_ERR_INVALID;
+  if (cfg->tp_ranks > 1 && cfg->dedup) return RC_ERR_INVALID;        // the content-addressed store is not sharded
   if ((cfg->staging_chunk_bytes / blk) * (2ull * cfg->layers) > 0x7FFFFFFFull) return RC_ERR_INVALID;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return RC_ERR_CUDA;   // no device, no library
@@ -301,6 +309,14 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   CC(cudaMalloc(&c->d_posmax, NB * 4), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_gain, dc * 4), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_protmap, NB), RC_ERR_NOMEM);
+  c->tp_ranks = cfg->tp_ranks ? cfg->tp_ranks : 1; c->tp_rank = cfg->tp_rank;
+  c->mailbox_bytes = TP_MAX_RANKS * 8 + (u64)c->tp_ranks * dc * sizeof(TpVerdict);
+  CC(cudaMalloc(&c->d_mailbox, c->mailbox_bytes), RC_ERR_NOMEM);
+  CC(cudaMemset(c->d_mailbox, 0, c->mailbox_bytes), RC_ERR_CUDA);
+  CC(cudaMalloc(&c->d_verd, dc * sizeof(TpVerdict)), RC_ERR_NOMEM);
+  CC(cudaMalloc(&c->d_gath, (u64)c->tp_ranks * dc * sizeof(TpVerdict)), RC_ERR_NOMEM);
+  CC(cudaHostAlloc(&c->h_verd, (u64)c->tp_ranks * dc * sizeof(TpVerdict), cudaHostAllocDefault), RC_ERR_NOMEM);
+  c->peer_mb[c->tp_rank] = c->d_mailbox;
   CC(cudaMemset(c->d_used, 0, NB), RC_ERR_CUDA);
   CC(cudaMemset(c->d_ref, 0, NB * 4), RC_ERR_CUDA);
   CC(cudaMemset(c->d_evcount, 0, 8), RC_ERR_CUDA);
@@ -392,7 +408,8 @@ static int fetch_res(rc_ctx* c, int set, u32 n) {
   return RC_OK;
 }
 static int emit(rc_ctx* c, int set, u32 n, int mode, u64 request_id = 0) {
-  k_emit<<<1, 256, 0, c->meta>>>(c->d_desc[set], c->d_res[set], n, mode, c->d_ring, c->cfg.max_events, c->d_evcount, request_id);
+  k_emit<<<1, 256, 0, c->meta>>>(c->d_desc[set], c->d_res[set], n, mode, c->d_ring, c->cfg.max_events, c->d_evcount, request_id,
+                                 c->tp_ranks > 1);
   CKL();
   c->st.kernel_launches++;
   return RC_OK;
@@ -755,6 +772,7 @@ static int wait_offload(rc_ctx* c) {
 // ---- a5-a8 restore ---------------------------------------------------------------------------------------
 extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
   GUARD();
+  if (c->tp_pending) return RC_ERR_BUSY;                   // a split (TP) restore is waiting for its commit
   if (c->dedup) return restore_begin_dedup(c, n, id, st);
   Op& op = c->ops[1];
   if (op.active) return RC_ERR_BUSY;
@@ -879,10 +897,25 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   CK(cudaEventRecord(c->ev_body_a[1], c->scatter));
   CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[1], 0));
   k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_etmp[1], c->d_dg, c->d_dg2, c->d_bt,
-                                               c->d_used, c->d_ref, c->fill, c->cfg.block_size);
+                                               c->d_used, c->d_ref, c->fill, c->cfg.block_size, c->tp_split ? 0 : 1);
   CKL();
   c->st.kernel_launches++;
-  if ((rc = emit(c, 1, n, EM_RESTORE, c->request_id))) return rc;
+  if (c->tp_split) {
+    // TP: publish the local verdicts (to the host for the all-gather path, into the peers' mailboxes for the NVLink
+    // path); the merged verdict is applied and the outcomes are emitted by rc_tp_restore_commit
+    k_tp_verdicts<<<(n + 255) / 256, 256, 0, c->meta>>>(c->d_res[1], n, c->d_verd);
+    CKL();
+    TpPeers peers;
+    for (u32 r = 0; r < TP_MAX_RANKS; ++r) {
+      u8* mb = r < c->tp_ranks ? c->peer_mb[r] : nullptr;
+      peers.flag[r] = (u64*)mb;
+      peers.rec[r] = mb ? (TpVerdict*)(mb + TP_MAX_RANKS * 8) : nullptr;
+    }
+    k_tp_push<<<1, 1024, 0, c->meta>>>(c->d_verd, n, peers, c->tp_ranks, c->tp_rank, (u32)c->desc_cap, c->tp_epoch);
+    CKL();
+    c->st.kernel_launches += 2;
+    CK(cudaMemcpyAsync(c->h_verd, c->d_verd, (u64)n * sizeof(TpVerdict), cudaMemcpyDeviceToHost, c->meta));
+  } else if ((rc = emit(c, 1, n, EM_RESTORE, c->request_id))) return rc;
   CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
   CK(cudaEventRecord(op.done, c->meta));
   c->ev_reserved += 4ull * n_served;
@@ -927,7 +960,7 @@ static int wait_restore(rc_ctx* c) {
 extern "C" int rc_wait(rc_ctx* c, int which) {
   GUARD();
   if (which == 0) return wait_offload(c);
-  if (which == 1) return wait_restore(c);
+  if (which == 1) return c->tp_pending ? RC_ERR_BUSY : wait_restore(c);   // a split restore ends with rc_tp_restore_commit
   return RC_ERR_INVALID;
 }
 extern "C" int rc_offload(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
@@ -937,6 +970,121 @@ extern "C" int rc_offload(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st
 extern "C" int rc_restore(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
   const int rc = rc_restore_begin(c, n, id, st);
   return rc ? rc : wait_restore(c);
+}
+
+// ---- NEXT-4: TP-sharded restore (rc.h; DESIGN.md 8 / R24) ---------------------------------------------------------
+extern "C" int rc_tp_restore_verify(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st, rc_tp_verdict* local) {
+  GUARD();
+  if (c->dedup || c->tp_pending || (n && (!id || !st || !local))) return RC_ERR_INVALID;
+  if (c->ops[1].active) return RC_ERR_BUSY;
+  ++c->tp_epoch;
+  c->tp_split = true;
+  const int rc = rc_restore_begin(c, n, id, st);
+  c->tp_split = false;
+  if (rc) { --c->tp_epoch; return rc; }
+  for (u32 k = 0; k < n; ++k) { local[k].flags = 0; local[k].bad = 0xFFFFFFFFu; }
+  Op& op = c->ops[1];
+  if (op.active) {
+    CK(cudaEventSynchronize(op.done));
+    memcpy(local, c->h_verd, (u64)n * sizeof(TpVerdict));
+    for (u32 k = 0; k < n; ++k) if (op.cl[k]) st[k] = -1;            // pending: decided by the commit
+  } else {
+    // nothing was served: this rank still publishes its (empty) records so that the peers' commits see its epoch
+    TpPeers peers;
+    for (u32 r = 0; r < TP_MAX_RANKS; ++r) {
+      u8* mb = r < c->tp_ranks ? c->peer_mb[r] : nullptr;
+      peers.flag[r] = (u64*)mb;
+      peers.rec[r] = mb ? (TpVerdict*)(mb + TP_MAX_RANKS * 8) : nullptr;
+    }
+    if (n) {
+      memcpy(c->h_verd, local, (u64)n * sizeof(TpVerdict));
+      CK(cudaMemcpyAsync(c->d_verd, c->h_verd, (u64)n * sizeof(TpVerdict), cudaMemcpyHostToDevice, c->meta));
+    }
+    k_tp_push<<<1, 1024, 0, c->meta>>>(c->d_verd, n, peers, c->tp_ranks, c->tp_rank, (u32)c->desc_cap, c->tp_epoch);
+    CKL();
+    c->st.kernel_launches++;
+    CK(cudaStreamSynchronize(c->meta));
+  }
+  c->tp_pending = true; c->tp_n = n;
+  return RC_OK;
+}
+
+extern "C" int rc_tp_restore_commit(rc_ctx* c, uint32_t n, uint32_t ranks, const rc_tp_verdict* gathered, int32_t* st) {
+  GUARD();
+  if (!c->tp_pending || n != c->tp_n || ranks != c->tp_ranks || (n && !st)) return RC_ERR_INVALID;
+  Op& op = c->ops[1];
+  const TpVerdict* src = nullptr;
+  u32 stride = 0;
+  CK(cudaMemsetAsync(c->d_counters, 0, 16, c->meta));
+  if (gathered) {                                          // all-gather path: [ranks][n] records from the caller
+    memcpy(c->h_verd, gathered, (u64)ranks * n * sizeof(TpVerdict));
+    if (n) CK(cudaMemcpyAsync(c->d_gath, c->h_verd, (u64)ranks * n * sizeof(TpVerdict), cudaMemcpyHostToDevice, c->meta));
+    src = c->d_gath; stride = n;
+  } else {                                                 // NVLink path: the peers wrote into this rank's mailbox
+    k_tp_ready<<<1, 32, 0, c->meta>>>((const u64*)c->d_mailbox, ranks, c->tp_epoch, c->d_counters);
+    CKL();
+    c->st.kernel_launches++;
+    CK(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->meta));
+    CK(cudaStreamSynchronize(c->meta));
+    if (c->h_counters[0]) return RC_ERR_BUSY;              // some peer has not published this epoch yet: barrier first
+    src = (const TpVerdict*)(c->d_mailbox + TP_MAX_RANKS * 8); stride = (u32)c->desc_cap;
+  }
+  if (!op.active) {                                        // nothing was served here; the peers must agree
+    if (n && gathered) for (u64 i = 0; i < (u64)ranks * n; ++i) if (gathered[i].flags & TV_SERVED) return RC_ERR_INVALID;
+    c->tp_pending = false;
+    return RC_OK;
+  }
+  k_tp_merge<<<(n + 255) / 256, 256, 0, c->meta>>>(c->d_res[1], n, src, stride, ranks, c->d_counters + 1);
+  CKL();
+  c->st.kernel_launches++;
+  CK(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->meta));
+  CK(cudaStreamSynchronize(c->meta));
+  if (c->h_counters[1]) return RC_ERR_INVALID;             // a rank disagrees on which claims were served: nothing applied
+  k_tp_apply<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_bt, c->d_used, c->d_ref, c->fill,
+                                                 c->cfg.block_size);
+  CKL();
+  c->st.kernel_launches++;
+  int rc;
+  if ((rc = emit(c, 1, n, EM_RESTORE, 0))) return rc;
+  CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
+  CK(cudaEventRecord(op.done, c->meta));
+  op.status = st;
+  c->tp_pending = false;
+  return wait_restore(c);
+}
+
+extern "C" int rc_tp_mailbox(rc_ctx* c, void** dev, uint64_t* bytes) {
+  GUARD();
+  if (!dev || !bytes) return RC_ERR_INVALID;
+  *dev = c->d_mailbox; *bytes = c->mailbox_bytes;
+  return RC_OK;
+}
+extern "C" int rc_tp_set_peer(rc_ctx* c, uint32_t rank, void* mailbox_dev) {
+  GUARD();
+  if (rank >= c->tp_ranks || rank == c->tp_rank) return RC_ERR_INVALID;
+  if (c->peer_ipc[rank] && c->peer_mb[rank]) { cudaIpcCloseMemHandle(c->peer_mb[rank]); c->peer_ipc[rank] = false; }
+  c->peer_mb[rank] = (u8*)mailbox_dev;
+  return RC_OK;
+}
+extern "C" int rc_tp_ipc_handle(rc_ctx* c, void* handle64) {
+  GUARD();
+  if (!handle64) return RC_ERR_INVALID;
+  cudaIpcMemHandle_t h;
+  CK(cudaIpcGetMemHandle(&h, c->d_mailbox));
+  static_assert(sizeof(h) == 64, "CUDA IPC handles are 64 bytes");
+  memcpy(handle64, &h, 64);
+  return RC_OK;
+}
+extern "C" int rc_tp_open_peer(rc_ctx* c, uint32_t rank, const void* handle64) {
+  GUARD();
+  if (rank >= c->tp_ranks || rank == c->tp_rank || !handle64) return RC_ERR_INVALID;
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle64, 64);
+  void* p = nullptr;
+  CK(cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess));
+  if (c->peer_ipc[rank] && c->peer_mb[rank]) cudaIpcCloseMemHandle(c->peer_mb[rank]);
+  c->peer_mb[rank] = (u8*)p; c->peer_ipc[rank] = true;
+  return RC_OK;
 }
 
 #include "rc_dedup.inl"

@@ -310,7 +310,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
   CK(cudaEventRecord(c->ev_body_a[1], c->scatter));
   CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[1], 0));
   k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_etmp[1], c->d_dg, c->d_dg2, c->d_bt,
-                                               c->d_used, c->d_ref, c->fill, c->cfg.block_size);
+                                               c->d_used, c->d_ref, c->fill, c->cfg.block_size, 1);
   CKL();
   c->st.kernel_launches++;
   if ((rc = emit(c, 1, n, EM_RESTORE, c->request_id))) return rc;

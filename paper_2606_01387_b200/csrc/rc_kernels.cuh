@@ -472,13 +472,24 @@ __global__ void k_restore_plan(const Desc* __restrict__ desc, Res* __restrict__ 
   }
 }
 
+// ok: fill of the claim's new blocks := leading tokens they hold.  not ok: the new blocks are freed.  (one warp)
+__device__ __forceinline__ void apply_verdict(const Desc& d, bool ok, const u32* __restrict__ bt, u8* __restrict__ used,
+                                              u32* __restrict__ ref, u8* __restrict__ fill, u32 BS) {
+  const u32 lane = threadIdx.x & 31;
+  for (u32 i = lane; i < d.nb; i += 32) {
+    const u32 b = bt[d.bt_off + i];
+    if (ok) { const u32 rem = d.M - i * BS; fill[b] = (u8)(rem < BS ? rem : BS); }
+    else { used[b] = 0; ref[b] = 0; fill[b] = 0; }
+  }
+}
+
 // K4 tail: verdict per served claim.  bad = first block whose recomputed digest differs; ok iff the
 // transfer was not suppressed, no block differs and the recomputed chain equals the recorded one.
 // ok: fill of the new blocks := leading tokens they hold.  not ok: the new blocks are freed.
 __global__ void k_verify(const Desc* __restrict__ desc, Res* __restrict__ res, u32 n, const u32* __restrict__ off,
                          const u64* __restrict__ d_tmp, const u64* __restrict__ e_tmp, const u64* __restrict__ dg,
                          const u64* __restrict__ dg2, const u32* __restrict__ bt,
-                         u8* __restrict__ used, u32* __restrict__ ref, u8* __restrict__ fill, u32 BS) {
+                         u8* __restrict__ used, u32* __restrict__ ref, u8* __restrict__ fill, u32 BS, int apply) {
   const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (k >= n) return;
   if (!(res[k].flag & R_SERVED)) return;
@@ -497,12 +508,75 @@ __global__ void k_verify(const Desc* __restrict__ desc, Res* __restrict__ res, u
     }
     ok = bad == 0xFFFFFFFFu && h == d.chain;
   }
-  for (u32 i = lane; i < d.nb; i += 32) {
-    const u32 b = bt[d.bt_off + i];
-    if (ok) { const u32 rem = d.M - i * BS; fill[b] = (u8)(rem < BS ? rem : BS); }
-    else { used[b] = 0; ref[b] = 0; fill[b] = 0; }
-  }
+  if (apply) apply_verdict(d, ok, bt, used, ref, fill, BS);          // TP mode applies the MERGED verdict later (k_tp_apply)
   if (lane == 0) res[k] = Res{R_SERVED | (ok ? (u32)R_OK : 0u), bad, d.chain};
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-4: TP-sharded KV, one common verdict (DESIGN.md 8 / R24).  Every rank verifies its kv_head shard
+// (k_verify, apply = 0) and publishes one 8-byte record per claim: flags (1 served, 2 locally ok) and bad.  k_tp_push
+// stores this rank's records straight into every peer's mailbox (peer-mapped device memory: the stores cross NVLink)
+// and then releases a per-source epoch flag; k_tp_merge folds the G records of each claim -- ok = AND, bad = min over
+// the failing ranks -- into res[], from a gathered buffer (all-gather path) or from this rank's own mailbox; k_tp_apply
+// is the second half of k_verify under the merged verdict.  No kernel ever waits for another rank: a mailbox whose
+// flags are not at the expected epoch is reported (k_tp_ready) and the host refuses the commit.
+// ---------------------------------------------------------------------------------------------
+struct TpVerdict { u32 flags, bad; };
+enum { TV_SERVED = 1, TV_OK = 2 };
+constexpr int TP_MAX_RANKS = 16;
+struct TpPeers { u64* flag[TP_MAX_RANKS]; TpVerdict* rec[TP_MAX_RANKS]; };   // per peer: its epoch flags, its record area
+
+__global__ void k_tp_verdicts(const Res* __restrict__ res, u32 n, TpVerdict* __restrict__ out) {
+  const u32 k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const Res r = res[k];
+  out[k] = (r.flag & R_SERVED) ? TpVerdict{(u32)TV_SERVED | ((r.flag & R_OK) ? (u32)TV_OK : 0u), r.val} : TpVerdict{0u, 0xFFFFFFFFu};
+}
+// one CTA: records to every open peer (slot [my_rank][k] of the peer's area), then the epoch flags, released system-wide
+__global__ void k_tp_push(const TpVerdict* __restrict__ local, u32 n, TpPeers peers, u32 G, u32 my_rank, u32 stride, u64 epoch) {
+  for (u32 p = 0; p < G; ++p) {
+    if (!peers.rec[p]) continue;
+    TpVerdict* dst = peers.rec[p] + (u64)my_rank * stride;
+    for (u32 k = threadIdx.x; k < n; k += blockDim.x) dst[k] = local[k];
+  }
+  __threadfence_system();
+  __syncthreads();
+  if (threadIdx.x < G && peers.flag[threadIdx.x]) {
+    asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(peers.flag[threadIdx.x] + my_rank), "l"(epoch) : "memory");
+  }
+}
+__global__ void k_tp_ready(const u64* __restrict__ flags, u32 G, u64 epoch, u32* __restrict__ not_ready) {
+  if (threadIdx.x < G) {
+    u64 v;
+    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(flags + threadIdx.x) : "memory");
+    if (v != epoch) atomicAdd(not_ready, 1u);
+  }
+}
+// src[r*stride + k] = record of rank r for batch entry k.  A rank that disagrees on `served` is a call-level error.
+__global__ void k_tp_merge(Res* __restrict__ res, u32 n, const TpVerdict* __restrict__ src, u32 stride, u32 G,
+                           u32* __restrict__ errors) {
+  const u32 k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  Res r = res[k];
+  const u32 served = (r.flag & R_SERVED) ? (u32)TV_SERVED : 0u;
+  bool ok = true; u32 bad = 0xFFFFFFFFu;
+  for (u32 q = 0; q < G; ++q) {
+    const TpVerdict v = src[(u64)q * stride + k];
+    if ((v.flags & TV_SERVED) != served) { atomicAdd(errors, 1u); return; }
+    if (!(v.flags & TV_OK)) { ok = false; bad = v.bad < bad ? v.bad : bad; }
+  }
+  if (!served) return;
+  r.flag = R_SERVED | (ok ? (u32)R_OK : 0u);
+  r.val = ok ? 0xFFFFFFFFu : bad;
+  res[k] = r;
+}
+__global__ void k_tp_apply(const Desc* __restrict__ desc, const Res* __restrict__ res, u32 n, const u32* __restrict__ bt,
+                           u8* __restrict__ used, u32* __restrict__ ref, u8* __restrict__ fill, u32 BS) {
+  const u32 k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (k >= n) return;
+  const Res r = res[k];
+  if (!(r.flag & R_SERVED)) return;
+  apply_verdict(desc[k], (r.flag & R_OK) != 0, bt, used, ref, fill, BS);
 }
 
 // K5: drop the claim's references to all its table blocks; a block whose count reaches 0 is free.
@@ -559,7 +633,7 @@ __global__ void k_accept(const Desc* __restrict__ desc, Res* __restrict__ res, u
 // records of claim k precede those of claim k+1 and seq is gap-free (P:L27 order per claim).
 // ---------------------------------------------------------------------------------------------
 __global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ res, u32 n, int mode,
-                       Event* __restrict__ ring, u32 ring_cap, u64* __restrict__ ev_count, u64 request_id) {
+                       Event* __restrict__ ring, u32 ring_cap, u64* __restrict__ ev_count, u64 request_id, int tp) {
   __shared__ u32 wt[32];
   const u64 seq0 = *ev_count;
   u32 carry = 0, carry_b = 0;
@@ -586,12 +660,12 @@ __global__ void k_emit(const Desc* __restrict__ desc, const Res* __restrict__ re
       };
       if (mode == EM_ACCEPT) put(EV_ACCEPTED, d.N, d.P);
       else if (mode == EM_MATERIALIZE) put(EV_MATERIALIZED, r.val, 0);
-      else if (mode == EM_OFFLOAD) put(EV_OFFLOADED, d.nb, r.chain);
+      else if (mode == EM_OFFLOAD) put(EV_OFFLOADED, d.nb, tp ? 0 : r.chain);   // TP: chains are rank-local, streams identical
       else if (mode == EM_DEMOTE) put(EV_DEMOTED, d.bt_len, request_id);          // victim: the boundary precedes the loss
       else if (mode == EM_CONFLICT) put(EV_CONFLICT_REFUSED, REQ_FLAG | n, request_id);   // all n descs are blocking claims
       else {
         put(EV_RESTORE_REQUIRED, d.M, 0);
-        if (r.flag & R_OK) put(EV_RESTORED, d.nb, d.chain);
+        if (r.flag & R_OK) put(EV_RESTORED, d.nb, tp ? 0 : d.chain);
         else {
           put(EV_LOAD_FAILED, r.val, 0);
           put(EV_RESTORATION_FAILED, 0, 0);

@@ -14,6 +14,7 @@ from . import build as _build
 
 EVENT_DTYPE = np.dtype([("seq", "<u8"), ("claim_id", "<u8"), ("code", "<u4"), ("aux", "<u4"), ("arg", "<u8")])
 FAULT_DTYPE = np.dtype([("claim_id", "<u8"), ("kind", "<u4"), ("param", "<u4")])
+TP_VERDICT_DTYPE = np.dtype([("flags", "<u4"), ("bad", "<u4")])      # rc_tp_verdict: flags 1 = served, 2 = locally ok
 
 OK, ERR_INVALID, ERR_CUDA, ERR_NOMEM, ERR_CAPACITY, ERR_BUSY = 0, -1, -2, -3, -4, -5
 ST_OK, ST_PRED_FALSE, ST_UNKNOWN_CLAIM, ST_BAD_STATE, ST_DUPLICATE_ID, ST_BAD_TABLE = 0, 1, 2, 3, 4, 5
@@ -25,7 +26,8 @@ POLICY_REFUSE, POLICY_DEMOTE, POLICY_EXPIRE = 0, 1, 2
 
 EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_accept", "rc_materialize", "rc_offload",
            "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_set_policy", "rc_restore_request",
-           "rc_restore_request_begin", "rc_protect", "rc_make_room", "rc_protected_map", "rc_outcomes", "rc_set_faults",
+           "rc_restore_request_begin", "rc_tp_restore_verify", "rc_tp_restore_commit", "rc_tp_mailbox", "rc_tp_set_peer",
+           "rc_tp_ipc_handle", "rc_tp_open_peer", "rc_protect", "rc_make_room", "rc_protected_map", "rc_outcomes", "rc_set_faults",
            "rc_release", "rc_claim_info", "rc_claim_blocks", "rc_claim_digests", "rc_host_read", "rc_host_store", "rc_sync", "rc_pool_state",
            "rc_stats_get", "rc_stats_reset", "rc_measure_link", "rc_digest_blocks", "rc_validate_trace", "rc_strerror",
            "rc_last_cuda_error"]
@@ -39,7 +41,8 @@ class Config(C.Structure):
                 ("pool_dev", C.c_void_p), ("fill_dev", C.c_void_p),
                 ("stream_meta", C.c_void_p), ("stream_gather", C.c_void_p), ("stream_d2h", C.c_void_p),
                 ("stream_scatter", C.c_void_p), ("stream_h2d", C.c_void_p),
-                ("mover", C.c_uint32), ("grid_ctas", C.c_uint32), ("dedup", C.c_uint32), ("direct_offload", C.c_uint32)]
+                ("mover", C.c_uint32), ("grid_ctas", C.c_uint32), ("dedup", C.c_uint32), ("direct_offload", C.c_uint32),
+                ("tp_ranks", C.c_uint32), ("tp_rank", C.c_uint32)]
 
 
 class ClaimInfo(C.Structure):
@@ -106,7 +109,8 @@ class RC:
 
     def __init__(self, layers, kv_heads, head_dim, elem_bytes, block_size, pool_blocks, pool, fill,
                  host_store_bytes, staging_chunk_bytes=None, staging_chunks=2, max_claims=8192,
-                 max_table_entries=None, max_events=1 << 17, streams=None, mover=MOVER_AUTO, grid_ctas=0, dedup=False, direct_offload=False):
+                 max_table_entries=None, max_events=1 << 17, streams=None, mover=MOVER_AUTO, grid_ctas=0, dedup=False, direct_offload=False,
+                 tp_ranks=0, tp_rank=0):
         self.L = lib()
         page = block_size * kv_heads * head_dim * elem_bytes
         self.page, self.blk, self.NB = page, 2 * layers * page, pool_blocks
@@ -118,7 +122,8 @@ class RC:
         cfg = Config(layers, kv_heads, head_dim, elem_bytes, block_size, pool_blocks, max_claims,
                      max_table_entries or max(4 * pool_blocks, 1 << 16), max_events, staging_chunks,
                      staging_chunk_bytes or min(1 << 30, max(self.blk, host_store_bytes)), host_store_bytes,
-                     pool.data_ptr(), fill.data_ptr(), s[0], s[1], s[2], s[3], s[4], mover, grid_ctas, int(dedup), int(direct_offload))
+                     pool.data_ptr(), fill.data_ptr(), s[0], s[1], s[2], s[3], s[4], mover, grid_ctas, int(dedup), int(direct_offload), tp_ranks, tp_rank)
+        self.tp_ranks = max(1, tp_ranks)
         self.h = C.c_void_p()
         rc = self.L.rc_create(C.byref(cfg), C.byref(self.h))
         if rc != 0:
@@ -211,6 +216,43 @@ class RC:
     def set_policy(self, ids, policy):
         ids, policy = _u64(ids), _u32(policy)
         return self.L.rc_set_policy(self.h, ids.size, _p(ids), _p(policy))
+
+    def tp_restore_verify(self, ids):
+        """Phase 1 of a TP-sharded restore (rc.h): returns (statuses, local verdict records)."""
+        ids = _u64(ids)
+        st = np.full(ids.size, -1, np.int32)
+        v = np.zeros(ids.size, TP_VERDICT_DTYPE)
+        self._ck(self.L.rc_tp_restore_verify(self.h, ids.size, _p(ids), _p(st), _p(v)), "rc_tp_restore_verify")
+        return st, v
+
+    def tp_restore_commit(self, gathered, st, check=True):
+        """Phase 2: gathered = [ranks, n] records of all ranks, or None to read this rank's peer mailbox."""
+        if gathered is None:
+            rc = self.L.rc_tp_restore_commit(self.h, st.size, self.tp_ranks, None, _p(st))
+        else:
+            g = np.ascontiguousarray(gathered, dtype=TP_VERDICT_DTYPE)
+            assert g.ndim == 2
+            rc = self.L.rc_tp_restore_commit(self.h, g.shape[1], g.shape[0], _p(g), _p(st))
+        if check:
+            self._ck(rc, "rc_tp_restore_commit")
+            return st
+        return rc, st
+
+    def tp_mailbox(self):
+        p, n = C.c_void_p(), C.c_uint64()
+        self._ck(self.L.rc_tp_mailbox(self.h, C.byref(p), C.byref(n)), "rc_tp_mailbox")
+        return p.value, n.value
+
+    def tp_set_peer(self, rank, mailbox_ptr):
+        return self.L.rc_tp_set_peer(self.h, rank, C.c_void_p(mailbox_ptr))
+
+    def tp_ipc_handle(self):
+        buf = C.create_string_buffer(64)
+        self._ck(self.L.rc_tp_ipc_handle(self.h, buf), "rc_tp_ipc_handle")
+        return buf.raw
+
+    def tp_open_peer(self, rank, handle):
+        self._ck(self.L.rc_tp_open_peer(self.h, rank, C.c_char_p(handle)), "rc_tp_open_peer")
 
     def protect(self, ids, on):
         ids, on = _u64(ids), _u32(on)
