@@ -161,16 +161,30 @@ int rc_offload(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* statu
  * its new blocks are freed). */
 int rc_restore(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
 
-/* Split forms (BASELINE.json configs[4]: restore of batch k overlapped with the offload of
- * batch k+1).  _begin validates, enqueues all device work and returns; the status array must
- * stay valid until rc_wait fills it in.  At most one offload and one restore may be in flight;
- * their data movement runs on separate stream pairs and overlaps; their metadata steps
- * (allocation, reference drops, verdicts, event emission) execute in _begin order, so the
- * result equals the synchronous calls made in that order.  rc_restore_begin blocks only until
- * its allocation plan is known.  which: 0 = offload, 1 = restore. */
+/* Split forms (BASELINE.json configs[4]: restore of batch k overlapped with the offload of the next batches on
+ * separate streams).  _begin validates, enqueues the data movement and returns; rc_wait completes the operation: the
+ * status array must stay valid until rc_wait fills it in.  which: 0 = offload, 1 = restore.
+ *   rc_offload_begin  enqueues a1-a3 and the chain on the gather / d2h streams.  Up to TWO offloads may be open; they
+ *       run back to back, so the D2H direction stays busy while a slower restore is still in flight.  The claims stay
+ *       referenced (their pool blocks are not free) until the offload is completed.  RC_ERR_BUSY with two open (one
+ *       in dedup / direct_offload mode; in dedup mode the content store is looked up and extended by this call).
+ *   rc_wait(ctx, 0)   completes the OLDEST open offload: waits for its transfer, then a4 -- reference drop, OFFLOADED.
+ *   rc_restore_begin  a5 (grant, allocation of the new blocks, fault decision) takes place now; a6 and the scatter are
+ *       enqueued on the h2d / scatter streams.  One restore may be in flight.  Blocks only until the plan is known.
+ *   rc_wait(ctx, 1)   completes the restore: waits for its data movement, then a7-a8 -- verdicts, fill / release of
+ *       the new blocks, RESTORE_REQUIRED and the outcome records; the host copy (its bytes in the pinned store) is
+ *       given back here.
+ * Between _begin and rc_wait the metadata stream is idle: accept / materialize / release of OTHER claims, rc_outcomes
+ * and further _begin calls do not wait for the transfers.  Metadata steps execute in call order on one stream, so
+ * every observable (statuses, allocation, events, seq numbers) equals the synchronous calls made in this order: an
+ * offload at its rc_wait(0); a restore's plan at its _begin and its outcome at its rc_wait(1) (the oracle's
+ * rco_restore_begin / rco_restore_end).  The claims of an operation in flight answer BAD_STATE to every other call.
+ * rc_test: *done = 1 if rc_wait(ctx, which) would not have to wait for data movement (the oldest open offload's gather
+ * and D2H have finished / the restore's H2D and scatter have finished / nothing is in flight), else 0.  Never blocks. */
 int rc_offload_begin(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
 int rc_restore_begin(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);
 int rc_wait(rc_ctx* ctx, int which);
+int rc_test(rc_ctx* ctx, int which, int* done);
 
 /* NEXT-3.  rc_set_policy: what a failed restoration means for each named claim -- refusal
  * (default), demotion or expiry ("claim-scoped restoration failure/refusal, demotion, expiry");
@@ -255,7 +269,8 @@ int rc_host_read(rc_ctx* ctx, uint64_t claim_id, void* dst, uint64_t cap, uint64
  * released or offloaded again; RC_ERR_BUSY while the claim's offload is in flight; RC_ERR_INVALID if the claim holds no
  * such host block.  (rc_host_read is the copying form.) */
 int rc_host_store(rc_ctx* ctx, uint64_t claim_id, uint32_t block, const void** p, uint64_t* contiguous_bytes);
-/* Completes every in-flight operation (as rc_wait(0), rc_wait(1)) and drains the library's streams. */
+/* Completes every in-flight operation (every open offload in _begin order as rc_wait(0), then rc_wait(1)) and drains
+ * the library's streams.  rc_offload (synchronous) likewise completes the offloads opened before it, then its own. */
 int rc_sync(rc_ctx* ctx);
 int rc_pool_state(rc_ctx* ctx, uint8_t* used /*NB*/, uint32_t* ref /*NB*/);
 int rc_stats_get(rc_ctx* ctx, rc_stats* out);

@@ -135,6 +135,9 @@ struct Claim {
   std::vector<Key> hkeys;     // dedup mode (NEXT-2): the claim's blocks as keys into the content-addressed store
 };
 
+struct Verdict { u32 flags, bad; };                     // flags: 1 = served, 2 = locally ok; bad = first bad block / 0xFFFFFFFF
+enum { V_SERVED = 1, V_OK = 2 };
+
 struct Ctx {
   u32 L, H, D, e, BS, NB;
   u64 page, blk, host_cap, host_used = 0;
@@ -150,6 +153,7 @@ struct Ctx {
   // NEXT-4: TP mode and the restore that waits between its two phases for the merged verdict
   u32 tp_ranks = 0;
   bool tp_pending = false; std::vector<u64> tp_ids; std::vector<void*> tp_served;
+  std::vector<Verdict> split_v; u64 split_request = 0;     // split form of restore: phase-1 verdicts and the request id
   // NEXT-2: content-addressed host store keyed by block digest, so blocks shared between claims
   // are held (and cross the link) once.  DESIGN.md "Dedup".
   bool dedup = false;
@@ -291,8 +295,6 @@ static void do_offload(Ctx* c, u32 n, const u64* ids, int32_t* st) {
 // arg = request id) -- blocking_claim_ids is exactly the failed subset ("smeared" ids fail closed).
 // The call is written in two phases so that a TP-sharded deployment (NEXT-4; below) can put the
 // cross-rank verdict merge between them; rco_restore runs them back to back with the local verdicts.
-struct Verdict { u32 flags, bad; };                     // flags: 1 = served, 2 = locally ok; bad = first bad block / 0xFFFFFFFF
-enum { V_SERVED = 1, V_OK = 2 };
 
 // phase 1: steps 1-3 and, of step 4, everything but the events: fault decision, write, re-digest, LOCAL verdict
 static void restore_verify(Ctx* c, u32 n, const u64* ids, int32_t* st, std::vector<Claim*>& served, std::vector<Verdict>& v) {
@@ -571,6 +573,32 @@ int rco_tp_restore_commit(void* h, u32 n, u32 G, const Verdict* gathered, int32_
     if (((merged[k].flags & V_SERVED) != 0) != (served[k] != nullptr)) return E_INVALID;
   }
   restore_commit(c, n, c->tp_ids.data(), st, served, merged, 0);
+  c->tp_pending = false;
+  return E_OK;
+}
+// Split form of restore (rc.h rc_restore_begin / rc_wait(1); reading R25): the same two phases that
+// rco_restore runs back to back, with other calls allowed in between -- phase 1 (eligibility, grant, allocation, fault
+// decision, write, re-digest, verdict) at _begin, phase 2 (RESTORE_REQUIRED and the outcome records, release of the host
+// copy, release of the blocks of failed claims) at _end.  No arithmetic of its own.
+int rco_restore_begin(void* h, u64 request_id, u32 n, const u64* id, int32_t* st) {
+  Ctx* c = (Ctx*)h;
+  if (c->tp_pending) return E_INVALID;
+  std::vector<Claim*> served;
+  restore_verify(c, n, id, st, served, c->split_v);
+  for (u32 k = 0; k < n; ++k) if (served[k]) st[k] = -1;      // pending: decided by _end
+  c->tp_ids.assign(id, id + n);
+  c->tp_served.assign(served.begin(), served.end());
+  c->split_request = request_id;
+  c->tp_pending = true;
+  return E_OK;
+}
+int rco_restore_end(void* h, int32_t* st) {
+  Ctx* c = (Ctx*)h;
+  if (!c->tp_pending) return E_INVALID;
+  const u32 n = (u32)c->tp_ids.size();
+  std::vector<Claim*> served(n);
+  for (u32 k = 0; k < n; ++k) served[k] = (Claim*)c->tp_served[k];
+  restore_commit(c, n, c->tp_ids.data(), st, served, c->split_v, c->split_request);
   c->tp_pending = false;
   return E_OK;
 }

@@ -193,6 +193,23 @@ class Oracle:
             raise ValueError("rco_tp_restore_commit: %d" % rc)
         return st
 
+    def restore_begin(self, ids, request_id=0):
+        """Split form (rc.h rc_restore_begin): phase 1 now; returns the statuses, -1 for served claims."""
+        ids = _u64(ids)
+        st = np.zeros(ids.size, np.int32)
+        rc = self.L.rco_restore_begin(self.h, C.c_uint64(request_id), ids.size, _p(ids), _p(st))
+        if rc != 0:
+            raise ValueError("rco_restore_begin: %d" % rc)
+        self._split_st = st
+        return st
+
+    def restore_end(self):
+        """Split form (rc_wait(1)): phase 2; completes and returns the statuses of restore_begin."""
+        rc = self.L.rco_restore_end(self.h, _p(self._split_st))
+        if rc != 0:
+            raise ValueError("rco_restore_end: %d" % rc)
+        return self._split_st
+
     def protect(self, ids, on):
         ids, on = _u64(ids), _u32(on)
         return self.L.rco_protect(self.h, ids.size, _p(ids), _p(on))

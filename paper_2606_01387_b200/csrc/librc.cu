@@ -103,6 +103,8 @@ struct Op {
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> t_kernel, t_copy;
   u64 blocks = 0, copy_bytes = 0, launches = 0;
   cudaEvent_t done = nullptr;
+  // restore: the reuse request it belongs to (0: per-claim refusals), TP split form, verdict kernels already enqueued
+  u64 request_id = 0; bool tp = false, tail = false;
 };
 
 }  // namespace
@@ -116,6 +118,7 @@ struct rc_ctx {
   bool own[5] = {false, false, false, false, false};
   u8* pool = nullptr; u8* fill = nullptr;
   u8* d_used = nullptr; u32* d_ref = nullptr; u32* d_bt = nullptr; u64* d_dg = nullptr; u64* d_dg2 = nullptr;
+  Event* h_evbuf = nullptr; u64 ev_bounce_cap = 0;         // rc_outcomes: mapped pinned bounce buffer
   Event* d_ring = nullptr; u64* d_evcount = nullptr; u32* d_bitmaps = nullptr; u32* d_up = nullptr;
   u32* d_counters = nullptr; u32* d_alloc = nullptr; u64* d_flip = nullptr;
   u32 *d_posmax = nullptr, *d_gain = nullptr; u8* d_protmap = nullptr; u64 accept_seq = 0;   // NEXT-3 allocator-side protection
@@ -123,14 +126,17 @@ struct rc_ctx {
   u32 tp_ranks = 0, tp_rank = 0, tp_n = 0; bool tp_split = false, tp_pending = false; u64 tp_epoch = 0;
   u8* d_mailbox = nullptr; u64 mailbox_bytes = 0; TpVerdict *d_verd = nullptr, *d_gath = nullptr, *h_verd = nullptr;
   u8* peer_mb[TP_MAX_RANKS] = {}; bool peer_ipc[TP_MAX_RANKS] = {};
-  Desc* d_desc[3] = {}; Res* d_res[3] = {}; u32* d_off[3] = {};
-  Desc* h_desc[3] = {}; Res* h_res[3] = {};
+  // descriptor / result sets: 0 = offload slot 0, 1 = restore, 2 = the synchronous metadata calls, 3 = offload slot 1
+  Desc* d_desc[4] = {}; Res* d_res[4] = {}; u32* d_off[4] = {};
+  Desc* h_desc[4] = {}; Res* h_res[4] = {};
   u32* h_up = nullptr; u64* h_flip = nullptr; u32* h_counters = nullptr;
-  u32* d_phys[2] = {}; u64* d_dtmp[2] = {}; u64* d_etmp[2] = {};
+  // per operation in flight: work list and block digests.  Index = op index: 0 = offload slot 0, 1 = restore, 2 = offload slot 1
+  u32* d_phys[3] = {}; u64* d_dtmp[3] = {}; u64* d_etmp[3] = {};
   std::vector<u8*> staging[2]; std::vector<u64*> part[2];
   std::vector<cudaEvent_t> ev_free[2], ev_ready[2];
   std::vector<bool> slot_used[2];
-  cudaEvent_t ev_plan[2] = {}, ev_body_a[2] = {}, ev_body_b[2] = {};
+  cudaEvent_t ev_plan[2] = {}, ev_body_a[3] = {}, ev_body_b[3] = {};   // ev_body_*: by op index
+  u64 chunk_seq[2] = {0, 0};                               // staging ring position per direction, running across operations
   std::vector<cudaEvent_t> ev_pool;
   u8* h_store = nullptr;
   ExtAlloc host_alloc, bt_alloc, dg_alloc;
@@ -139,7 +145,8 @@ struct rc_ctx {
   std::vector<rc_fault> faults; u32 fault_flags = 0;
   u64 ev_emitted = 0, ev_drained = 0, ev_reserved = 0;
   rc_stats st;
-  Op ops[2];
+  Op ops[3];                                               // by op index (above)
+  int off_q[2] = {0, 0}; int off_open = 0;                 // offloads begun and not yet completed by rc_wait(0), oldest first
   bool poisoned = false;
   std::string cuda_err;
   int accept_ctas = 32;
@@ -147,7 +154,6 @@ struct rc_ctx {
   u64 request_id = 0;                                    // NEXT-3: the reuse request of the restore being begun (0: per-claim)
   bool dedup = false;
   std::unordered_map<Key, std::pair<u32, u32>, KeyHash> store;   // (d, e) -> (slot, references)
-  std::vector<u32> pending_free;                         // slots of an in-flight restore, recycled at its completion
   u64 *h_dig = nullptr, *h_dig2 = nullptr; u32 *h_iw = nullptr, *h_ispos = nullptr, *d_iw = nullptr, *d_ispos = nullptr;
   // NEXT-4 (first half): gather straight into the mapped pinned store, no staging, no copy engine
   bool direct = false; u8* h_store_dev = nullptr; u32 *h_hpos = nullptr, *d_hpos = nullptr;
@@ -173,6 +179,23 @@ static cudaEvent_t get_event(rc_ctx* c) {
   cudaEventCreate(&e);
   return e;
 }
+
+// ---- small transfers ----------------------------------------------------------------------------------------
+// host_ptr is a mapped pinned buffer of the library (cudaHostAllocMapped); the words cross PCIe in a kernel on `s`, in
+// stream order, never through a copy engine (rc_kernels.cuh: k_copy_words).  bytes % 4 == 0.
+static cudaError_t small_copy(cudaStream_t s, void* dst, const void* src, u64 bytes, bool dst_is_host) {
+  if (!bytes) return cudaSuccess;
+  void* hd = nullptr;
+  cudaError_t e = cudaHostGetDevicePointer(&hd, dst_is_host ? dst : const_cast<void*>(src), 0);
+  if (e != cudaSuccess) return e;
+  const u64 n = bytes / 4;
+  const u32 grid = (u32)std::min<u64>((n + 255) / 256, 592);
+  if (dst_is_host) k_copy_words<<<grid, 256, 0, s>>>((u32*)hd, (const u32*)src, n);
+  else k_copy_words<<<grid, 256, 0, s>>>((u32*)dst, (const u32*)hd, n);
+  return cudaGetLastError();
+}
+static inline cudaError_t to_dev(cudaStream_t s, void* d, const void* h, u64 bytes) { return small_copy(s, d, h, bytes, false); }
+static inline cudaError_t to_host(cudaStream_t s, void* h, const void* d, u64 bytes) { return small_copy(s, h, d, bytes, true); }
 
 // ---- data movers -----------------------------------------------------------------------------
 template <int MODE>
@@ -227,19 +250,21 @@ extern "C" int rc_destroy(rc_ctx* c) {
   F(c->d_counters); F(c->d_alloc); F(c->d_flip); F(c->d_posmax); F(c->d_gain); F(c->d_protmap);
   for (u32 r = 0; r < TP_MAX_RANKS; ++r) if (c->peer_ipc[r] && c->peer_mb[r]) cudaIpcCloseMemHandle(c->peer_mb[r]);
   F(c->d_mailbox); F(c->d_verd); F(c->d_gath); FH(c->h_verd);
-  for (int i = 0; i < 3; ++i) { F(c->d_desc[i]); F(c->d_res[i]); F(c->d_off[i]); FH(c->h_desc[i]); FH(c->h_res[i]); }
-  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_store); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
+  for (int i = 0; i < 4; ++i) { F(c->d_desc[i]); F(c->d_res[i]); F(c->d_off[i]); FH(c->h_desc[i]); FH(c->h_res[i]); }
+  for (int i = 0; i < 3; ++i) {
+    F(c->d_phys[i]); F(c->d_dtmp[i]); F(c->d_etmp[i]);
+    if (c->ev_body_a[i]) cudaEventDestroy(c->ev_body_a[i]);
+    if (c->ev_body_b[i]) cudaEventDestroy(c->ev_body_b[i]);
+    if (c->ops[i].done) cudaEventDestroy(c->ops[i].done);
+  }
+  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_evbuf); FH(c->h_store); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
   F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
   for (int d = 0; d < 2; ++d) {
-    F(c->d_phys[d]); F(c->d_dtmp[d]); F(c->d_etmp[d]);
     for (auto p : c->staging[d]) F(p);
     for (auto p : c->part[d]) F(p);
     for (auto e : c->ev_free[d]) cudaEventDestroy(e);
     for (auto e : c->ev_ready[d]) cudaEventDestroy(e);
     if (c->ev_plan[d]) cudaEventDestroy(c->ev_plan[d]);
-    if (c->ev_body_a[d]) cudaEventDestroy(c->ev_body_a[d]);
-    if (c->ev_body_b[d]) cudaEventDestroy(c->ev_body_b[d]);
-    if (c->ops[d].done) cudaEventDestroy(c->ops[d].done);
   }
   for (auto e : c->ev_pool) cudaEventDestroy(e);
   cudaStream_t* ss[5] = {&c->meta, &c->gather, &c->d2h, &c->scatter, &c->h2d};
@@ -315,40 +340,47 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   CC(cudaMemset(c->d_mailbox, 0, c->mailbox_bytes), RC_ERR_CUDA);
   CC(cudaMalloc(&c->d_verd, dc * sizeof(TpVerdict)), RC_ERR_NOMEM);
   CC(cudaMalloc(&c->d_gath, (u64)c->tp_ranks * dc * sizeof(TpVerdict)), RC_ERR_NOMEM);
-  CC(cudaHostAlloc(&c->h_verd, (u64)c->tp_ranks * dc * sizeof(TpVerdict), cudaHostAllocDefault), RC_ERR_NOMEM);
+  CC(cudaHostAlloc(&c->h_verd, (u64)c->tp_ranks * dc * sizeof(TpVerdict), cudaHostAllocMapped), RC_ERR_NOMEM);
   c->peer_mb[c->tp_rank] = c->d_mailbox;
   CC(cudaMemset(c->d_used, 0, NB), RC_ERR_CUDA);
   CC(cudaMemset(c->d_ref, 0, NB * 4), RC_ERR_CUDA);
   CC(cudaMemset(c->d_evcount, 0, 8), RC_ERR_CUDA);
   CC(cudaMemset(c->d_bitmaps, 0, (u64)c->accept_ctas * ((NB + 31) / 32) * 4), RC_ERR_CUDA);
-  for (int i = 0; i < 3; ++i) {
+  for (int i = 0; i < 4; ++i) {
     CC(cudaMalloc(&c->d_desc[i], dc * sizeof(Desc)), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_res[i], dc * sizeof(Res)), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_off[i], (dc + 1) * 4), RC_ERR_NOMEM);
-    CC(cudaHostAlloc(&c->h_desc[i], dc * sizeof(Desc), cudaHostAllocDefault), RC_ERR_NOMEM);
-    CC(cudaHostAlloc(&c->h_res[i], dc * sizeof(Res), cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_desc[i], dc * sizeof(Desc), cudaHostAllocMapped), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_res[i], dc * sizeof(Res), cudaHostAllocMapped), RC_ERR_NOMEM);
   }
-  CC(cudaHostAlloc(&c->h_up, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
-  CC(cudaHostAlloc(&c->h_flip, dc * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
-  CC(cudaHostAlloc(&c->h_counters, 16, cudaHostAllocDefault), RC_ERR_NOMEM);
+  CC(cudaHostAlloc(&c->h_up, cap * 4, cudaHostAllocMapped), RC_ERR_NOMEM);
+  CC(cudaHostAlloc(&c->h_flip, dc * 8, cudaHostAllocMapped), RC_ERR_NOMEM);
+  CC(cudaHostAlloc(&c->h_counters, 16, cudaHostAllocMapped), RC_ERR_NOMEM);
+  c->ev_bounce_cap = std::min<u64>(cfg->max_events, 1u << 16);
+  CC(cudaHostAlloc(&c->h_evbuf, c->ev_bounce_cap * sizeof(Event), cudaHostAllocMapped), RC_ERR_NOMEM);
   c->dedup = cfg->dedup != 0;
   c->direct = cfg->direct_offload != 0 && !c->dedup;
   if (c->direct) {
-    CC(cudaHostAlloc(&c->h_hpos, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_hpos, cap * 4, cudaHostAllocMapped), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_hpos, cap * 4), RC_ERR_NOMEM);
   }
   if (c->dedup) {
-    CC(cudaHostAlloc(&c->h_dig, cap * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
-    CC(cudaHostAlloc(&c->h_dig2, cap * 8, cudaHostAllocDefault), RC_ERR_NOMEM);
-    CC(cudaHostAlloc(&c->h_iw, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
-    CC(cudaHostAlloc(&c->h_ispos, cap * 4, cudaHostAllocDefault), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_dig, cap * 8, cudaHostAllocMapped), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_dig2, cap * 8, cudaHostAllocMapped), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_iw, cap * 4, cudaHostAllocMapped), RC_ERR_NOMEM);
+    CC(cudaHostAlloc(&c->h_ispos, cap * 4, cudaHostAllocMapped), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_iw, cap * 4), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_ispos, cap * 4), RC_ERR_NOMEM);
   }
+  for (int i = 0; i < 3; ++i) {
+    CC(cudaMalloc(&c->d_phys[i], cap * 4), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_dtmp[i], cap * 8), RC_ERR_NOMEM);
+    CC(cudaMalloc(&c->d_etmp[i], cap * 8), RC_ERR_NOMEM);
+    CC(cudaEventCreateWithFlags(&c->ev_body_a[i], cudaEventDisableTiming), RC_ERR_CUDA);
+    CC(cudaEventCreateWithFlags(&c->ev_body_b[i], cudaEventDisableTiming), RC_ERR_CUDA);
+    CC(cudaEventCreateWithFlags(&c->ops[i].done, cudaEventDisableTiming), RC_ERR_CUDA);
+  }
   for (int d = 0; d < 2; ++d) {
-    CC(cudaMalloc(&c->d_phys[d], cap * 4), RC_ERR_NOMEM);
-    CC(cudaMalloc(&c->d_dtmp[d], cap * 8), RC_ERR_NOMEM);
-    CC(cudaMalloc(&c->d_etmp[d], cap * 8), RC_ERR_NOMEM);
     c->staging[d].assign(c->R, nullptr); c->part[d].assign(c->R, nullptr);
     c->ev_free[d].assign(c->R, nullptr); c->ev_ready[d].assign(c->R, nullptr);
     c->slot_used[d].assign(c->R, false);
@@ -359,9 +391,6 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
       CC(cudaEventCreateWithFlags(&c->ev_ready[d][r], cudaEventDisableTiming), RC_ERR_CUDA);
     }
     CC(cudaEventCreateWithFlags(&c->ev_plan[d], cudaEventDisableTiming), RC_ERR_CUDA);
-    CC(cudaEventCreateWithFlags(&c->ev_body_a[d], cudaEventDisableTiming), RC_ERR_CUDA);
-    CC(cudaEventCreateWithFlags(&c->ev_body_b[d], cudaEventDisableTiming), RC_ERR_CUDA);
-    CC(cudaEventCreateWithFlags(&c->ops[d].done, cudaEventDisableTiming), RC_ERR_CUDA);
   }
   if (c->host_blocks) CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocMapped), RC_ERR_NOMEM);
   if (c->host_blocks && c->direct) CC(cudaHostGetDevicePointer((void**)&c->h_store_dev, c->h_store, 0), RC_ERR_CUDA);
@@ -400,11 +429,11 @@ static int ev_room(rc_ctx* c, u64 extra) {
   return (c->ev_emitted - c->ev_drained) + c->ev_reserved + extra <= c->cfg.max_events;
 }
 static int upload_desc(rc_ctx* c, int set, u32 n) {
-  CK(cudaMemcpyAsync(c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc), cudaMemcpyHostToDevice, c->meta));
+  CK(to_dev(c->meta, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
   return RC_OK;
 }
 static int fetch_res(rc_ctx* c, int set, u32 n) {
-  CK(cudaMemcpyAsync(c->h_res[set], c->d_res[set], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
+  CK(to_host(c->meta, c->h_res[set], c->d_res[set], (u64)n * sizeof(Res)));
   return RC_OK;
 }
 static int emit(rc_ctx* c, int set, u32 n, int mode, u64 request_id = 0) {
@@ -425,7 +454,7 @@ static int mark(rc_ctx* c, u32 n, const u32* ids, int val) {
   for (u32 s = 0; s < n; s += (u32)c->cap_entries) {
     const u32 m = (u32)std::min<u64>(n - s, c->cap_entries);
     memcpy(c->h_up, ids + s, (u64)m * 4);
-    CK(cudaMemcpyAsync(c->d_up, c->h_up, (u64)m * 4, cudaMemcpyHostToDevice, c->meta));
+    CK(to_dev(c->meta, c->d_up, c->h_up, (u64)m * 4));
     k_mark<<<(m + 255) / 256, 256, 0, c->meta>>>(c->d_up, m, c->d_used, c->d_ref, val);
     CKL();
     c->st.kernel_launches++;
@@ -467,7 +496,7 @@ static int accept_run(rc_ctx* c, u32 n, const u64* id, const u32* P, const u32* 
   if (cand.empty()) return RC_OK;
   int rc;
   if ((rc = upload_desc(c, 2, n))) return rc;
-  CK(cudaMemcpyAsync(c->d_up, c->h_up, up * 4, cudaMemcpyHostToDevice, c->meta));
+  CK(to_dev(c->meta, c->d_up, c->h_up, up * 4));
   k_accept<<<std::min<u32>(n, c->accept_ctas), 256, 0, c->meta>>>(c->d_desc[2], c->d_res[2], n, c->d_up, c->d_bt, c->d_used,
                                                                  c->d_ref, c->NB, c->d_bitmaps);
   CKL();
@@ -606,16 +635,41 @@ extern "C" int rc_wait(rc_ctx* c, int which);
 // ---- a1-a4 offload ------------------------------------------------------------------------------------
 static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st);
 static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st);
+static void dedup_drop(rc_ctx* c, Claim& cl);
+
+// ---- offload slots ------------------------------------------------------------------------------------
+// Up to OFF_DEPTH offloads may be open (begun, not yet completed by rc_wait(0)); they run back to back on the gather
+// and d2h streams.  _begin enqueues a1-a3 and the chain; the a4 bookkeeping -- reference drop, OFFLOADED -- is enqueued
+// on `meta` when rc_wait(0) completes the oldest open offload, so on `meta` it takes the place of that call.
+constexpr int OFF_DEPTH = 2;
+static inline int off_oi(int slot) { return slot ? 2 : 0; }      // op index: ops[], d_phys[], d_dtmp[], d_etmp[], ev_body_*[]
+static inline int off_set(int slot) { return slot ? 3 : 0; }     // descriptor / result set
+static int off_take_slot(const rc_ctx* c) {
+  if (c->off_open >= OFF_DEPTH) return -1;
+  return c->off_open == 0 ? 0 : (c->off_q[0] ^ 1);
+}
+// data movement of the offload in `slot` is enqueued: mark its end on both streams and open it
+static int offload_opened(rc_ctx* c, int slot, u32 n_served) {
+  const int oi = off_oi(slot);
+  CK(cudaEventRecord(c->ev_body_a[oi], c->gather));
+  CK(cudaEventRecord(c->ev_body_b[oi], c->d2h));
+  c->ev_reserved += n_served;
+  c->ops[oi].active = true;
+  c->off_q[c->off_open++] = slot;
+  return RC_OK;
+}
 
 extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
   GUARD();
   if (c->dedup) return offload_begin_dedup(c, n, id, st);
-  Op& op = c->ops[0];
-  if (op.active) return RC_ERR_BUSY;
+  const int slot_o = off_take_slot(c);
+  if (slot_o < 0 || (c->direct && c->off_open)) return RC_ERR_BUSY;   // the direct mover's index buffer is single
   if (n == 0) return RC_OK;
   if (!id || !st || n > c->desc_cap) return RC_ERR_INVALID;
   if (!ev_room(c, n)) return RC_ERR_CAPACITY;
-  Desc* hd = c->h_desc[0];
+  const int oi = off_oi(slot_o), set = off_set(slot_o);
+  Op& op = c->ops[oi];
+  Desc* hd = c->h_desc[set];
   op.cl.assign(n, nullptr);
   std::vector<Seg> segs;
   std::vector<u32> served;
@@ -647,9 +701,8 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     old_dg.push_back({cl.dg_off, cl.dg_len});
     cl.dg_off = (u32)dgo; cl.dg_len = cl.nb;
     cl.host.clear();
-    // host space is granted by count in _begin order; the extents of a restore still in flight are
-    // physically released when it completes
-    if (c->host_alloc.free_total < cl.nb && c->ops[1].active) { const int wr = rc_wait(c, 1); if (wr) return wr; }
+    // host space is granted by count in _begin order (a restore in flight still holds its bytes: it gives them
+    // back when rc_wait(1) completes it)
     c->host_alloc.alloc_split(cl.nb, cl.host);
     c->host_used += (u64)cl.nb * c->blk;
     cl.busy = true;
@@ -668,17 +721,16 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   int rc;
   // The head (offsets, compaction) only reads tables that completed calls wrote, so it runs on the gather
   // stream: an offload begun after a restore does not queue behind that restore's tail on `meta`.
-  CK(cudaMemcpyAsync(c->d_desc[0], c->h_desc[0], (u64)n * sizeof(Desc), cudaMemcpyHostToDevice, c->gather));
-  k_offsets<<<1, 1024, 0, c->gather>>>(c->d_desc[0], n, c->d_off[0]);
+  CK(to_dev(c->gather, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
+  k_offsets<<<1, 1024, 0, c->gather>>>(c->d_desc[set], n, c->d_off[set]);
   CKL();
-  k_worklist<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_bt, nullptr, c->d_phys[0], 0);
+  k_worklist<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[set], c->d_res[set], n, c->d_off[set], c->d_bt, nullptr, c->d_phys[oi], 0);
   CKL();
   c->st.kernel_launches += 2;
   size_t si = 0;
-  u32 ci = 0;
-  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks, ++ci) {
+  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks) {
     const u64 w1 = std::min(T, w0 + c->chunk_blocks);
-    const u32 slot = ci % c->R, m = (u32)(w1 - w0);
+    const u32 slot = (u32)(c->chunk_seq[0]++ % c->R), m = (u32)(w1 - w0);      // the ring runs on across operations
     if (c->direct) {
       // the mover's destination is the claim's place in the mapped pinned store: the bulk stores of the gather
       // kernel cross the link themselves (item -> host block through the same indirection the dedup restore uses)
@@ -687,15 +739,15 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
         for (u64 w = std::max(g.w0, w0); w < std::min(g.w0 + g.n, w1); ++w) c->h_hpos[w] = (u32)(g.hoff + (w - g.w0));
         if (g.w0 + g.n <= w1) ++si; else break;
       }
-      CK(cudaMemcpyAsync(c->d_hpos + w0, c->h_hpos + w0, (u64)m * 4, cudaMemcpyHostToDevice, c->gather));
+      CK(to_dev(c->gather, c->d_hpos + w0, c->h_hpos + w0, (u64)m * 4));
       cudaEvent_t t0 = get_event(c), t1 = get_event(c);
       CK(cudaEventRecord(t0, c->gather));
-      launch_move<MV_GATHER>(c, c->gather, c->h_store_dev, c->d_phys[0] + w0, c->part[0][slot], m, nullptr, c->d_hpos + w0);
+      launch_move<MV_GATHER>(c, c->gather, c->h_store_dev, c->d_phys[oi] + w0, c->part[0][slot], m, nullptr, c->d_hpos + w0);
       CKL();
       CK(cudaEventRecord(t1, c->gather));
       op.t_copy.push_back({t0, t1});                       // the kernel IS the transfer
       op.copy_bytes += (u64)m * c->blk;
-      k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, c->d_etmp[0] + w0, m, c->G, nullptr);
+      k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[oi] + w0, c->d_etmp[oi] + w0, m, c->G, nullptr);
       CKL();
       c->st.kernel_launches++;
       continue;
@@ -703,12 +755,12 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     if (c->slot_used[0][slot]) CK(cudaStreamWaitEvent(c->gather, c->ev_free[0][slot], 0));
     cudaEvent_t t0 = get_event(c), t1 = get_event(c);
     CK(cudaEventRecord(t0, c->gather));
-    launch_move<MV_GATHER>(c, c->gather, c->staging[0][slot], c->d_phys[0] + w0, c->part[0][slot], m);
+    launch_move<MV_GATHER>(c, c->gather, c->staging[0][slot], c->d_phys[oi] + w0, c->part[0][slot], m);
     CKL();
     CK(cudaEventRecord(t1, c->gather));
     op.t_kernel.push_back({t0, t1});
     op.launches++;
-    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, c->d_etmp[0] + w0, m, c->G, nullptr);
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[oi] + w0, c->d_etmp[oi] + w0, m, c->G, nullptr);
     CKL();
     c->st.kernel_launches++;
     CK(cudaEventRecord(c->ev_ready[0][slot], c->gather));
@@ -721,41 +773,48 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     CK(cudaEventRecord(c->ev_free[0][slot], c->d2h));
     c->slot_used[0][slot] = true;
   }
-  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_dtmp[0], c->d_etmp[0], c->d_dg, c->d_dg2);
+  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[set], c->d_res[set], n, c->d_off[set], c->d_dtmp[oi], c->d_etmp[oi], c->d_dg, c->d_dg2);
   CKL();
   c->st.kernel_launches++;
-  CK(cudaEventRecord(c->ev_body_a[0], c->gather));
-  CK(cudaEventRecord(c->ev_body_b[0], c->d2h));
-  CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[0], 0));
-  CK(cudaStreamWaitEvent(c->meta, c->ev_body_b[0], 0));          // "offloaded" follows the finished transfer
-  k_unref<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[0], n, c->d_bt, c->d_used, c->d_ref);
-  CKL();
-  c->st.kernel_launches++;
-  if ((rc = emit(c, 0, n, EM_OFFLOAD))) return rc;
-  CK(cudaMemcpyAsync(c->h_res[0], c->d_res[0], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
-  CK(cudaEventRecord(op.done, c->meta));
-  c->ev_reserved += served.size();
-  op.active = true;
-  return RC_OK;
+  return offload_opened(c, slot_o, (u32)served.size());
 }
 
 static int collect_times(rc_ctx* c, Op& op, float& ms_k, float& ms_c) {
+  static const bool trace = getenv("RC_TRACE_LAUNCHES") != nullptr;      // diagnostics: per-launch device times on stderr
+  if (trace) {
+    const int dir = &op == &c->ops[1];
+    for (auto& p : op.t_kernel) { float ms = 0; cudaEventElapsedTime(&ms, p.first, p.second); fprintf(stderr, "librc trace: %s kernel %.4f ms\n", dir ? "scatter" : "gather", ms); }
+    for (auto& p : op.t_copy) { float ms = 0; cudaEventElapsedTime(&ms, p.first, p.second); fprintf(stderr, "librc trace: %s copy %.4f ms\n", dir ? "h2d" : "d2h", ms); }
+  }
   for (auto& p : op.t_kernel) { float ms = 0; CK(cudaEventElapsedTime(&ms, p.first, p.second)); ms_k += ms; c->ev_pool.push_back(p.first); c->ev_pool.push_back(p.second); }
   for (auto& p : op.t_copy) { float ms = 0; CK(cudaEventElapsedTime(&ms, p.first, p.second)); ms_c += ms; c->ev_pool.push_back(p.first); c->ev_pool.push_back(p.second); }
   op.t_kernel.clear(); op.t_copy.clear();
   return RC_OK;
 }
 
+// Completes the oldest open offload: a4 on `meta` (after the transfer: "offloaded" follows the finished copy),
+// then the host-side claim records.
 static int wait_offload(rc_ctx* c) {
-  Op& op = c->ops[0];
-  if (!op.active) return RC_OK;
-  CK(cudaEventSynchronize(op.done));
+  if (!c->off_open) return RC_OK;
+  const int slot = c->off_q[0], oi = off_oi(slot), set = off_set(slot);
+  Op& op = c->ops[oi];
+  const u32 n = op.n;
+  int rc;
+  CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[oi], 0));
+  CK(cudaStreamWaitEvent(c->meta, c->ev_body_b[oi], 0));
+  k_unref<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[set], n, c->d_bt, c->d_used, c->d_ref);
+  CKL();
+  c->st.kernel_launches++;
+  if ((rc = emit(c, set, n, EM_OFFLOAD))) return rc;
+  CK(to_host(c->meta, c->h_res[set], c->d_res[set], (u64)n * sizeof(Res)));
+  CK(cudaStreamSynchronize(c->meta));
   op.active = false;
+  c->off_q[0] = c->off_q[1]; --c->off_open;
   u64 served = 0;
   for (u32 k = 0; k < op.n; ++k) {
     Claim* cl = op.cl[k];
     if (!cl) continue;
-    cl->chain = c->h_res[0][k].chain;
+    cl->chain = c->h_res[set][k].chain;
     cl->state = RC_CS_OFFLOADED;
     c->bt_alloc.release(cl->bt_off, cl->bt_len);
     cl->bt_len = 0;
@@ -770,6 +829,50 @@ static int wait_offload(rc_ctx* c) {
 }
 
 // ---- a5-a8 restore ---------------------------------------------------------------------------------------
+// the restore's data movement is enqueued: mark its end and open it.  Its verdicts and outcome records (a7-a8) are
+// enqueued on `meta` by rc_wait(1), so on `meta` they take the place of that call; the plan (a5) took place at _begin.
+static int restore_opened(rc_ctx* c, u32 n_served) {
+  Op& op = c->ops[1];
+  CK(cudaEventRecord(c->ev_body_a[1], c->scatter));
+  op.request_id = c->request_id; op.tp = c->tp_split; op.tail = false;
+  c->ev_reserved += 4ull * n_served;
+  op.active = true;
+  return RC_OK;
+}
+// a7 on `meta`, after the data movement: digests and chain compared, verdict; then a8 -- or, in the TP split form, the
+// local verdict records published (to the host for the all-gather path, into the peers' mailboxes for the NVLink path):
+// there the merged verdict is applied and the outcomes are emitted by rc_tp_restore_commit.
+static int restore_tail(rc_ctx* c) {
+  Op& op = c->ops[1];
+  if (op.tail) return RC_OK;
+  const u32 n = op.n;
+  int rc;
+  CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[1], 0));
+  k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_etmp[1], c->d_dg, c->d_dg2, c->d_bt,
+                                               c->d_used, c->d_ref, c->fill, c->cfg.block_size, op.tp ? 0 : 1);
+  CKL();
+  c->st.kernel_launches++;
+  if (op.tp) {
+    k_tp_verdicts<<<(n + 255) / 256, 256, 0, c->meta>>>(c->d_res[1], n, c->d_verd);
+    CKL();
+    TpPeers peers;
+    for (u32 r = 0; r < TP_MAX_RANKS; ++r) {
+      u8* mb = r < c->tp_ranks ? c->peer_mb[r] : nullptr;
+      peers.flag[r] = (u64*)mb;
+      peers.rec[r] = mb ? (TpVerdict*)(mb + TP_MAX_RANKS * 8) : nullptr;
+    }
+    k_tp_push<<<1, 1024, 0, c->meta>>>(c->d_verd, n, peers, c->tp_ranks, c->tp_rank, (u32)c->desc_cap, c->tp_epoch);
+    CKL();
+    c->st.kernel_launches += 2;
+    CK(to_host(c->meta, c->h_verd, c->d_verd, (u64)n * sizeof(TpVerdict)));
+  } else {
+    if ((rc = emit(c, 1, n, EM_RESTORE, op.request_id))) return rc;
+    CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
+  }
+  op.tail = true;
+  return RC_OK;
+}
+
 extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
   GUARD();
   if (c->tp_pending) return RC_ERR_BUSY;                   // a split (TP) restore is waiting for its commit
@@ -809,7 +912,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
                                           c->d_counters);
   CKL();
   c->st.kernel_launches++;
-  CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
+  CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
   CK(cudaStreamSynchronize(c->meta));                    // the grant (which claims are served) is needed to plan the copies
   std::vector<Seg> segs;
   std::vector<std::pair<u64, u64>> flips;                // (work position, byte in block)
@@ -826,7 +929,6 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     }
     ++n_served;
     cl.busy = true;
-    c->host_used -= (u64)cl.nb * c->blk;                 // granted back at once (count); extents at completion
     // fault decision: the first armed entry naming exactly this claim, one-shot.  Entries naming any
     // other id never fire for it (wrong-claim / unclaimed failures are not claim outcomes: P:L25)
     rc_fault flt{0, 0, 0};
@@ -857,10 +959,9 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   std::sort(flips.begin(), flips.end());
   size_t si = 0, fi = 0;
   u64 flip_base = 0;
-  u32 ci = 0;
-  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks, ++ci) {
+  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks) {
     const u64 w1 = std::min(T, w0 + c->chunk_blocks);
-    const u32 slot = ci % c->R, m = (u32)(w1 - w0);
+    const u32 slot = (u32)(c->chunk_seq[1]++ % c->R), m = (u32)(w1 - w0);
     if (c->slot_used[1][slot]) CK(cudaStreamWaitEvent(c->h2d, c->ev_free[1][slot], 0));
     cudaEvent_t c0 = get_event(c), c1 = get_event(c);
     CK(cudaEventRecord(c0, c->h2d));
@@ -875,7 +976,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
       ++fi;
     }
     if (nf) {
-      CK(cudaMemcpyAsync(c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8, cudaMemcpyHostToDevice, c->scatter));
+      CK(to_dev(c->scatter, c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8));
       k_bitflip<<<(nf + 63) / 64, 64, 0, c->scatter>>>(c->staging[1][slot], c->d_flip + flip_base, nf);
       CKL();
       c->st.kernel_launches++;
@@ -894,45 +995,24 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     CK(cudaEventRecord(c->ev_free[1][slot], c->scatter));
     c->slot_used[1][slot] = true;
   }
-  CK(cudaEventRecord(c->ev_body_a[1], c->scatter));
-  CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[1], 0));
-  k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_etmp[1], c->d_dg, c->d_dg2, c->d_bt,
-                                               c->d_used, c->d_ref, c->fill, c->cfg.block_size, c->tp_split ? 0 : 1);
-  CKL();
-  c->st.kernel_launches++;
-  if (c->tp_split) {
-    // TP: publish the local verdicts (to the host for the all-gather path, into the peers' mailboxes for the NVLink
-    // path); the merged verdict is applied and the outcomes are emitted by rc_tp_restore_commit
-    k_tp_verdicts<<<(n + 255) / 256, 256, 0, c->meta>>>(c->d_res[1], n, c->d_verd);
-    CKL();
-    TpPeers peers;
-    for (u32 r = 0; r < TP_MAX_RANKS; ++r) {
-      u8* mb = r < c->tp_ranks ? c->peer_mb[r] : nullptr;
-      peers.flag[r] = (u64*)mb;
-      peers.rec[r] = mb ? (TpVerdict*)(mb + TP_MAX_RANKS * 8) : nullptr;
-    }
-    k_tp_push<<<1, 1024, 0, c->meta>>>(c->d_verd, n, peers, c->tp_ranks, c->tp_rank, (u32)c->desc_cap, c->tp_epoch);
-    CKL();
-    c->st.kernel_launches += 2;
-    CK(cudaMemcpyAsync(c->h_verd, c->d_verd, (u64)n * sizeof(TpVerdict), cudaMemcpyDeviceToHost, c->meta));
-  } else if ((rc = emit(c, 1, n, EM_RESTORE, c->request_id))) return rc;
-  CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
-  CK(cudaEventRecord(op.done, c->meta));
-  c->ev_reserved += 4ull * n_served;
-  op.active = true;
-  return RC_OK;
+  return restore_opened(c, n_served);
 }
 
 static int wait_restore(rc_ctx* c) {
   Op& op = c->ops[1];
   if (!op.active) return RC_OK;
-  CK(cudaEventSynchronize(op.done));
+  int rc;
+  if ((rc = restore_tail(c))) return rc;
+  CK(cudaStreamSynchronize(c->meta));
   op.active = false;
   const Desc* hd = c->h_desc[1];
   for (u32 k = 0; k < op.n; ++k) {
     Claim* cl = op.cl[k];
     if (!cl) continue;
     const Res r = c->h_res[1][k];
+    // the host copy ends with the restore (success or not): space and extents go back now
+    if (c->dedup) dedup_drop(c, *cl);
+    else c->host_used -= (u64)cl->nb * c->blk;
     for (auto& e : cl->host) c->host_alloc.release(e.first, e.second);
     cl->host.clear();
     cl->busy = false;
@@ -950,8 +1030,6 @@ static int wait_restore(rc_ctx* c) {
       op.status[k] = RC_ST_RESTORE_FAILED;
     }
   }
-  for (u32 sl : c->pending_free) c->host_alloc.release(sl, 1);
-  c->pending_free.clear();
   c->st.bytes_h2d += op.copy_bytes;
   c->st.scatter_launches += op.launches; c->st.scatter_blocks += op.blocks;
   return collect_times(c, op, c->st.ms_scatter, c->st.ms_h2d);
@@ -964,8 +1042,23 @@ extern "C" int rc_wait(rc_ctx* c, int which) {
   return RC_ERR_INVALID;
 }
 extern "C" int rc_offload(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
-  const int rc = rc_offload_begin(c, n, id, st);
-  return rc ? rc : wait_offload(c);
+  int rc = rc_offload_begin(c, n, id, st);
+  while (rc == RC_OK && c->off_open) rc = wait_offload(c);     // open offloads complete in _begin order, this one last
+  return rc;
+}
+extern "C" int rc_test(rc_ctx* c, int which, int* done) {
+  GUARD();
+  if (!done || which < 0 || which > 1) return RC_ERR_INVALID;
+  *done = 1;
+  cudaError_t e = cudaSuccess;
+  if (which == 0 && c->off_open) {                             // the transfer of the oldest open offload
+    const int oi = off_oi(c->off_q[0]);
+    e = cudaEventQuery(c->ev_body_a[oi]);
+    if (e == cudaSuccess) e = cudaEventQuery(c->ev_body_b[oi]);
+  } else if (which == 1 && c->ops[1].active) e = cudaEventQuery(c->ev_body_a[1]);   // H2D + scatter + digests
+  if (e == cudaErrorNotReady) { *done = 0; return RC_OK; }
+  CK(e);
+  return RC_OK;
 }
 extern "C" int rc_restore(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
   const int rc = rc_restore_begin(c, n, id, st);
@@ -985,7 +1078,9 @@ extern "C" int rc_tp_restore_verify(rc_ctx* c, uint32_t n, const uint64_t* id, i
   for (u32 k = 0; k < n; ++k) { local[k].flags = 0; local[k].bad = 0xFFFFFFFFu; }
   Op& op = c->ops[1];
   if (op.active) {
-    CK(cudaEventSynchronize(op.done));
+    int rt;
+    if ((rt = restore_tail(c))) return rt;               // local verdicts, published
+    CK(cudaStreamSynchronize(c->meta));
     memcpy(local, c->h_verd, (u64)n * sizeof(TpVerdict));
     for (u32 k = 0; k < n; ++k) if (op.cl[k]) st[k] = -1;            // pending: decided by the commit
   } else {
@@ -998,7 +1093,7 @@ extern "C" int rc_tp_restore_verify(rc_ctx* c, uint32_t n, const uint64_t* id, i
     }
     if (n) {
       memcpy(c->h_verd, local, (u64)n * sizeof(TpVerdict));
-      CK(cudaMemcpyAsync(c->d_verd, c->h_verd, (u64)n * sizeof(TpVerdict), cudaMemcpyHostToDevice, c->meta));
+      CK(to_dev(c->meta, c->d_verd, c->h_verd, (u64)n * sizeof(TpVerdict)));
     }
     k_tp_push<<<1, 1024, 0, c->meta>>>(c->d_verd, n, peers, c->tp_ranks, c->tp_rank, (u32)c->desc_cap, c->tp_epoch);
     CKL();
@@ -1018,13 +1113,13 @@ extern "C" int rc_tp_restore_commit(rc_ctx* c, uint32_t n, uint32_t ranks, const
   CK(cudaMemsetAsync(c->d_counters, 0, 16, c->meta));
   if (gathered) {                                          // all-gather path: [ranks][n] records from the caller
     memcpy(c->h_verd, gathered, (u64)ranks * n * sizeof(TpVerdict));
-    if (n) CK(cudaMemcpyAsync(c->d_gath, c->h_verd, (u64)ranks * n * sizeof(TpVerdict), cudaMemcpyHostToDevice, c->meta));
+    if (n) CK(to_dev(c->meta, c->d_gath, c->h_verd, (u64)ranks * n * sizeof(TpVerdict)));
     src = c->d_gath; stride = n;
   } else {                                                 // NVLink path: the peers wrote into this rank's mailbox
     k_tp_ready<<<1, 32, 0, c->meta>>>((const u64*)c->d_mailbox, ranks, c->tp_epoch, c->d_counters);
     CKL();
     c->st.kernel_launches++;
-    CK(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->meta));
+    CK(to_host(c->meta, c->h_counters, c->d_counters, 16));
     CK(cudaStreamSynchronize(c->meta));
     if (c->h_counters[0]) return RC_ERR_BUSY;              // some peer has not published this epoch yet: barrier first
     src = (const TpVerdict*)(c->d_mailbox + TP_MAX_RANKS * 8); stride = (u32)c->desc_cap;
@@ -1037,7 +1132,7 @@ extern "C" int rc_tp_restore_commit(rc_ctx* c, uint32_t n, uint32_t ranks, const
   k_tp_merge<<<(n + 255) / 256, 256, 0, c->meta>>>(c->d_res[1], n, src, stride, ranks, c->d_counters + 1);
   CKL();
   c->st.kernel_launches++;
-  CK(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->meta));
+  CK(to_host(c->meta, c->h_counters, c->d_counters, 16));
   CK(cudaStreamSynchronize(c->meta));
   if (c->h_counters[1]) return RC_ERR_INVALID;             // a rank disagrees on which claims were served: nothing applied
   k_tp_apply<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_bt, c->d_used, c->d_ref, c->fill,
@@ -1046,8 +1141,7 @@ extern "C" int rc_tp_restore_commit(rc_ctx* c, uint32_t n, uint32_t ranks, const
   c->st.kernel_launches++;
   int rc;
   if ((rc = emit(c, 1, n, EM_RESTORE, 0))) return rc;
-  CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
-  CK(cudaEventRecord(op.done, c->meta));
+  CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
   op.status = st;
   c->tp_pending = false;
   return wait_restore(c);
@@ -1144,7 +1238,7 @@ extern "C" int rc_make_room(rc_ctx* c, uint64_t request_id, uint32_t need, int32
                             uint32_t* n_ids) {
   GUARD();
   if (request_id == 0 || !status || !n_ids || (cap && !ids)) return RC_ERR_INVALID;
-  if (c->ops[0].active || c->ops[1].active) return RC_ERR_BUSY;
+  if (c->off_open || c->ops[1].active) return RC_ERR_BUSY;
   *n_ids = 0;
   std::vector<Claim*> list;
   u32 U = 0;
@@ -1166,7 +1260,7 @@ extern "C" int rc_make_room(rc_ctx* c, uint64_t request_id, uint32_t need, int32
   k_vic_decide<<<1, 1024, 0, c->meta>>>(c->d_gain, n, U, need, c->d_used, c->NB, c->d_counters);
   CKL();
   c->st.kernel_launches++;
-  CK(cudaMemcpyAsync(c->h_counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->meta));
+  CK(to_host(c->meta, c->h_counters, c->d_counters, 16));
   CK(cudaStreamSynchronize(c->meta));
   const u32 oc = c->h_counters[0], lo = c->h_counters[1], hi = c->h_counters[2];
   if (oc == VO_FITS) { *status = RC_ST_OK; return RC_OK; }
@@ -1204,7 +1298,7 @@ extern "C" int rc_make_room(rc_ctx* c, uint64_t request_id, uint32_t need, int32
 extern "C" int rc_protected_map(rc_ctx* c, uint8_t* prot) {
   GUARD();
   if (!prot) return RC_ERR_INVALID;
-  if (c->ops[0].active || c->ops[1].active) return RC_ERR_BUSY;
+  if (c->off_open || c->ops[1].active) return RC_ERR_BUSY;
   std::vector<Claim*> list;
   u32 U = 0;
   victim_list(c, list, U);
@@ -1230,13 +1324,19 @@ extern "C" int rc_outcomes(rc_ctx* c, rc_event* buf, uint64_t cap, uint64_t* n_o
   GUARD();
   if (!n_out || (cap && !buf)) return RC_ERR_INVALID;
   const u64 m = std::min<u64>(cap, c->ev_emitted - c->ev_drained), E = c->cfg.max_events;
+  // the records come back through a mapped pinned bounce buffer (small transfers: no copy engine), then to the caller
   u64 done = 0;
   while (done < m) {
-    const u64 at = (c->ev_drained + done) % E, l = std::min(m - done, E - at);
-    CK(cudaMemcpyAsync(buf + done, c->d_ring + at, l * sizeof(Event), cudaMemcpyDeviceToHost, c->util));
-    done += l;
+    u64 part = std::min<u64>(m - done, c->ev_bounce_cap), got = 0;
+    while (got < part) {
+      const u64 at = (c->ev_drained + done + got) % E, l = std::min(part - got, E - at);
+      CK(to_host(c->util, c->h_evbuf + got, c->d_ring + at, l * sizeof(Event)));
+      got += l;
+    }
+    CK(cudaStreamSynchronize(c->util));
+    memcpy(buf + done, c->h_evbuf, part * sizeof(Event));
+    done += part;
   }
-  CK(cudaStreamSynchronize(c->util));
   c->ev_drained += m;
   *n_out = m;
   return RC_OK;
@@ -1273,7 +1373,7 @@ extern "C" int rc_release(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st
     if (cl.dg_len) c->dg_alloc.release(cl.dg_off, cl.dg_len);
     for (auto& e : cl.host) c->host_alloc.release(e.first, e.second);
     if (!cl.host.empty()) c->host_used -= (u64)cl.nb * c->blk;
-    if (!cl.hkeys.empty()) dedup_drop(c, cl, c->ops[1].active);
+    if (!cl.hkeys.empty()) dedup_drop(c, cl);
     c->claims.erase(it);
     st[k] = RC_ST_OK;
   }
@@ -1364,8 +1464,8 @@ extern "C" int rc_host_store(rc_ctx* c, uint64_t id, uint32_t block, const void*
 }
 extern "C" int rc_sync(rc_ctx* c) {
   GUARD();
-  int rc = wait_offload(c);
-  if (rc) return rc;
+  int rc = RC_OK;
+  while (c->off_open) if ((rc = wait_offload(c))) return rc;
   if ((rc = wait_restore(c))) return rc;
   cudaStream_t ss[6] = {c->meta, c->gather, c->d2h, c->scatter, c->h2d, c->util};
   for (cudaStream_t s : ss) CK(cudaStreamSynchronize(s));
@@ -1402,7 +1502,7 @@ extern "C" int rc_stats_reset(rc_ctx* c) {
 extern "C" int rc_measure_link(rc_ctx* c, uint64_t bytes, int direction, int reps, double* gbs) {
   GUARD();
   if (!gbs || direction < 0 || direction > 2 || reps < 1) return RC_ERR_INVALID;
-  if (c->ops[0].active || c->ops[1].active) return RC_ERR_BUSY;
+  if (c->off_open || c->ops[1].active) return RC_ERR_BUSY;
   if (c->host_used != 0 || !c->store.empty()) return RC_ERR_BUSY;   // the measurement writes over the pinned store: only while it holds no claim bytes
   const u64 hs = c->host_blocks * c->blk, cs = c->chunk_blocks * c->blk;
   const u64 hmax = direction == 2 ? hs / 2 : hs;
@@ -1438,7 +1538,7 @@ extern "C" int rc_digest_blocks(rc_ctx* c, const void* src, uint32_t n_blocks, u
                                 float* ms_out) {
   GUARD();
   if (!src || ((uintptr_t)src & 15) || n_blocks > c->cap_entries) return RC_ERR_INVALID;
-  if (c->ops[0].active) return RC_ERR_BUSY;
+  if (c->off_open) return RC_ERR_BUSY;
   cudaEvent_t t0 = get_event(c), t1 = get_event(c);
   float total = 0;
   for (u64 w0 = 0; w0 < n_blocks; w0 += c->chunk_blocks) {

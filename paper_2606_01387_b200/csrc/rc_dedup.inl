@@ -7,24 +7,23 @@
 // item -> staged-block indirection, so a shared block crosses the link once per call; a claim with an injected
 // BITFLIP gets private staged copies, which keeps the corruption -- and the attribution -- on that claim alone
 // (P:L384).  Host space is granted as if every block were new (prefix sum, R7) and charged by content.
-// Reference drops of a restore take effect at _begin (so a later offload re-copies what the restore released,
-// exactly as the synchronous order would); the slots themselves are recycled when the restore completes.
+// The store is looked up and extended by rc_offload_begin (the keys come back chunk by chunk while the call runs); a
+// restore's references to the store end when rc_wait(1) completes it.
 
 static bool dedup_alloc_slot(rc_ctx* c, u32& slot, int& err) {
   u64 o;
   err = RC_OK;
-  if (c->host_alloc.free_total == 0 && c->ops[1].active) { err = rc_wait(c, 1); if (err) return false; }
   if (!c->host_alloc.alloc(1, o)) return false;
   slot = (u32)o;
   return true;
 }
 
-static void dedup_drop(rc_ctx* c, Claim& cl, bool defer) {      // the claim's references to the store
+static void dedup_drop(rc_ctx* c, Claim& cl) {                  // the claim's references to the store
   for (size_t i = 0; i < cl.hkeys.size(); ++i) {
     auto it = c->store.find(cl.hkeys[i]);
     if (it == c->store.end()) continue;
     if (--it->second.second == 0) {
-      if (defer) c->pending_free.push_back(it->second.first); else c->host_alloc.release(it->second.first, 1);
+      c->host_alloc.release(it->second.first, 1);
       c->store.erase(it);
       c->host_used -= c->blk;
     }
@@ -33,12 +32,13 @@ static void dedup_drop(rc_ctx* c, Claim& cl, bool defer) {      // the claim's r
 }
 
 static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
-  Op& op = c->ops[0];
-  if (op.active) return RC_ERR_BUSY;
+  if (c->off_open) return RC_ERR_BUSY;                     // one open offload: the keys come back through one host buffer
+  const int slot_o = 0, oi = off_oi(slot_o), set = off_set(slot_o);
+  Op& op = c->ops[oi];
   if (n == 0) return RC_OK;
   if (!id || !st || n > c->desc_cap) return RC_ERR_INVALID;
   if (!ev_room(c, n)) return RC_ERR_CAPACITY;
-  Desc* hd = c->h_desc[0];
+  Desc* hd = c->h_desc[set];
   op.cl.assign(n, nullptr);
   std::vector<u32> served;
   std::vector<u64> first_w;
@@ -80,30 +80,29 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
   for (auto& od : old_dg) if (od.second) c->dg_alloc.release(od.first, od.second);
   op.n = n; op.status = st; op.blocks = T; op.copy_bytes = 0; op.launches = 0;
   int rc;
-  CK(cudaMemcpyAsync(c->d_desc[0], c->h_desc[0], (u64)n * sizeof(Desc), cudaMemcpyHostToDevice, c->gather));
-  k_offsets<<<1, 1024, 0, c->gather>>>(c->d_desc[0], n, c->d_off[0]);
+  CK(to_dev(c->gather, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
+  k_offsets<<<1, 1024, 0, c->gather>>>(c->d_desc[set], n, c->d_off[set]);
   CKL();
-  k_worklist<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_bt, nullptr, c->d_phys[0], 0);
+  k_worklist<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[set], c->d_res[set], n, c->d_off[set], c->d_bt, nullptr, c->d_phys[oi], 0);
   CKL();
   c->st.kernel_launches += 2;
   size_t ci_claim = 0;                                     // served claim that owns the current work position
-  u32 ci = 0;
-  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks, ++ci) {
+  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks) {
     const u64 w1 = std::min(T, w0 + c->chunk_blocks);
-    const u32 slot = ci % c->R, m = (u32)(w1 - w0);
+    const u32 slot = (u32)(c->chunk_seq[0]++ % c->R), m = (u32)(w1 - w0);
     if (c->slot_used[0][slot]) CK(cudaStreamWaitEvent(c->gather, c->ev_free[0][slot], 0));
     cudaEvent_t t0 = get_event(c), t1 = get_event(c);
     CK(cudaEventRecord(t0, c->gather));
-    launch_move<MV_GATHER>(c, c->gather, c->staging[0][slot], c->d_phys[0] + w0, c->part[0][slot], m);
+    launch_move<MV_GATHER>(c, c->gather, c->staging[0][slot], c->d_phys[oi] + w0, c->part[0][slot], m);
     CKL();
     CK(cudaEventRecord(t1, c->gather));
     op.t_kernel.push_back({t0, t1});
     op.launches++;
-    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[0] + w0, c->d_etmp[0] + w0, m, c->G, nullptr);
+    k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[oi] + w0, c->d_etmp[oi] + w0, m, c->G, nullptr);
     CKL();
     c->st.kernel_launches++;
-    CK(cudaMemcpyAsync(c->h_dig + w0, c->d_dtmp[0] + w0, (u64)m * 8, cudaMemcpyDeviceToHost, c->gather));
-    CK(cudaMemcpyAsync(c->h_dig2 + w0, c->d_etmp[0] + w0, (u64)m * 8, cudaMemcpyDeviceToHost, c->gather));
+    CK(to_host(c->gather, c->h_dig + w0, c->d_dtmp[oi] + w0, (u64)m * 8));
+    CK(to_host(c->gather, c->h_dig2 + w0, c->d_etmp[oi] + w0, (u64)m * 8));
     CK(cudaEventRecord(c->ev_ready[0][slot], c->gather));
     CK(cudaStreamSynchronize(c->gather));                  // the keys decide which blocks cross the link
     CK(cudaStreamWaitEvent(c->d2h, c->ev_ready[0][slot], 0));
@@ -140,22 +139,10 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     CK(cudaEventRecord(c->ev_free[0][slot], c->d2h));
     c->slot_used[0][slot] = true;
   }
-  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[0], c->d_res[0], n, c->d_off[0], c->d_dtmp[0], c->d_etmp[0], c->d_dg, c->d_dg2);
+  k_chain<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[set], c->d_res[set], n, c->d_off[set], c->d_dtmp[oi], c->d_etmp[oi], c->d_dg, c->d_dg2);
   CKL();
   c->st.kernel_launches++;
-  CK(cudaEventRecord(c->ev_body_a[0], c->gather));
-  CK(cudaEventRecord(c->ev_body_b[0], c->d2h));
-  CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[0], 0));
-  CK(cudaStreamWaitEvent(c->meta, c->ev_body_b[0], 0));
-  k_unref<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[0], n, c->d_bt, c->d_used, c->d_ref);
-  CKL();
-  c->st.kernel_launches++;
-  if ((rc = emit(c, 0, n, EM_OFFLOAD))) return rc;
-  CK(cudaMemcpyAsync(c->h_res[0], c->d_res[0], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
-  CK(cudaEventRecord(op.done, c->meta));
-  c->ev_reserved += served.size();
-  op.active = true;
-  return RC_OK;
+  return offload_opened(c, slot_o, (u32)served.size());
 }
 
 static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st) {
@@ -193,7 +180,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
                                           c->d_counters);
   CKL();
   c->st.kernel_launches++;
-  CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
+  CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
   CK(cudaStreamSynchronize(c->meta));
   // staged blocks in first-appearance order; items = (work position, staged block)
   std::vector<u32> su;                                     // staged index -> host slot
@@ -231,7 +218,6 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     T += cl.nb;
   }
   if (n_served == 0) return RC_OK;
-  for (u32 k : elig) if (op.cl[k]) dedup_drop(c, *op.cl[k], true);   // references end here (order of calls); slots at completion
   if (c->fault_flags & RC_FAULT_ALLOW_UNCLAIMED)
     for (size_t f = 0; f < c->faults.size();)
       if (c->faults[f].claim_id == 0) { c->st.generic_failures++; c->faults.erase(c->faults.begin() + f); } else ++f;
@@ -245,8 +231,8 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     return a.first / c->chunk_blocks < b.first / c->chunk_blocks; });
   for (size_t j = 0; j < items.size(); ++j) { c->h_iw[j] = items[j].second; c->h_ispos[j] = (u32)(items[j].first % c->chunk_blocks); }
   if (!items.empty()) {
-    CK(cudaMemcpyAsync(c->d_iw, c->h_iw, items.size() * 4, cudaMemcpyHostToDevice, c->meta));
-    CK(cudaMemcpyAsync(c->d_ispos, c->h_ispos, items.size() * 4, cudaMemcpyHostToDevice, c->meta));
+    CK(to_dev(c->meta, c->d_iw, c->h_iw, items.size() * 4));
+    CK(to_dev(c->meta, c->d_ispos, c->h_ispos, items.size() * 4));
   }
   CK(cudaEventRecord(c->ev_plan[1], c->meta));
   CK(cudaStreamWaitEvent(c->scatter, c->ev_plan[1], 0));
@@ -257,7 +243,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
   const u64 U = su.size();
   for (u64 u0 = 0; u0 < U; u0 += c->chunk_blocks, ++ci) {
     const u64 u1 = std::min(U, u0 + c->chunk_blocks);
-    const u32 slot = ci % c->R;
+    const u32 slot = (u32)(c->chunk_seq[1]++ % c->R);
     if (c->slot_used[1][slot]) CK(cudaStreamWaitEvent(c->h2d, c->ev_free[1][slot], 0));
     cudaEvent_t c0 = get_event(c), c1 = get_event(c);
     CK(cudaEventRecord(c0, c->h2d));
@@ -282,7 +268,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
       ++fi;
     }
     if (nf) {
-      CK(cudaMemcpyAsync(c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8, cudaMemcpyHostToDevice, c->scatter));
+      CK(to_dev(c->scatter, c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8));
       k_bitflip<<<(nf + 63) / 64, 64, 0, c->scatter>>>(c->staging[1][slot], c->d_flip + flip_base, nf);
       CKL();
       c->st.kernel_launches++;
@@ -307,16 +293,5 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     CK(cudaEventRecord(c->ev_free[1][slot], c->scatter));
     c->slot_used[1][slot] = true;
   }
-  CK(cudaEventRecord(c->ev_body_a[1], c->scatter));
-  CK(cudaStreamWaitEvent(c->meta, c->ev_body_a[1], 0));
-  k_verify<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_off[1], c->d_dtmp[1], c->d_etmp[1], c->d_dg, c->d_dg2, c->d_bt,
-                                               c->d_used, c->d_ref, c->fill, c->cfg.block_size, 1);
-  CKL();
-  c->st.kernel_launches++;
-  if ((rc = emit(c, 1, n, EM_RESTORE, c->request_id))) return rc;
-  CK(cudaMemcpyAsync(c->h_res[1], c->d_res[1], (u64)n * sizeof(Res), cudaMemcpyDeviceToHost, c->meta));
-  CK(cudaEventRecord(op.done, c->meta));
-  c->ev_reserved += 4ull * n_served;
-  op.active = true;
-  return RC_OK;
+  return restore_opened(c, n_served);
 }

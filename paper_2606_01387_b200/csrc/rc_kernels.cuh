@@ -773,6 +773,13 @@ __global__ void k_prot_map(const Desc* __restrict__ desc, u32 n, const u32* __re
   for (u32 i = lane; i < d.bt_len; i += 32) map[bt[d.bt_off + i]] = 1;
 }
 
+// Small metadata transfers (descriptors, tables, results, event records: bytes to a few MB) between mapped pinned host
+// memory and device memory, word by word over PCIe.  The copy engines are left to the GiB-sized chunk copies: a 20 KB
+// cudaMemcpyAsync queued behind one of those in an engine's FIFO waits tens of milliseconds.
+__global__ void k_copy_words(u32* __restrict__ dst, const u32* __restrict__ src, u64 n_words) {
+  for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (u64)gridDim.x * blockDim.x) dst[i] = src[i];
+}
+
 // fault injection (CPU->GPU transfers only): flip bit 0 of the listed staged bytes
 __global__ void k_bitflip(u8* staging, const u64* __restrict__ offs, u32 n) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;

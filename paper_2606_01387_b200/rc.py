@@ -25,7 +25,7 @@ REQ_FLAG = 0x80000000
 POLICY_REFUSE, POLICY_DEMOTE, POLICY_EXPIRE = 0, 1, 2
 
 EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_accept", "rc_materialize", "rc_offload",
-           "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_set_policy", "rc_restore_request",
+           "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_test", "rc_set_policy", "rc_restore_request",
            "rc_restore_request_begin", "rc_tp_restore_verify", "rc_tp_restore_commit", "rc_tp_mailbox", "rc_tp_set_peer",
            "rc_tp_ipc_handle", "rc_tp_open_peer", "rc_protect", "rc_make_room", "rc_protected_map", "rc_outcomes", "rc_set_faults",
            "rc_release", "rc_claim_info", "rc_claim_blocks", "rc_claim_digests", "rc_host_read", "rc_host_store", "rc_sync", "rc_pool_state",
@@ -186,14 +186,14 @@ class RC:
         ids = _u64(ids)
         st = np.full(ids.size, -1, np.int32)
         self._ck(self.L.rc_offload_begin(self.h, ids.size, _p(ids), _p(st)), "rc_offload_begin")
-        self._pending[0] = (ids, st)
+        self._pending.setdefault(0, []).append((ids, st))      # up to two offloads may be open (rc.h)
         return st
 
     def restore_begin(self, ids):
         ids = _u64(ids)
         st = np.full(ids.size, -1, np.int32)
         self._ck(self.L.rc_restore_begin(self.h, ids.size, _p(ids), _p(st)), "rc_restore_begin")
-        self._pending[1] = (ids, st)
+        self._pending[1] = [(ids, st)]
         return st
 
     def restore_request(self, request_id, ids, check=True):
@@ -210,7 +210,7 @@ class RC:
         st = np.full(ids.size, -1, np.int32)
         self._ck(self.L.rc_restore_request_begin(self.h, C.c_uint64(request_id), ids.size, _p(ids), _p(st)),
                  "rc_restore_request_begin")
-        self._pending[1] = (ids, st)
+        self._pending[1] = [(ids, st)]
         return st
 
     def set_policy(self, ids, policy):
@@ -273,8 +273,14 @@ class RC:
 
     def wait(self, which):
         self._ck(self.L.rc_wait(self.h, which), "rc_wait")
-        ent = self._pending.pop(which, None)
-        return None if ent is None else ent[1]
+        q = self._pending.get(which)
+        return q.pop(0)[1] if q else None
+
+    def test(self, which):
+        """True if rc_wait(which) would not wait for a transfer."""
+        d = C.c_int(0)
+        self._ck(self.L.rc_test(self.h, which, C.byref(d)), "rc_test")
+        return bool(d.value)
 
     def outcomes(self, cap=1 << 20):
         buf = np.zeros(cap, EVENT_DTYPE)

@@ -97,8 +97,8 @@ def test_config1_full_size_bench_configuration():
 
 
 # ---- configs[2], [3], [4] at BASELINE.json's full size, in bench.py's launch configuration ----------------------------
-# (2 GiB staging chunks, default TMA movers, restore(k) overlapped with offload(k+1), waves placed as bench.py places
-# them).  What is checked, per wave: statuses and M from the recipe; for sampled claims (always the largest one, so the
+# (2 GiB staging chunks, default TMA movers, restore(k) overlapped with offload(k+1) and offload(k+2), waves placed as
+# bench.py places them).  What is checked, per wave: statuses and M from the recipe; for sampled claims (always the largest one, so the
 # claim spans the most staging chunks) sampled blocks -- first, last, both sides of every chunk boundary, random -- are
 # compared byte for byte between a torch copy taken before the offload, the pinned host store (rc_host_store view) and the
 # restored pool; their digests d, e and the claim's chain are recomputed by the oracle from the host bytes; every block of
@@ -126,7 +126,7 @@ class FullSize:
         _need(g.pool_bytes + (14 << 30), host_bytes + (12 << 30))
         self.dev = dev = torch.device("cuda:0")
         region = g.pool_blocks // wave_frac
-        self.waves = W.plan_waves(wl, host_bytes // 2, pool_blocks=region, max_claims_per_wave=max_claims_per_wave)[:n_waves]
+        self.waves = W.plan_waves(wl, host_bytes // 3, pool_blocks=region, max_claims_per_wave=max_claims_per_wave)[:n_waves]
         for wi, w in enumerate(self.waves):                       # bench.py's placement: two alternating top regions
             base = np.uint32(g.pool_blocks - (1 + wi % 2) * region)
             w.bt_ids, w.used_ids, w.fill_ids = w.bt_ids + base, w.used_ids + base, w.fill_ids + base
@@ -134,7 +134,7 @@ class FullSize:
         self.fill = torch.zeros(g.pool_blocks, dtype=torch.uint8, device=dev)
         n_max = max(len(w.claim_idx) for w in self.waves)
         self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, self.pool, self.fill,
-                       host_bytes, staging_chunk_bytes=2 << 30, staging_chunks=2, max_claims=max(1024, 2 * n_max),
+                       host_bytes, staging_chunk_bytes=2 << 30, staging_chunks=2, max_claims=max(1024, 4 * n_max),
                        max_table_entries=max(4 * g.pool_blocks, 1 << 16), max_events=max(1 << 16, 16 * n_max), dedup=dedup)
         self.view = self.pool.view(2 * g.layers, g.pool_blocks, g.page_bytes)
         self.rng = np.random.default_rng(100 + index)
@@ -233,32 +233,44 @@ class FullSize:
         torch.cuda.synchronize()
 
     def run(self, extra_faults=(), flags=0):
-        """bench.py's pipelined schedule: restore(k) is in flight while offload(k+1) runs."""
+        """bench.py's pipelined schedule: while restore(k) is in flight, offload(k+1) and offload(k+2) run back to back
+        (two open offloads); rc_wait(0) completes offload(k) before restore(k) begins."""
         r = self.r
-        a = self.admit(self.waves[0])
-        st = r.offload(a["ids"])
-        self.check_offloaded(a, st)
+        adm = [self.admit(w) for w in self.waves[:2]]
+        st_o = [r.offload_begin(a["ids"]) for a in adm]
         for k in range(len(self.waves)):
-            nxt = self.admit(self.waves[k + 1]) if k + 1 < len(self.waves) else None
+            a = adm[k]
+            r.wait(0)                                                        # completes offload(k)
+            self.check_offloaded(a, st_o[k])
+            if k + 2 < len(self.waves):
+                adm.append(self.admit(self.waves[k + 2]))                    # the region offload(k) has just left
             self.poison_free()                                               # restore must read the host copy
             faults = [(c.claim_id,) + c.fault for c in a["cl"] if c.fault] + list(extra_faults)
             assert r.set_faults(faults, flags) == 0
             st_r = r.restore_begin(a["ids"])
-            if nxt:
-                st_o = r.offload_begin(nxt["ids"])
-                r.wait(0)
+            if k + 2 < len(self.waves):
+                st_o.append(r.offload_begin(adm[k + 2]["ids"]))              # open: offload(k+1), offload(k+2)
             r.wait(1)
             self.check_restored(a, st_r)
-            if nxt:
-                self.check_offloaded(nxt, st_o)
             self.events.append(r.outcomes())
             assert not r.release(a["ids"]).any()
-            a = nxt
         ev = np.concatenate(self.events)
         ok, why = V.validate(ev)
         assert ok, why
         assert list(ev["seq"]) == list(range(len(ev)))
         return ev
+
+
+def test_config1_full_size_two_open_offloads():
+    """configs[1] (the workload bench.py's `value` is quoted on) in bench.py's default launch configuration: waves of 1/8 of
+    the 16 GiB pool in two alternating top regions, 2 GiB staging chunks, two open offloads ahead of the restore."""
+    fs = FullSize(1, wave_frac=8, host_bytes=16 << 30, n_waves=6)
+    ev = fs.run()
+    n_fault = sum(1 for w in fs.waves for k in w.claim_idx if fs.wl.claims[k].fault)
+    s = fs.r.stats()
+    assert s["claims_refused"] == n_fault and int((ev["code"] == 8).sum()) == n_fault
+    assert s["bytes_d2h"] == s["gather_blocks"] * fs.g.blk_bytes and s["bytes_h2d"] <= s["bytes_d2h"]
+    fs.close()
 
 
 def test_config2_llama70b_full_size():

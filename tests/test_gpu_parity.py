@@ -115,11 +115,13 @@ def test_config4_long_context_interleaved_reduced():
         if prev is None:
             assert np.array_equal(o.offload(ids), r.offload(ids))
         else:
-            # oracle: restore(prev) then offload(ids); cuda: both in flight at once, begun in that order
-            sa_r, sa_o = o.restore(prev), o.offload(ids)
+            # cuda: both in flight at once; the restore's plan takes effect at its _begin, the offload at rc_wait(0), the
+            # restore's verdicts and records at rc_wait(1) (rc.h split forms) -- the oracle makes exactly these calls
+            o.restore_begin(prev)
             r.restore_begin(prev)
             r.offload_begin(ids)
-            sb_o, sb_r = r.wait(0), r.wait(1)
+            sa_o, sb_o = o.offload(ids), r.wait(0)
+            sa_r, sb_r = o.restore_end(), r.wait(1)
             assert np.array_equal(sa_r, sb_r) and np.array_equal(sa_o, sb_o)
             p.check_claims(prev, "restore(k)")
             assert np.array_equal(o.release(prev), r.release(prev))
@@ -133,6 +135,82 @@ def test_config4_long_context_interleaved_reduced():
     ok, why = V.validate(ev)
     assert ok, why
     p.close()
+
+
+def test_two_open_offloads_run_ahead_of_a_restore():
+    """rc.h split forms: up to two offloads may be open; each takes effect (reference drop, OFFLOADED) at its rc_wait(0),
+    each restore at its _begin.  The bench schedule -- restore(k) in flight, offload(k+1) and offload(k+2) queued behind
+    each other on the D2H side -- must equal the oracle making the synchronous calls in exactly that order; a third open
+    offload is refused; rc_test never blocks."""
+    wl = W.make_workload(0, n_claims=32, pool_blocks=2048)      # tiny geometry: claim 6 is PRED_FALSE, claim 3 has a fault
+    p = Pair(wl, 1 << 30, chunk_blocks=37)                      # ~7 ragged chunks per wave
+    o, r = p.o, p.r
+    waves = W.plan_waves(wl, 1 << 30, max_claims_per_wave=8)
+    assert len(waves) == 4
+    top = wl.geom.pool_blocks
+
+    def admit(wave):                                            # tables at the top of the pool, restores land at the bottom
+        nonlocal top
+        cl = [wl.claims[k] for k in wave.claim_idx]
+        ids = [c.claim_id for c in cl]
+        remap = np.zeros(wl.geom.pool_blocks, np.uint32)
+        top -= wave.used_ids.size
+        remap[wave.used_ids] = np.arange(top, top + wave.used_ids.size, dtype=np.uint32)
+        p.set_fill(remap[wave.fill_ids], wave.fill_val)
+        assert o.mark_used(remap[wave.used_ids]) == 0 and r.mark_used(remap[wave.used_ids]) == 0
+        args = (ids, [c.P for c in cl], [c.N for c in cl], wave.bt_off, remap[wave.bt_ids])
+        assert np.array_equal(o.accept(*args), r.accept(*args))
+        assert np.array_equal(o.materialize(ids), r.materialize(ids))
+        return ids
+
+    ids = [admit(w) for w in waves]
+    assert r.test(0) and r.test(1)                              # nothing in flight
+    r.offload_begin(ids[0])
+    r.offload_begin(ids[1])
+    rc3, _ = r._batch(r.L.rc_offload_begin, "rc_offload_begin", ids[2], check=False)
+    assert rc3 == rc.ERR_BUSY                                   # a third open offload is refused and changes nothing
+    assert np.array_equal(o.offload(ids[0]), r.wait(0))         # completes O0 only
+    p.check_claims(ids[0], "O0", host=True)
+    assert r.claim_info(ids[1][0])["state"] == 2                # O1 is open: still MATERIALIZED, blocks still referenced
+    for k in range(3):
+        p.poison_free()
+        fl = [(ids[k][1], rc.FAULT_BITFLIP, 12345 + k)] if k != 1 else [(ids[k][2], rc.FAULT_XFER_ERROR, 0)]
+        fl += wl_faults(wl, ids[k])
+        assert o.set_faults(fl) == 0 and r.set_faults(fl) == 0
+        sa_r = o.restore(ids[k])                                # oracle: R(k), then O(k+1) where cuda completes it
+        r.restore_begin(ids[k])
+        if k + 2 < 4:
+            r.offload_begin(ids[k + 2])                         # open now: O(k+1), O(k+2); R(k) in flight
+        while not (r.test(0) and r.test(1)):
+            pass
+        assert np.array_equal(sa_r, r.wait(1))
+        assert np.array_equal(o.offload(ids[k + 1]), r.wait(0))
+        p.check_claims(ids[k], "R%d" % k)
+        p.check_claims(ids[k + 1], "O%d" % (k + 1), host=True)
+        p.check_pool_state("round %d" % k, bytes_too=True)
+        assert np.array_equal(o.release(ids[k]), r.release(ids[k]))
+    p.poison_free()
+    assert np.array_equal(o.restore(ids[3]), r.restore(ids[3]))
+    p.check_pool_state("last restore")
+    back = [c for c in ids[3] if r.claim_info(c)["state"] == 4]
+    r.offload_begin(back[:4])                                   # two open offloads completed by rc_sync, in _begin order
+    r.offload_begin(back[4:])
+    o.offload(back[:4]), o.offload(back[4:])
+    r.sync()
+    p.check_claims(back, "sync", host=True)
+    p.check_pool_state("sync", bytes_too=False)
+    ev = p.check_events("two open offloads")
+    ok, why = V.validate(ev)
+    assert ok, why
+    s = r.stats()
+    assert o.link_bytes() == (s["bytes_d2h"], s["bytes_h2d"])
+    p.close()
+
+
+def wl_faults(wl, ids):
+    """the workload's own fault entries for the claims in ids"""
+    want = set(ids)
+    return [(c.claim_id,) + c.fault for c in wl.claims if c.fault and c.claim_id in want]
 
 
 def test_edge_cases_fail_closed():
@@ -338,8 +416,8 @@ def test_dedup_config2_shared_prefixes_reduced():
 
 
 def test_dedup_overlapped_begin_wait_matches_synchronous_order():
-    """restore(k) in flight while offload(k+1) dedups against the store: the restore's reference drops
-    take effect at _begin, so the overlapped run equals the oracle's synchronous order."""
+    """restore(k) in flight while offload(k+1) dedups against the store: the restore holds its references until
+    rc_wait(1), so blocks of k that reappear in k+1 are not copied again; equal to the oracle making the same split calls."""
     wl, wave, copies = make_shared_tiny()
     ids = [c.claim_id for c in wl.claims]
     p = Pair(wl, 1 << 30, chunk_blocks=11, dedup=True, copies=copies)
@@ -353,10 +431,11 @@ def test_dedup_overlapped_begin_wait_matches_synchronous_order():
     a, b = ids[:3], ids[3:]
     assert np.array_equal(o.offload(a), r.offload(a))
     p.poison_free()
-    sa_r, sa_o = o.restore(a), o.offload(b)
+    o.restore_begin(a)
     r.restore_begin(a)
-    r.offload_begin(b)
-    sb_o, sb_r = r.wait(0), r.wait(1)
+    r.offload_begin(b)                       # the store is looked up now: a's blocks are still held by the restore in flight
+    sa_o, sb_o = o.offload(b), r.wait(0)
+    sa_r, sb_r = o.restore_end(), r.wait(1)
     assert np.array_equal(sa_r, sb_r) and np.array_equal(sa_o, sb_o)
     p.check_claims(ids, "overlap", host=True)
     p.check_pool_state("overlap")
