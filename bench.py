@@ -95,6 +95,7 @@ class Job:
         # of the pool (>= 2 so that two waves fit) keep the un-overlapped first offload and last restore short;
         # serial: one wave owns the pool and the host store
         self.pipelined = pipelined
+        self.one_open = bool(dedup or direct)
         mc = self.wl.batch or None                    # configs[4]: interleaved batches of 8 claims
         if pipelined:
             while True:                               # largest claims (configs[4]: up to 8192 blocks) may need bigger waves
@@ -188,7 +189,7 @@ class Job:
             nmax = max(p["n"] for p in self.prep)
             # how many waves may be admitted ahead of the wave being restored: wave j+2 of a two-wave workload (j+1 of a
             # one-wave workload) carries the claim ids of wave j and can only be admitted after its release
-            ahead = min(2, len(self.prep) - 1)
+            ahead = min(1 if self.one_open else 2, len(self.prep) - 1)   # dedup / direct_offload: one open offload (rc.h)
             adm = 0
 
             def push():

@@ -23,6 +23,8 @@
 #include <unordered_map>
 #include <unordered_set>
 #include <vector>
+#include <sys/mman.h>
+#include <thread>
 
 using namespace rck;
 
@@ -138,7 +140,7 @@ struct rc_ctx {
   cudaEvent_t ev_plan[2] = {}, ev_body_a[3] = {}, ev_body_b[3] = {};   // ev_body_*: by op index
   u64 chunk_seq[2] = {0, 0};                               // staging ring position per direction, running across operations
   std::vector<cudaEvent_t> ev_pool;
-  u8* h_store = nullptr;
+  u8* h_store = nullptr; bool h_store_registered = false; u64 h_store_bytes = 0;
   ExtAlloc host_alloc, bt_alloc, dg_alloc;
   u64 host_used = 0;
   std::unordered_map<u64, Claim> claims;
@@ -257,8 +259,10 @@ extern "C" int rc_destroy(rc_ctx* c) {
     if (c->ev_body_b[i]) cudaEventDestroy(c->ev_body_b[i]);
     if (c->ops[i].done) cudaEventDestroy(c->ops[i].done);
   }
-  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_evbuf); FH(c->h_store); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
+  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_evbuf); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
   F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
+  if (c->h_store && c->h_store_registered) { cudaHostUnregister(c->h_store); munmap(c->h_store, c->h_store_bytes); }
+  else FH(c->h_store);
   for (int d = 0; d < 2; ++d) {
     for (auto p : c->staging[d]) F(p);
     for (auto p : c->part[d]) F(p);
@@ -392,7 +396,24 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
     }
     CC(cudaEventCreateWithFlags(&c->ev_plan[d], cudaEventDisableTiming), RC_ERR_CUDA);
   }
-  if (c->host_blocks) CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocMapped), RC_ERR_NOMEM);
+  if (c->host_blocks) {
+    // The pinned store.  RC_HOST_STORE=thp: anonymous memory advised to transparent huge pages, touched in parallel,
+    // then registered -- 2 MiB-contiguous physical runs for the link's address translation; default: cudaHostAlloc.
+    const char* hs = getenv("RC_HOST_STORE");
+    if (hs && !strcmp(hs, "thp")) {
+      const u64 bytes = (c->host_blocks * blk + (2ull << 20) - 1) & ~((2ull << 20) - 1);
+      void* p = mmap(nullptr, bytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0);
+      if (p == MAP_FAILED) return fail(RC_ERR_NOMEM, "mmap(host store)", cudaSuccess);
+      madvise(p, bytes, MADV_HUGEPAGE);
+      const unsigned nt = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+      std::vector<std::thread> th;
+      for (unsigned t = 0; t < nt; ++t)
+        th.emplace_back([=]() { for (u64 o = (u64)t << 21; o < bytes; o += (u64)nt << 21) memset((u8*)p + o, 0, std::min<u64>(2ull << 20, bytes - o)); });
+      for (auto& t : th) t.join();
+      c->h_store = (u8*)p; c->h_store_bytes = bytes; c->h_store_registered = true;
+      CC(cudaHostRegister(p, bytes, cudaHostRegisterPortable | cudaHostRegisterMapped), RC_ERR_NOMEM);
+    } else CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocMapped), RC_ERR_NOMEM);
+  }
   if (c->host_blocks && c->direct) CC(cudaHostGetDevicePointer((void**)&c->h_store_dev, c->h_store, 0), RC_ERR_CUDA);
   // launch geometry of the movers
   c->mover = cfg->mover == RC_MOVER_AUTO ? RC_MOVER_TMA : cfg->mover;
