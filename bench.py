@@ -82,7 +82,8 @@ def host_ram_bytes():
 class Job:
     """One rank's workload: context, resident pool, pre-marshalled waves."""
 
-    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=8, dedup=False, direct=False):
+    def __init__(self, index, rank, n_gpus, chunk_bytes, mover, grid_ctas, host_cap=None, pipelined=True, wave_frac=8, dedup=False, direct=False,
+                 layer_major=False):
         import torch
         from paper_2606_01387_b200 import rc
         self.torch, self.rc = torch, rc
@@ -116,7 +117,7 @@ class Job:
         self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, self.pool, self.fill,
                        self.host_store, staging_chunk_bytes=min(chunk_bytes, self.host_store), staging_chunks=2,
                        max_claims=max(1024, 4 * n_max), max_table_entries=max(4 * g.pool_blocks, 1 << 16),
-                       max_events=max(1 << 16, 16 * n_max), mover=mover, grid_ctas=grid_ctas, dedup=dedup, direct_offload=direct)
+                       max_events=max(1 << 16, 16 * n_max), mover=mover, grid_ctas=grid_ctas, dedup=dedup, direct_offload=direct, layer_major=layer_major)
         region = g.pool_blocks // wave_frac if pipelined else 0
         dev_ = dev
 
@@ -376,6 +377,7 @@ def main():
     ap.add_argument("--wave-frac", type=int, default=8, help="pipelined schedule: a wave uses 1/N of the pool (N >= 2)")
     ap.add_argument("--dedup", action="store_true", help="NEXT-2: content-addressed host store; value counts claim-logical bytes")
     ap.add_argument("--direct-offload", action="store_true", help="NEXT-4 experiment: gather straight into the mapped pinned store")
+    ap.add_argument("--layer-major", action="store_true", help="NEXT-4: layer-major host copy and streaming order")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--per-config-budget-s", type=float, default=160.0,
@@ -413,7 +415,8 @@ def main():
     from paper_2606_01387_b200 import rc, tp
     numa = tp.bind_to_gpu_numa_node(local)      # before rc_create: the pinned store is first touched on the GPU's node
     mover = {"auto": rc.MOVER_AUTO, "ldg": rc.MOVER_LDG, "tma": rc.MOVER_TMA}[a.mover]
-    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac), dedup=a.dedup, direct=a.direct_offload)
+    job = Job(a.config, rank, world, a.chunk_mib << 20, mover, a.grid, pipelined=not a.serial, wave_frac=max(2, a.wave_frac), dedup=a.dedup, direct=a.direct_offload,
+              layer_major=a.layer_major)
     g = job.g
     link = {}
 
@@ -511,7 +514,7 @@ def main():
                        "waves": len(job.waves), "host_store_bytes": job.host_store, "staging_chunk_bytes": a.chunk_mib << 20,
                        "mover": a.mover, "schedule": "serial" if a.serial else "restore(k) overlapped with offload(k+1) and offload(k+2) (two open offloads); waves of consecutive steps form one sequence", "l2": "inputs larger than L2 (pool %d GiB, staging chunks %d MiB, L2 126 MB)" % (g.pool_bytes >> 30, a.chunk_mib),
                        "parallelism": "claims independent: one replica of the workload per GPU, no collective",
-                       "numa_node": numa},
+                       "numa_node": numa, "layer_major": bool(a.layer_major)},
             "claims_per_s": claims_all / (ms_max / 1e3), "payload_bytes_per_step": payload_all / a.steps,
             "wall_ms_per_step": wall_ms / a.steps, "clocks": clocks, "gpu_launches": int(launches_all),
             "dedup": ({"link_bytes_per_step": link_bytes / a.steps, "logical_bytes_per_step": payload / a.steps,

@@ -105,6 +105,14 @@ typedef struct rc_config {
                                tp_rank of tp_ranks (<= 16); kv_heads above is the PER-RANK head count.  0 / 1 = off.
                                With tp_ranks > 1 OFFLOADED / RESTORED carry arg = 0 (chains are rank-local) so that
                                every rank emits the byte-identical stream; not combinable with dedup.          */
+  uint32_t layer_major;     /* NEXT-4: 1 = layer-major streaming order.  A claim's host copy is laid out [g][block][page]
+                               (g = layer*2 + kv: all its blocks' page 0, then page 1, ...) instead of [block][g][page], a
+                               staging chunk is [g][item][page], and the copies of a chunk are issued plane by plane, so
+                               layer 0 crosses the link first.  Digests, chains, statuses, allocation and events do not
+                               change; rc_host_read returns the layer-major bytes; rc_host_store (a contiguous block) is
+                               RC_ERR_INVALID; an injected BITFLIP's param indexes the host copy in its own layout.
+                               Nothing is usable before the claim's verdict (RESTORED precedes use).  Not combinable
+                               with dedup or direct_offload.                                                       */
 } rc_config;
 
 typedef struct rc_claim_info_t {

@@ -157,6 +157,7 @@ struct Ctx {
   // NEXT-2: content-addressed host store keyed by block digest, so blocks shared between claims
   // are held (and cross the link) once.  DESIGN.md "Dedup".
   bool dedup = false;
+  bool layer_major = false;                             // NEXT-4: host copy laid out [g][block][page] (DESIGN R28)
   std::map<Key, std::pair<std::vector<u8>, u32>> store;   // (d, e) -> (blk bytes, references)
   u64 link_d2h = 0, link_h2d = 0;                          // bytes that have to cross the host link, by definition
   void emit(u64 c, u32 code, u32 aux, u64 arg) {
@@ -230,17 +231,30 @@ static void drop_host(Ctx* c, Claim& cl) {
   }
 }
 
+// Where page g of the claim's block i sits in its host copy (nb blocks).  Block-major (default): blocks one after the
+// other, each its 2L pages.  Layer-major (NEXT-4, DESIGN R28): all blocks' page 0, then all blocks' page 1, ...
+static u64 host_page_offset(const Ctx* c, u32 nb, u32 i, u32 g) {
+  return c->layer_major ? ((u64)g * nb + i) * c->page : (u64)i * c->blk + (u64)g * c->page;
+}
+// block i of a host copy as contiguous bytes, pages g = 0 .. 2L-1
+static std::vector<u8> block_of(const Ctx* c, const std::vector<u8>& host, u32 nb, u32 i) {
+  std::vector<u8> out(c->blk);
+  for (u32 g = 0; g < 2 * c->L; ++g) memcpy(out.data() + (u64)g * c->page, host.data() + host_page_offset(c, nb, i, g), c->page);
+  return out;
+}
+
 // offload: P:L343-346 (E2-E5).  Host bytes = concatenation, block-major,
-// then page g = l*2+kv.  Never failed by injection (CPU->GPU only).
+// then page g = l*2+kv (layer-major mode: see above).  Never failed by injection (CPU->GPU only).
 static void do_offload_one(Ctx* c, u64 id, Claim& cl) {
   u32 G = 2 * c->L;
   cl.host.resize((u64)cl.nb * c->blk);
   for (u32 i = 0; i < cl.nb; ++i)
     for (u32 g = 0; g < G; ++g)
-      memcpy(cl.host.data() + (u64)i * c->blk + (u64)g * c->page, c->page_ptr(g, cl.bt[i]), c->page);
+      memcpy(cl.host.data() + host_page_offset(c, cl.nb, i, g), c->page_ptr(g, cl.bt[i]), c->page);
   cl.d.resize(cl.nb); cl.e.resize(cl.nb);
   for (u32 i = 0; i < cl.nb; ++i) {
-    Dig2 x = block_digest2(cl.host.data() + (u64)i * c->blk, G, c->page);
+    std::vector<u8> blk = block_of(c, cl.host, cl.nb, i);   // the block's 2L pages, g ascending: what the digest is defined on
+    Dig2 x = block_digest2(blk.data(), G, c->page);
     cl.d[i] = x.d; cl.e[i] = x.e;
   }
   cl.chain = chain_of(id, cl.d.data(), cl.nb);
@@ -344,10 +358,11 @@ static void restore_verify(Ctx* c, u32 n, const u64* ids, int32_t* st, std::vect
       std::vector<u64> d2(cl.nb), e2(cl.nb);
       for (u32 i = 0; i < cl.nb; ++i) {
         for (u32 g = 0; g < G; ++g)
-          memcpy(c->page_ptr(g, cl.bt[i]), staged.data() + (u64)i * c->blk + (u64)g * c->page, c->page);
+          memcpy(c->page_ptr(g, cl.bt[i]), staged.data() + host_page_offset(c, cl.nb, i, g), c->page);
         u32 rem = cl.M - i * c->BS;
         c->fill[cl.bt[i]] = (u8)(rem < c->BS ? rem : c->BS);
-        Dig2 x = block_digest2(staged.data() + (u64)i * c->blk, G, c->page);
+        std::vector<u8> blk = block_of(c, staged, cl.nb, i);
+        Dig2 x = block_digest2(blk.data(), G, c->page);
         d2[i] = x.d; e2[i] = x.e;
       }
       bool found = false;
@@ -690,8 +705,13 @@ int rco_stats(void* h, u64* out4) {                     // host_used, n_claims, 
 }
 int rco_set_dedup(void* h, int on) {                    // only while no claim holds host bytes
   Ctx* c = (Ctx*)h;
-  if (c->host_used != 0) return E_INVALID;
+  if (c->host_used != 0 || (on && c->layer_major)) return E_INVALID;
   c->dedup = on != 0; return E_OK;
+}
+int rco_set_layer_major(void* h, int on) {              // only while no claim holds host bytes; not with dedup
+  Ctx* c = (Ctx*)h;
+  if (c->host_used != 0 || c->dedup) return E_INVALID;
+  c->layer_major = on != 0; return E_OK;
 }
 int rco_link_bytes(void* h, u64* out2) { Ctx* c = (Ctx*)h; out2[0] = c->link_d2h; out2[1] = c->link_h2d; return E_OK; }
 // checksum primitives, exported so the pins can reach each one directly

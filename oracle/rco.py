@@ -281,6 +281,9 @@ class Oracle:
     def set_dedup(self, on=True):
         return self.L.rco_set_dedup(self.h, int(on))
 
+    def set_layer_major(self, on=True):
+        return self.L.rco_set_layer_major(self.h, int(on))
+
     def link_bytes(self):
         o = np.zeros(2, np.uint64)
         self.L.rco_link_bytes(self.h, _p(o))

@@ -23,8 +23,6 @@
 #include <unordered_map>
 #include <unordered_set>
 #include <vector>
-#include <sys/mman.h>
-#include <thread>
 
 using namespace rck;
 
@@ -140,7 +138,7 @@ struct rc_ctx {
   cudaEvent_t ev_plan[2] = {}, ev_body_a[3] = {}, ev_body_b[3] = {};   // ev_body_*: by op index
   u64 chunk_seq[2] = {0, 0};                               // staging ring position per direction, running across operations
   std::vector<cudaEvent_t> ev_pool;
-  u8* h_store = nullptr; bool h_store_registered = false; u64 h_store_bytes = 0;
+  u8* h_store = nullptr;
   ExtAlloc host_alloc, bt_alloc, dg_alloc;
   u64 host_used = 0;
   std::unordered_map<u64, Claim> claims;
@@ -158,6 +156,7 @@ struct rc_ctx {
   std::unordered_map<Key, std::pair<u32, u32>, KeyHash> store;   // (d, e) -> (slot, references)
   u64 *h_dig = nullptr, *h_dig2 = nullptr; u32 *h_iw = nullptr, *h_ispos = nullptr, *d_iw = nullptr, *d_ispos = nullptr;
   // NEXT-4 (first half): gather straight into the mapped pinned store, no staging, no copy engine
+  bool lm = false;                                       // NEXT-4: layer-major host copy and chunk layout (rc.h)
   bool direct = false; u8* h_store_dev = nullptr; u32 *h_hpos = nullptr, *d_hpos = nullptr;
 };
 
@@ -201,21 +200,22 @@ static inline cudaError_t to_host(cudaStream_t s, void* h, const void* d, u64 by
 
 // ---- data movers -----------------------------------------------------------------------------
 template <int MODE>
-static void launch_ldg(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items, const u32* iw, const u32* ispos) {
+static void launch_ldg(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items, const u32* iw, const u32* ispos,
+                       u32 sw, u32 sg) {
   const u32 pages = n_items * c->G;
   const u32 grid = std::min(pages, c->grid);
   const u32 vpt = c->vpp / LANES;
   if (vpt % 8 == 0)
-    k_move_hash<MODE, 8><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos);
+    k_move_hash<MODE, 8><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos, sw, sg);
   else if (vpt % 4 == 0)
-    k_move_hash<MODE, 4><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos);
+    k_move_hash<MODE, 4><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos, sw, sg);
   else
-    k_move_hash<MODE, 1><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos);
+    k_move_hash<MODE, 1><<<grid, LANES, 0, s>>>((uint4*)c->pool, (uint4*)staging, phys, part, n_items, c->G, c->NB, c->vpp, iw, ispos, sw, sg);
 }
 
 // (TILE, STAGES per group, consumer groups, CTAs/SM) variants of the TMA mover; RC_TMA_VARIANT=<index> overrides the
 // default choice (tuning sweeps, profiles/r02_mover_sweep.md)
-typedef void (*tma_fn)(u8*, u8*, const u32*, u64*, u32, u32, u32, u32, const u32*, const u32*);
+typedef void (*tma_fn)(u8*, u8*, const u32*, u64*, u32, u32, u32, u32, const u32*, const u32*, u32, u32);
 struct TmaVariant { u32 tile, stages, groups, ctas_per_sm; tma_fn fn[3]; };
 #define TMA_V(T, S, NG, C) {T, S, NG, C, {k_move_hash_tma<MV_GATHER, S, T, NG>, k_move_hash_tma<MV_SCATTER, S, T, NG>, k_move_hash_tma<MV_DIGEST, S, T, NG>}}
 static const TmaVariant kTma[] = {
@@ -233,12 +233,13 @@ static inline u32 tma_block(const TmaVariant& v) { return v.groups * LANES + 64;
 
 template <int MODE>
 static void launch_move(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items,
-                        const u32* iw = nullptr, const u32* ispos = nullptr) {
+                        const u32* iw = nullptr, const u32* ispos = nullptr, bool layer_major = false) {
+  const u32 sw = layer_major ? 1u : c->G, sg = layer_major ? n_items : 1u;     // staged page of (item, g): w*sw + g*sg
   if (c->mover == RC_MOVER_TMA) {
     const TmaVariant& v = kTma[c->tma_variant[MODE]];
     const u32 grid = std::min(n_items * c->G, c->tma_grid[MODE]);
-    v.fn[MODE]<<<grid, tma_block(v), tma_smem(v), s>>>(c->pool, staging, phys, part, n_items, c->G, c->NB, (u32)c->page, iw, ispos);
-  } else launch_ldg<MODE>(c, s, staging, phys, part, n_items, iw, ispos);
+    v.fn[MODE]<<<grid, tma_block(v), tma_smem(v), s>>>(c->pool, staging, phys, part, n_items, c->G, c->NB, (u32)c->page, iw, ispos, sw, sg);
+  } else launch_ldg<MODE>(c, s, staging, phys, part, n_items, iw, ispos, sw, sg);
   c->st.kernel_launches++;
 }
 
@@ -261,8 +262,7 @@ extern "C" int rc_destroy(rc_ctx* c) {
   }
   FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_evbuf); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
   F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
-  if (c->h_store && c->h_store_registered) { cudaHostUnregister(c->h_store); munmap(c->h_store, c->h_store_bytes); }
-  else FH(c->h_store);
+  FH(c->h_store);
   for (int d = 0; d < 2; ++d) {
     for (auto p : c->staging[d]) F(p);
     for (auto p : c->part[d]) F(p);
@@ -290,6 +290,7 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   if (cfg->staging_chunk_bytes < blk || cfg->mover > RC_MOVER_TMA) return RC_ERR_INVALID;
   if (cfg->tp_ranks > TP_MAX_RANKS || (cfg->tp_ranks ? cfg->tp_rank >= cfg->tp_ranks : cfg->tp_rank != 0)) return RC_ERR_INVALID;
   if (cfg->tp_ranks > 1 && cfg->dedup) return RC_ERR_INVALID;        // the content-addressed store is not sharded
+  if (cfg->layer_major > 1 || (cfg->layer_major && (cfg->dedup || cfg->direct_offload))) return RC_ERR_INVALID;
   if ((cfg->staging_chunk_bytes / blk) * (2ull * cfg->layers) > 0x7FFFFFFFull) return RC_ERR_INVALID;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return RC_ERR_CUDA;   // no device, no library
@@ -364,6 +365,7 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   CC(cudaHostAlloc(&c->h_evbuf, c->ev_bounce_cap * sizeof(Event), cudaHostAllocMapped), RC_ERR_NOMEM);
   c->dedup = cfg->dedup != 0;
   c->direct = cfg->direct_offload != 0 && !c->dedup;
+  c->lm = cfg->layer_major != 0;
   if (c->direct) {
     CC(cudaHostAlloc(&c->h_hpos, cap * 4, cudaHostAllocMapped), RC_ERR_NOMEM);
     CC(cudaMalloc(&c->d_hpos, cap * 4), RC_ERR_NOMEM);
@@ -396,24 +398,7 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
     }
     CC(cudaEventCreateWithFlags(&c->ev_plan[d], cudaEventDisableTiming), RC_ERR_CUDA);
   }
-  if (c->host_blocks) {
-    // The pinned store.  RC_HOST_STORE=thp: anonymous memory advised to transparent huge pages, touched in parallel,
-    // then registered -- 2 MiB-contiguous physical runs for the link's address translation; default: cudaHostAlloc.
-    const char* hs = getenv("RC_HOST_STORE");
-    if (hs && !strcmp(hs, "thp")) {
-      const u64 bytes = (c->host_blocks * blk + (2ull << 20) - 1) & ~((2ull << 20) - 1);
-      void* p = mmap(nullptr, bytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0);
-      if (p == MAP_FAILED) return fail(RC_ERR_NOMEM, "mmap(host store)", cudaSuccess);
-      madvise(p, bytes, MADV_HUGEPAGE);
-      const unsigned nt = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
-      std::vector<std::thread> th;
-      for (unsigned t = 0; t < nt; ++t)
-        th.emplace_back([=]() { for (u64 o = (u64)t << 21; o < bytes; o += (u64)nt << 21) memset((u8*)p + o, 0, std::min<u64>(2ull << 20, bytes - o)); });
-      for (auto& t : th) t.join();
-      c->h_store = (u8*)p; c->h_store_bytes = bytes; c->h_store_registered = true;
-      CC(cudaHostRegister(p, bytes, cudaHostRegisterPortable | cudaHostRegisterMapped), RC_ERR_NOMEM);
-    } else CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocMapped), RC_ERR_NOMEM);
-  }
+  if (c->host_blocks) CC(cudaHostAlloc(&c->h_store, c->host_blocks * blk, cudaHostAllocMapped), RC_ERR_NOMEM);
   if (c->host_blocks && c->direct) CC(cudaHostGetDevicePointer((void**)&c->h_store_dev, c->h_store, 0), RC_ERR_CUDA);
   // launch geometry of the movers
   c->mover = cfg->mover == RC_MOVER_AUTO ? RC_MOVER_TMA : cfg->mover;
@@ -652,6 +637,49 @@ static int copy_chunk(rc_ctx* c, int dir, cudaStream_t s, u8* stg, u64 w0, u64 w
   return RC_OK;
 }
 
+// Layer-major mode (rc.h rc_config.layer_major): a claim's host copy is [g][block i][page] -- all its blocks' page 0, then
+// page 1, ... -- laid over its host-store extents in order, and a staging chunk of m items is [g][item][page].  The copies
+// of a chunk are issued plane by plane, so within a chunk the bytes cross the link in layer order.
+struct LmClaim { u64 w0; u32 nb; const std::vector<std::pair<u64, u64>>* host; };
+static int copy_chunk_lm(rc_ctx* c, int dir, cudaStream_t s, u8* stg, u64 w0, u64 w1, const std::vector<LmClaim>& cls, size_t& ci,
+                         u64& bytes) {
+  const u64 m = w1 - w0, page = c->page;
+  u8 *ha = nullptr, *da = nullptr; u64 len = 0;
+  auto flush = [&]() -> cudaError_t {
+    if (!len) return cudaSuccess;
+    cudaError_t e = dir == 0 ? cudaMemcpyAsync(ha, da, len, cudaMemcpyDeviceToHost, s)
+                             : cudaMemcpyAsync(da, ha, len, cudaMemcpyHostToDevice, s);
+    bytes += len; len = 0;
+    return e;
+  };
+  size_t last = ci;
+  for (u32 g = 0; g < c->G; ++g) {
+    for (size_t k = ci; k < cls.size() && cls[k].w0 < w1; ++k) {
+      const LmClaim& q = cls[k];
+      const u64 a = std::max(q.w0, w0), b = std::min(q.w0 + q.nb, w1);
+      if (a >= b) continue;
+      last = k;
+      u64 v = ((u64)g * q.nb + (a - q.w0)) * page, left = (b - a) * page;        // run in the claim's host copy
+      u8* d = stg + ((u64)g * m + (a - w0)) * page;
+      u64 base = 0;                                                              // virtual offset of the extent
+      for (auto& e : *q.host) {
+        const u64 eb = e.second * c->blk;
+        if (left && v < base + eb) {
+          const u64 l = std::min(left, base + eb - v);
+          u8* h = c->h_store + e.first * c->blk + (v - base);
+          if (len && h == ha + len && d == da + len) len += l;
+          else { CK(flush()); ha = h; da = d; len = l; }
+          v += l; d += l; left -= l;
+        }
+        base += eb;
+      }
+    }
+  }
+  CK(flush());
+  if (last < cls.size() && cls[last].w0 + cls[last].nb <= w1) ci = last + 1; else ci = last;   // first claim of the next chunk
+  return RC_OK;
+}
+
 extern "C" int rc_wait(rc_ctx* c, int which);
 // ---- a1-a4 offload ------------------------------------------------------------------------------------
 static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st);
@@ -693,6 +721,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   Desc* hd = c->h_desc[set];
   op.cl.assign(n, nullptr);
   std::vector<Seg> segs;
+  std::vector<LmClaim> lmc;                               // layer-major mode: served claims by work position
   std::vector<u32> served;
   bool full = false;
   u64 T = 0;
@@ -733,6 +762,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     hd[k].dg_off = cl.dg_off; hd[k].flags = D_ELIG;
     u64 w = T;
     for (auto& e : cl.host) { segs.push_back({w, e.second, e.first}); w += e.second; }
+    if (c->lm) lmc.push_back({T, cl.nb, &cl.host});
     T += cl.nb;
     st[k] = -1;
   }
@@ -748,7 +778,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   k_worklist<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[set], c->d_res[set], n, c->d_off[set], c->d_bt, nullptr, c->d_phys[oi], 0);
   CKL();
   c->st.kernel_launches += 2;
-  size_t si = 0;
+  size_t si = 0, li = 0;
   for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks) {
     const u64 w1 = std::min(T, w0 + c->chunk_blocks);
     const u32 slot = (u32)(c->chunk_seq[0]++ % c->R), m = (u32)(w1 - w0);      // the ring runs on across operations
@@ -776,7 +806,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     if (c->slot_used[0][slot]) CK(cudaStreamWaitEvent(c->gather, c->ev_free[0][slot], 0));
     cudaEvent_t t0 = get_event(c), t1 = get_event(c);
     CK(cudaEventRecord(t0, c->gather));
-    launch_move<MV_GATHER>(c, c->gather, c->staging[0][slot], c->d_phys[oi] + w0, c->part[0][slot], m);
+    launch_move<MV_GATHER>(c, c->gather, c->staging[0][slot], c->d_phys[oi] + w0, c->part[0][slot], m, nullptr, nullptr, c->lm);
     CKL();
     CK(cudaEventRecord(t1, c->gather));
     op.t_kernel.push_back({t0, t1});
@@ -788,7 +818,8 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     CK(cudaStreamWaitEvent(c->d2h, c->ev_ready[0][slot], 0));
     cudaEvent_t c0 = get_event(c), c1 = get_event(c);
     CK(cudaEventRecord(c0, c->d2h));
-    if ((rc = copy_chunk(c, 0, c->d2h, c->staging[0][slot], w0, w1, segs, si, op.copy_bytes))) return rc;
+    if ((rc = c->lm ? copy_chunk_lm(c, 0, c->d2h, c->staging[0][slot], w0, w1, lmc, li, op.copy_bytes)
+                    : copy_chunk(c, 0, c->d2h, c->staging[0][slot], w0, w1, segs, si, op.copy_bytes))) return rc;
     CK(cudaEventRecord(c1, c->d2h));
     op.t_copy.push_back({c0, c1});
     CK(cudaEventRecord(c->ev_free[0][slot], c->d2h));
@@ -936,7 +967,8 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
   CK(cudaStreamSynchronize(c->meta));                    // the grant (which claims are served) is needed to plan the copies
   std::vector<Seg> segs;
-  std::vector<std::pair<u64, u64>> flips;                // (work position, byte in block)
+  std::vector<LmClaim> lmc;
+  std::vector<std::pair<u64, u64>> flips;                // (work position, byte in block = g*page + byte in page)
   u64 T = 0;
   u32 n_served = 0;
   bool reupload = false;
@@ -958,11 +990,15 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     if (flt.kind == RC_FAULT_XFER_ERROR) { hd[k].flags |= D_XFER; reupload = true; }
     else {
       if (flt.kind == RC_FAULT_BITFLIP) {
-        const u64 pos = flt.param % ((u64)cl.nb * c->blk);
-        flips.push_back({T + pos / c->blk, pos % c->blk});
+        const u64 pos = flt.param % ((u64)cl.nb * c->blk);   // a byte of the claim's host copy, in ITS layout
+        if (c->lm) {
+          const u64 plane = (u64)cl.nb * c->page, g = pos / plane, r = pos % plane;
+          flips.push_back({T + r / c->page, g * c->page + r % c->page});
+        } else flips.push_back({T + pos / c->blk, pos % c->blk});
       }
       u64 w = T;
       for (auto& e : cl.host) { segs.push_back({w, e.second, e.first}); w += e.second; }
+      if (c->lm) lmc.push_back({T, cl.nb, &cl.host});
     }
     T += cl.nb;
   }
@@ -978,7 +1014,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   CK(cudaEventRecord(c->ev_plan[1], c->meta));
   CK(cudaStreamWaitEvent(c->scatter, c->ev_plan[1], 0));
   std::sort(flips.begin(), flips.end());
-  size_t si = 0, fi = 0;
+  size_t si = 0, fi = 0, li = 0;
   u64 flip_base = 0;
   for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks) {
     const u64 w1 = std::min(T, w0 + c->chunk_blocks);
@@ -986,14 +1022,16 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     if (c->slot_used[1][slot]) CK(cudaStreamWaitEvent(c->h2d, c->ev_free[1][slot], 0));
     cudaEvent_t c0 = get_event(c), c1 = get_event(c);
     CK(cudaEventRecord(c0, c->h2d));
-    if ((rc = copy_chunk(c, 1, c->h2d, c->staging[1][slot], w0, w1, segs, si, op.copy_bytes))) return rc;
+    if ((rc = c->lm ? copy_chunk_lm(c, 1, c->h2d, c->staging[1][slot], w0, w1, lmc, li, op.copy_bytes)
+                    : copy_chunk(c, 1, c->h2d, c->staging[1][slot], w0, w1, segs, si, op.copy_bytes))) return rc;
     CK(cudaEventRecord(c1, c->h2d));
     op.t_copy.push_back({c0, c1});
     CK(cudaEventRecord(c->ev_ready[1][slot], c->h2d));
     CK(cudaStreamWaitEvent(c->scatter, c->ev_ready[1][slot], 0));
     u32 nf = 0;
     while (fi < flips.size() && flips[fi].first < w1) {  // injected corruption of the staged copy (host bytes stay intact)
-      c->h_flip[flip_base + nf++] = (flips[fi].first - w0) * c->blk + flips[fi].second;
+      const u64 fw = flips[fi].first - w0, fb = flips[fi].second;          // item in the chunk, byte in the block
+      c->h_flip[flip_base + nf++] = c->lm ? ((fb / c->page) * m + fw) * c->page + fb % c->page : fw * c->blk + fb;
       ++fi;
     }
     if (nf) {
@@ -1005,7 +1043,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
     }
     cudaEvent_t t0 = get_event(c), t1 = get_event(c);
     CK(cudaEventRecord(t0, c->scatter));
-    launch_move<MV_SCATTER>(c, c->scatter, c->staging[1][slot], c->d_phys[1] + w0, c->part[1][slot], m);
+    launch_move<MV_SCATTER>(c, c->scatter, c->staging[1][slot], c->d_phys[1] + w0, c->part[1][slot], m, nullptr, nullptr, c->lm);
     CKL();
     CK(cudaEventRecord(t1, c->scatter));
     op.t_kernel.push_back({t0, t1});
@@ -1461,6 +1499,7 @@ extern "C" int rc_host_read(rc_ctx* c, uint64_t id, void* dst, uint64_t cap, uin
 }
 extern "C" int rc_host_store(rc_ctx* c, uint64_t id, uint32_t block, const void** p, uint64_t* contiguous_bytes) {
   GUARD();
+  if (c->lm) return RC_ERR_INVALID;                      // layer-major: a block is not contiguous in the host copy (rc_host_read)
   auto it = c->claims.find(id);
   if (it == c->claims.end() || !p || !contiguous_bytes) return RC_ERR_INVALID;
   const Claim& cl = it->second;

@@ -108,7 +108,9 @@ __device__ __forceinline__ void fold2(u64& h, u64& g, const uint4& v) {
 // vectors t, t+256, ... of the page (each warp access = 512 contiguous bytes) and folds them in
 // that order; each warp writes the sums of its 32 lane terms (both families) to part[(page*8 + warp)*2 + {0,1}]
 // -- no block barrier and no atomics in the streaming loop.  MODE 0 gather (pool -> staging), 1 scatter
-// (staging -> pool), 2 digest only (read staging).
+// (staging -> pool), 2 digest only (read staging).  The staged position of page g of item w is w*sw + g*sg pages:
+// (sw, sg) = (G, 1) is the block-major chunk [item][g][page]; (1, n_items) the layer-major chunk [g][item][page]
+// (rc_config.layer_major, NEXT-4).  Partial sums are indexed by (item, g) either way, so the digests do not change.
 // ---------------------------------------------------------------------------------------------
 enum { MV_GATHER = 0, MV_SCATTER = 1, MV_DIGEST = 2 };
 
@@ -117,7 +119,8 @@ __global__ void __launch_bounds__(LANES)
 k_move_hash(uint4* __restrict__ pool, uint4* __restrict__ staging, const u32* __restrict__ phys,
             u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 vpp,
             const u32* __restrict__ iw /*item -> work position (nullptr: identity)*/,
-            const u32* __restrict__ ispos /*item -> staged block (nullptr: identity; NEXT-2 shared staging)*/) {
+            const u32* __restrict__ ispos /*item -> staged block (nullptr: identity; NEXT-2 shared staging)*/,
+            u32 sw, u32 sg /*staged page of (item w, page g) = w*sw + g*sg: (G, 1) block-major, (1, n_items) layer-major*/) {
   const u32 t = threadIdx.x;
   const u32 n_pages = n_items * G;
   const u32 vpt = vpp / LANES;
@@ -126,7 +129,7 @@ k_move_hash(uint4* __restrict__ pool, uint4* __restrict__ staging, const u32* __
     u32 b = 0;
     if (MODE != MV_DIGEST) { b = __ldg(phys + (iw ? __ldg(iw + w) : w)); if (b == SKIP) continue; }
     uint4* pp = pool + ((u64)g * NB + b) * vpp + t;
-    uint4* sp = staging + (ispos ? ((u64)__ldg(ispos + w) * G + g) : (u64)u) * vpp + t;
+    uint4* sp = staging + (ispos ? ((u64)__ldg(ispos + w) * G + g) : ((u64)w * sw + (u64)g * sg)) * vpp + t;
     const uint4* src = (MODE == MV_GATHER) ? pp : sp;
     uint4* dst = (MODE == MV_GATHER) ? sp : pp;
     u64 h = (u64)(t + 1) * C1, gq = (u64)(t + 1) * C4;
@@ -198,7 +201,7 @@ template <int MODE, int STAGES, int TILE, int NG>
 __global__ void __launch_bounds__(NG * LANES + 64, 1)
 k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __restrict__ phys,
                 u64* __restrict__ part, u32 n_items, u32 G, u32 NB, u32 page_bytes,
-                const u32* __restrict__ iw, const u32* __restrict__ ispos) {
+                const u32* __restrict__ iw, const u32* __restrict__ ispos, u32 sw, u32 sg) {
   extern __shared__ __align__(128) u8 smem[];
   __shared__ __align__(8) u64 full[NG * STAGES];
   __shared__ __align__(8) u64 empty[NG * STAGES];
@@ -227,7 +230,7 @@ k_move_hash_tma(u8* __restrict__ pool, u8* __restrict__ staging, const u32* __re
     skip = false;
     if (MODE != MV_DIGEST) { b = __ldg(phys + (iw ? __ldg(iw + w) : w)); skip = (b == SKIP); if (skip) b = 0; }
     u8* pp = pool + ((u64)g * NB + b) * page_bytes + (u64)tile * TILE;
-    u8* sp = staging + (ispos ? ((u64)__ldg(ispos + w) * G + g) : (u64)u) * page_bytes + (u64)tile * TILE;
+    u8* sp = staging + (ispos ? ((u64)__ldg(ispos + w) * G + g) : ((u64)w * sw + (u64)g * sg)) * page_bytes + (u64)tile * TILE;
     gsrc = (MODE == MV_GATHER) ? pp : sp;
     gdst = (MODE == MV_GATHER) ? sp : pp;
   };

@@ -42,7 +42,7 @@ class Config(C.Structure):
                 ("stream_meta", C.c_void_p), ("stream_gather", C.c_void_p), ("stream_d2h", C.c_void_p),
                 ("stream_scatter", C.c_void_p), ("stream_h2d", C.c_void_p),
                 ("mover", C.c_uint32), ("grid_ctas", C.c_uint32), ("dedup", C.c_uint32), ("direct_offload", C.c_uint32),
-                ("tp_ranks", C.c_uint32), ("tp_rank", C.c_uint32)]
+                ("tp_ranks", C.c_uint32), ("tp_rank", C.c_uint32), ("layer_major", C.c_uint32)]
 
 
 class ClaimInfo(C.Structure):
@@ -110,7 +110,7 @@ class RC:
     def __init__(self, layers, kv_heads, head_dim, elem_bytes, block_size, pool_blocks, pool, fill,
                  host_store_bytes, staging_chunk_bytes=None, staging_chunks=2, max_claims=8192,
                  max_table_entries=None, max_events=1 << 17, streams=None, mover=MOVER_AUTO, grid_ctas=0, dedup=False, direct_offload=False,
-                 tp_ranks=0, tp_rank=0):
+                 tp_ranks=0, tp_rank=0, layer_major=False):
         self.L = lib()
         page = block_size * kv_heads * head_dim * elem_bytes
         self.page, self.blk, self.NB = page, 2 * layers * page, pool_blocks
@@ -122,7 +122,7 @@ class RC:
         cfg = Config(layers, kv_heads, head_dim, elem_bytes, block_size, pool_blocks, max_claims,
                      max_table_entries or max(4 * pool_blocks, 1 << 16), max_events, staging_chunks,
                      staging_chunk_bytes or min(1 << 30, max(self.blk, host_store_bytes)), host_store_bytes,
-                     pool.data_ptr(), fill.data_ptr(), s[0], s[1], s[2], s[3], s[4], mover, grid_ctas, int(dedup), int(direct_offload), tp_ranks, tp_rank)
+                     pool.data_ptr(), fill.data_ptr(), s[0], s[1], s[2], s[3], s[4], mover, grid_ctas, int(dedup), int(direct_offload), tp_ranks, tp_rank, int(layer_major))
         self.tp_ranks = max(1, tp_ranks)
         self.h = C.c_void_p()
         rc = self.L.rc_create(C.byref(cfg), C.byref(self.h))

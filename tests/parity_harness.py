@@ -14,7 +14,7 @@ from paper_2606_01387_b200 import rc, workloads as W
 
 class Pair:
     def __init__(self, wl, host_store_bytes, chunk_blocks=None, staging_chunks=2, mover=rc.MOVER_AUTO,
-                 grid_ctas=0, oracle_host_store_bytes=None, max_events=1 << 17, seed=None, dedup=False, copies=(), direct_offload=False):
+                 grid_ctas=0, oracle_host_store_bytes=None, max_events=1 << 17, seed=None, dedup=False, copies=(), direct_offload=False, layer_major=False):
         g = wl.geom
         self.wl, self.g = wl, g
         dev = torch.device("cuda:0")
@@ -32,9 +32,12 @@ class Pair:
         self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks,
                        self.pool_t, self.fill_t, host_store_bytes,
                        staging_chunk_bytes=(chunk_blocks * g.blk_bytes) if chunk_blocks else None,
-                       staging_chunks=staging_chunks, mover=mover, grid_ctas=grid_ctas, max_events=max_events, dedup=dedup, direct_offload=direct_offload)
+                       staging_chunks=staging_chunks, mover=mover, grid_ctas=grid_ctas, max_events=max_events, dedup=dedup, direct_offload=direct_offload,
+                       layer_major=layer_major)
         if dedup:
             assert self.o.set_dedup(True) == 0
+        if layer_major:
+            assert self.o.set_layer_major(True) == 0
         self.dedup = dedup
         self.view_h = self.pool_h.reshape(2 * g.layers, g.pool_blocks, g.page_bytes)
         self.view_t = self.pool_t.view(2 * g.layers, g.pool_blocks, g.page_bytes)

@@ -510,6 +510,80 @@ def test_direct_offload_into_mapped_pinned_store(mover):
     p.close()
 
 
+# ---- NEXT-4: layer-major streaming order (rc_config.layer_major; DESIGN R28) ----------------------------------------------
+@pytest.mark.parametrize("mover", [rc.MOVER_LDG, rc.MOVER_TMA])
+@pytest.mark.parametrize("kind", [W.FK_BITFLIP, W.FK_XFER_ERROR])
+@pytest.mark.parametrize("chunk_blocks", [5, 64, 300])
+def test_layer_major_tiny_full_parity(mover, kind, chunk_blocks):
+    """Host copy [g][block][page], staging chunks [g][item][page]: host bytes, digests, chains, allocation, pool bytes and
+    events against the oracle in the same mode, with chunks that cut claims (5), hold two claims (64) or the whole wave."""
+    wl = W.make_workload(0)
+    p = Pair(wl, 1 << 30, chunk_blocks=chunk_blocks, mover=mover, layer_major=True)
+    wave = W.plan_waves(wl, 1 << 30)[0]
+    faults = [(cid, kind, prm) for cid, _, prm in wave.faults]
+    ev, st_r = p.run_wave(wave, faults=faults)
+    assert V.validate(ev)[0]
+    assert names(ev, wl.claims[3].claim_id) == GOLD["failure_path"] and st_r[3] == rc.ST_RESTORE_FAILED
+    assert p.r.host_store(wl.claims[0].claim_id, 0) is None          # no contiguous block in this layout
+    p.close()
+
+
+def test_layer_major_fragmented_host_store_and_interleaved_waves():
+    """Claims whose host copy is split over several extents of the store (the plane runs straddle the pieces), bit flips
+    on both sides of plane and chunk boundaries, restore(k) in flight with two offloads open."""
+    wl = W.make_workload(4, n_claims=24, pool_blocks=3072, scale=64)
+    host = 3 << 30
+    p = Pair(wl, host, chunk_blocks=64, layer_major=True)
+    o, r = p.o, p.r
+    waves = W.plan_waves(wl, host, max_claims_per_wave=8)
+    blk, page = wl.geom.blk_bytes, wl.geom.page_bytes
+
+    def admit(wave):
+        cl = [wl.claims[k] for k in wave.claim_idx]
+        ids = [c.claim_id for c in cl]
+        used, _ = o.pool_state()
+        free = np.nonzero(used == 0)[0].astype(np.uint32)
+        remap = np.zeros(wl.geom.pool_blocks, np.uint32)
+        remap[wave.used_ids] = free[: wave.used_ids.size]
+        p.set_fill(remap[wave.fill_ids], wave.fill_val)
+        assert o.mark_used(remap[wave.used_ids]) == 0 and r.mark_used(remap[wave.used_ids]) == 0
+        args = (ids, [c.P for c in cl], [c.N for c in cl], wave.bt_off, remap[wave.bt_ids])
+        assert np.array_equal(o.accept(*args), r.accept(*args))
+        assert np.array_equal(o.materialize(ids), r.materialize(ids))
+        return ids
+
+    # fragment the host store: offload wave 0 claim by claim, release every second claim
+    ids0 = admit(waves[0])
+    for c in ids0:
+        assert np.array_equal(o.offload([c]), r.offload([c]))
+    assert np.array_equal(o.release(ids0[::2]), r.release(ids0[::2]))
+    ids1 = admit(waves[1])
+    assert np.array_equal(o.offload(ids1), r.offload(ids1))            # lands in the holes: split extents
+    p.check_claims(ids1, "offload into a fragmented store", host=True)
+    nb, nb2 = r.claim_info(ids1[0])["nb"], r.claim_info(ids1[2])["nb"]
+    flips = [(ids1[0], rc.FAULT_BITFLIP, 2 * nb * page - 1), (ids1[1], rc.FAULT_BITFLIP, 0),
+             (ids1[2], rc.FAULT_BITFLIP, nb2 * blk - 1)]
+    p.poison_free()
+    assert o.set_faults(flips) == 0 and r.set_faults(flips) == 0
+    ids2 = admit(waves[2])
+    o.restore_begin(ids1)
+    r.restore_begin(ids1)
+    r.offload_begin(ids2[:4])
+    r.offload_begin(ids2[4:])
+    sa = [o.offload(ids2[:4]), o.offload(ids2[4:])]
+    assert np.array_equal(sa[0], r.wait(0)) and np.array_equal(sa[1], r.wait(0))
+    sa_r, sb_r = o.restore_end(), r.wait(1)
+    assert np.array_equal(sa_r, sb_r) and list(sb_r[:3]) == [8, 8, 8]
+    p.check_claims(ids1 + ids2, "interleaved", host=False)
+    p.check_claims(ids2, "offloaded", host=True)
+    p.check_pool_state("interleaved", bytes_too=True)
+    ev = p.check_events("layer-major")
+    assert V.validate(ev)[0]
+    bad = [int(e["aux"]) for e in ev if int(e["code"]) == 5]
+    assert bad == [nb - 1, 0, nb2 - 1]            # the block that the layer-major layout puts at each flipped byte
+    p.close()
+
+
 def test_large_batch_multi_tile_scans():
     """3000 claims in one batch on a 98304-block pool: every single-CTA scan (offsets, restore plan, allocation,
     event emission) runs over several tiles with carries; sub-batched restores hit NO_FREE_BLOCKS prefixes."""
