@@ -79,6 +79,49 @@ def host_ram_bytes():
         return 64 << 30
 
 
+def run_pipeline(r, seq, admit, n_distinct, one_open, ev_cap):
+    """The pipelined schedule over a sequence of pre-marshalled waves (dicts with "ids" and "faults"); `admit(p)` makes wave
+    p resident (fill, mark_used, accept, materialize).  While wave j is restored, waves j+1 and j+2 are offloaded back to
+    back (two open offloads, rc.h).  Between the end of restore(j-1) and the first H2D copy of restore(j) stand only:
+    rc_wait(0) -- offload(j) takes effect: reference drop, OFFLOADED --, the release of wave j-1 and rc_restore_begin (plan).
+    Everything else -- draining the records, admitting wave j+2 (its pool region is the one offload(j) has just left) and
+    queueing offload(j+2) behind offload(j+1) -- runs while both directions move data: the metadata stream is idle until
+    rc_wait(1) enqueues the restore's verdicts.  Returns the number of records drained.
+    `ahead` = how many waves may be admitted beyond the one being restored: wave j+2 of a two-wave workload (j+1 of a
+    one-wave workload) carries the claim ids of wave j and can only be admitted after its release; dedup / direct_offload
+    allow one open offload."""
+    ahead = min(1 if one_open else 2, n_distinct - 1)
+    adm = n_ev = 0
+
+    def push():
+        nonlocal adm
+        admit(seq[adm])
+        r.offload_begin(seq[adm]["ids"])
+        adm += 1
+    for _ in range(min(len(seq), max(1, ahead))):
+        push()
+    for j, p in enumerate(seq):
+        r.wait(0)
+        if j > 0 and ahead >= 1:
+            r.release(seq[j - 1]["ids"])
+        r.set_faults(p["faults"])
+        r.restore_begin(p["ids"])
+        if j > 0 and ahead >= 1:
+            n_ev += len(r.outcomes(cap=ev_cap))
+        if ahead >= 1 and adm < len(seq):
+            push()
+        r.wait(1)
+        if ahead == 0:
+            n_ev += len(r.outcomes(cap=ev_cap))
+            r.release(p["ids"])
+            if adm < len(seq):
+                push()
+    if ahead >= 1 and seq:
+        n_ev += len(r.outcomes(cap=ev_cap))
+        r.release(seq[-1]["ids"])
+    return n_ev
+
+
 class Job:
     """One rank's workload: context, resident pool, pre-marshalled waves."""
 
@@ -188,43 +231,7 @@ class Job:
             for _ in range(n_steps):
                 seq += self.prep if len(seq) % 2 == 0 else self.prep_alt
             nmax = max(p["n"] for p in self.prep)
-            # how many waves may be admitted ahead of the wave being restored: wave j+2 of a two-wave workload (j+1 of a
-            # one-wave workload) carries the claim ids of wave j and can only be admitted after its release
-            ahead = min(1 if self.one_open else 2, len(self.prep) - 1)   # dedup / direct_offload: one open offload (rc.h)
-            adm = 0
-
-            def push():
-                nonlocal adm
-                self._admit(seq[adm], e2e)
-                r.offload_begin(seq[adm]["ids"])
-                adm += 1
-            for _ in range(min(len(seq), max(1, ahead))):
-                push()
-            for j, p in enumerate(seq):
-                # On entry offload(j) and, behind it on the D2H side, offload(j+1) are open and restore(j-1) has just
-                # completed.  Between that moment and the first H2D copy of restore(j) stand only: rc_wait(0) -- offload(j)
-                # takes effect: reference drop, OFFLOADED --, the release of wave j-1 and rc_restore_begin (plan).
-                # Everything else -- draining the records, admitting wave j+2 (its pool region is the one offload(j) has
-                # just left) and queueing offload(j+2) behind offload(j+1) -- runs while both directions move data: the
-                # metadata stream is idle until rc_wait(1) enqueues the restore's verdicts.
-                r.wait(0)
-                if j > 0:
-                    r.release(seq[j - 1]["ids"])
-                r.set_faults(p["faults"])
-                r.restore_begin(p["ids"])
-                if j > 0:
-                    n_ev += len(r.outcomes(cap=32 * nmax))
-                if ahead >= 1 and adm < len(seq):
-                    push()
-                r.wait(1)
-                if ahead == 0:
-                    n_ev += len(r.outcomes(cap=32 * nmax))
-                    r.release(p["ids"])
-                    if adm < len(seq):
-                        push()
-            if ahead >= 1:
-                n_ev += len(r.outcomes(cap=32 * nmax))
-                r.release(seq[-1]["ids"])
+            n_ev = run_pipeline(r, seq, lambda p: self._admit(p, e2e), len(self.prep), self.one_open, 32 * nmax)
         self.events = n_ev // max(1, n_steps)
         return n_ev
 

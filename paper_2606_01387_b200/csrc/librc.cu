@@ -102,7 +102,6 @@ struct Op {
   std::vector<u32> new_bt;                // restore: new table extent offset per entry
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> t_kernel, t_copy;
   u64 blocks = 0, copy_bytes = 0, launches = 0;
-  cudaEvent_t done = nullptr;
   // restore: the reuse request it belongs to (0: per-claim refusals), TP split form, verdict kernels already enqueued
   u64 request_id = 0; bool tp = false, tail = false;
 };
@@ -258,7 +257,6 @@ extern "C" int rc_destroy(rc_ctx* c) {
     F(c->d_phys[i]); F(c->d_dtmp[i]); F(c->d_etmp[i]);
     if (c->ev_body_a[i]) cudaEventDestroy(c->ev_body_a[i]);
     if (c->ev_body_b[i]) cudaEventDestroy(c->ev_body_b[i]);
-    if (c->ops[i].done) cudaEventDestroy(c->ops[i].done);
   }
   FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_evbuf); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
   F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
@@ -384,7 +382,6 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
     CC(cudaMalloc(&c->d_etmp[i], cap * 8), RC_ERR_NOMEM);
     CC(cudaEventCreateWithFlags(&c->ev_body_a[i], cudaEventDisableTiming), RC_ERR_CUDA);
     CC(cudaEventCreateWithFlags(&c->ev_body_b[i], cudaEventDisableTiming), RC_ERR_CUDA);
-    CC(cudaEventCreateWithFlags(&c->ops[i].done, cudaEventDisableTiming), RC_ERR_CUDA);
   }
   for (int d = 0; d < 2; ++d) {
     c->staging[d].assign(c->R, nullptr); c->part[d].assign(c->R, nullptr);
@@ -770,8 +767,8 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   for (auto& od : old_dg) if (od.second) c->dg_alloc.release(od.first, od.second);
   op.n = n; op.status = st; op.blocks = T; op.copy_bytes = 0; op.launches = 0;
   int rc;
-  // The head (offsets, compaction) only reads tables that completed calls wrote, so it runs on the gather
-  // stream: an offload begun after a restore does not queue behind that restore's tail on `meta`.
+  // The head (offsets, compaction) only reads tables that completed calls wrote, so it runs on the gather stream;
+  // nothing of an offload touches `meta` before rc_wait(0).
   CK(to_dev(c->gather, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
   k_offsets<<<1, 1024, 0, c->gather>>>(c->d_desc[set], n, c->d_off[set]);
   CKL();
