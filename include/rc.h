@@ -186,7 +186,9 @@ int rc_restore(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* statu
  * and further _begin calls do not wait for the transfers.  Metadata steps execute in call order on one stream, so
  * every observable (statuses, allocation, events, seq numbers) equals the synchronous calls made in this order: an
  * offload at its rc_wait(0); a restore's plan at its _begin and its outcome at its rc_wait(1) (the oracle's
- * rco_restore_begin / rco_restore_end).  The claims of an operation in flight answer BAD_STATE to every other call.
+ * rco_restore_begin / rco_restore_end).  One decision of an offload is taken earlier than that: its host-space grant
+ * (NO_HOST_SPACE) is evaluated at _begin, against the space held then -- never less strict than at its rc_wait(0).
+ * The claims of an operation in flight answer BAD_STATE to every other call.
  * rc_test: *done = 1 if rc_wait(ctx, which) would not have to wait for data movement (the oldest open offload's gather
  * and D2H have finished / the restore's H2D and scatter have finished / nothing is in flight), else 0.  Never blocks. */
 int rc_offload_begin(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* status);

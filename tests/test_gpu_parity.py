@@ -730,3 +730,132 @@ def test_call_level_errors_change_nothing():
     assert list(r.offload(ids[:1])) == [0]                                                  # one claim still fits
     assert np.array_equal(r.host_read(ids[0]), hb)
     r.close()
+
+
+# ---- split forms under random interleavings -------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_split_forms_random_interleavings(seed):
+    """Random legal sequences of admit / rc_offload_begin (up to two open) / rc_wait(0) / rc_restore_begin / rc_wait(1) /
+    rc_release / poison, with other claims' metadata calls between a _begin and its rc_wait.  The oracle makes the calls rc.h
+    says they are equal to: an offload at its rc_wait(0), a restore as rco_restore_begin at its _begin and rco_restore_end at
+    its rc_wait(1).  Statuses, claim records, digests, host bytes, allocation and -- whenever nothing is in flight -- pool
+    bytes are compared on the way, the whole event stream at the end.  The pool is small enough for NO_FREE_BLOCKS to occur;
+    the host store is ample (an offload's host-space grant is taken at _begin: rc.h)."""
+    rng = np.random.default_rng(1000 + seed)
+    wl = W.make_workload(0, n_claims=48, pool_blocks=700)
+    g = wl.geom
+    p = Pair(wl, 1 << 30, chunk_blocks=41)
+    o, r = p.o, p.r
+    todo = list(range(len(wl.claims)))
+    resident, offloaded, back = [], [], []                     # claim ids by where they are (idle claims only)
+    open_q, in_restore = [], None
+    n_busy_status = n_nofree = 0
+
+    def admit(k):
+        c = wl.claims[k]
+        nt = -(-c.P // g.block_size)
+        used, _ = o.pool_state()
+        free = np.nonzero(used == 0)[0].astype(np.uint32)
+        if free.size < nt + 40:
+            return False
+        tab = rng.choice(free[free.size // 2:] if free.size // 2 >= nt else free, nt, replace=False).astype(np.uint32)
+        fv = np.array([min(g.block_size, max(0, c.M - i * g.block_size)) for i in range(nt)], np.uint8)
+        p.set_fill(tab, fv)
+        assert o.mark_used(tab) == 0 and r.mark_used(tab) == 0
+        args = ([c.claim_id], [c.P], [c.N], [0, nt], tab)
+        assert np.array_equal(o.accept(*args), r.accept(*args))
+        sa, sb = o.materialize([c.claim_id]), r.materialize([c.claim_id])
+        assert np.array_equal(sa, sb)
+        if sa[0] == 0:
+            resident.append(c.claim_id)
+        else:                                                  # PRED_FALSE: give the blocks back
+            assert np.array_equal(o.release([c.claim_id]), r.release([c.claim_id]))
+            assert o.mark_free(tab) == 0 and r.mark_free(tab) == 0
+        return True
+
+    def pick(lst, lo=1, hi=6):
+        n = int(rng.integers(lo, min(hi, len(lst)) + 1))
+        ids = [lst.pop(int(rng.integers(0, len(lst)))) for _ in range(n)]
+        return ids
+
+    for step in range(260):
+        acts = []
+        if todo:
+            acts.append("admit")
+        if resident and len(open_q) < 2:
+            acts += ["obegin"] * 2
+        if open_q:
+            acts += ["owait"] * 2
+        if offloaded and in_restore is None:
+            acts += ["rbegin"] * 2
+        if in_restore is not None:
+            acts.append("rwait")
+        if back:
+            acts.append("release")
+        acts.append("poison")
+        a = acts[int(rng.integers(0, len(acts)))]
+        if a == "admit":
+            if not admit(todo[0]):
+                continue
+            todo.pop(0)
+        elif a == "obegin":
+            ids = pick(resident)
+            extra = []
+            if open_q and rng.random() < 0.3:                  # a claim of an open offload answers BAD_STATE, no effect
+                extra = [open_q[0][0][0]]
+            st = r.offload_begin(ids + extra)
+            if extra:
+                assert st[-1] == rc.ST_BAD_STATE
+                n_busy_status += 1
+            open_q.append((ids, extra))
+        elif a == "owait":
+            ids, extra = open_q.pop(0)
+            sb = r.wait(0)
+            sa = o.offload(ids)
+            assert np.array_equal(sa, sb[: len(ids)]) and not sa.any()
+            p.check_claims(ids, "offload at rc_wait(0)", host=True)
+            offloaded += ids
+        elif a == "rbegin":
+            ids = pick(offloaded)
+            fl = []
+            for c in ids:
+                u = rng.random()
+                if u < 0.15:
+                    fl.append((c, rc.FAULT_BITFLIP, int(rng.integers(0, 1 << 31))))
+                elif u < 0.25:
+                    fl.append((c, rc.FAULT_XFER_ERROR, 0))
+            assert o.set_faults(fl) == 0 and r.set_faults(fl) == 0
+            sa, sb = o.restore_begin(ids), r.restore_begin(ids)
+            assert np.array_equal(sa, sb), (sa, sb)            # -1 for served claims, final for the others (NO_FREE_BLOCKS)
+            in_restore = ids
+        elif a == "rwait":
+            sa, sb = o.restore_end(), r.wait(1)
+            assert np.array_equal(sa, sb), (sa, sb)
+            p.check_claims(in_restore, "restore at rc_wait(1)")
+            for c, s in zip(in_restore, sa):
+                if s == 0:
+                    back.append(c)
+                elif s == rc.ST_NO_FREE_BLOCKS:
+                    offloaded.append(c)
+                    n_nofree += 1
+            in_restore = None
+        elif a == "release":
+            ids = pick(back, 1, 4)
+            assert np.array_equal(o.release(ids), r.release(ids))
+        else:
+            p.poison_free()
+        if not open_q and in_restore is None and step % 7 == 0:
+            p.check_pool_state("step %d" % step, bytes_too=True)
+    while open_q:
+        ids, extra = open_q.pop(0)
+        assert np.array_equal(o.offload(ids), r.wait(0)[: len(ids)])
+    if in_restore is not None:
+        assert np.array_equal(o.restore_end(), r.wait(1))
+    p.check_pool_state("end", bytes_too=True)
+    ev = p.check_events("random interleavings")
+    ok, why = V.validate(ev)
+    assert ok, why
+    assert len(ev) > 150
+    s = r.stats()
+    assert o.link_bytes() == (s["bytes_d2h"], s["bytes_h2d"]) and o.stats()["host_used"] == s["host_used_bytes"]
+    p.close()
