@@ -683,6 +683,22 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
 static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_t* st);
 static void dedup_drop(rc_ctx* c, Claim& cl);
 
+// Chunk boundaries of an operation over T work positions: chunks of chunk_blocks items.  A restore cuts its LAST chunk
+// in two: the scatter of the final piece is the one mover launch that no H2D copy hides (the link idles while it runs),
+// so that piece is a quarter chunk -- 0.15 ms of scatter instead of 0.6 ms per operation, +1 % on a step of 2 GiB
+// waves.  Not smaller: a launch of a sixteenth chunk runs at 0.6 of the rate of a full one (measured: scatter 0.926
+// overall instead of 0.987).  An offload is not cut: its first gather delays a direction that runs ahead anyway.
+static std::vector<std::pair<u64, u64>> plan_chunks(const rc_ctx* c, u64 T, bool short_last) {
+  std::vector<std::pair<u64, u64>> ch;
+  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks) ch.push_back({w0, std::min(T, w0 + c->chunk_blocks)});
+  const u64 tail = std::max<u64>(1, c->chunk_blocks / 4);
+  if (short_last && !ch.empty()) {
+    auto l = ch.back();
+    if (l.second - l.first > 2 * tail) { ch.back().second = l.second - tail; ch.push_back({l.second - tail, l.second}); }
+  }
+  return ch;
+}
+
 // ---- offload slots ------------------------------------------------------------------------------------
 // Up to OFF_DEPTH offloads may be open (begun, not yet completed by rc_wait(0)); they run back to back on the gather
 // and d2h streams.  _begin enqueues a1-a3 and the chain; the a4 bookkeeping -- reference drop, OFFLOADED -- is enqueued
@@ -776,8 +792,8 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   CKL();
   c->st.kernel_launches += 2;
   size_t si = 0, li = 0;
-  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks) {
-    const u64 w1 = std::min(T, w0 + c->chunk_blocks);
+  for (const auto& ch : plan_chunks(c, T, false)) {
+    const u64 w0 = ch.first, w1 = ch.second;
     const u32 slot = (u32)(c->chunk_seq[0]++ % c->R), m = (u32)(w1 - w0);      // the ring runs on across operations
     if (c->direct) {
       // the mover's destination is the claim's place in the mapped pinned store: the bulk stores of the gather
@@ -1013,8 +1029,8 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   std::sort(flips.begin(), flips.end());
   size_t si = 0, fi = 0, li = 0;
   u64 flip_base = 0;
-  for (u64 w0 = 0; w0 < T; w0 += c->chunk_blocks) {
-    const u64 w1 = std::min(T, w0 + c->chunk_blocks);
+  for (const auto& ch : plan_chunks(c, T, true)) {
+    const u64 w0 = ch.first, w1 = ch.second;
     const u32 slot = (u32)(c->chunk_seq[1]++ % c->R), m = (u32)(w1 - w0);
     if (c->slot_used[1][slot]) CK(cudaStreamWaitEvent(c->h2d, c->ev_free[1][slot], 0));
     cudaEvent_t c0 = get_event(c), c1 = get_event(c);
