@@ -19,9 +19,10 @@
 //   P:L384     path C: only the target claim is attributed.
 //   P:L199     ambiguity fails closed: an error status emits no event.
 // Everything the paper leaves open (byte layout, checksum, allocator, codes) is
-// build-defined: DESIGN.md "Readings" R1..R21.  Pins: tests/test_oracle_*.py.
-// Parity unpinned (beyond GPU==oracle): status-code numbering, aux/arg payload
-// choice, one-shot fault consumption, NO_FREE_BLOCKS / NO_HOST_SPACE policy.
+// build-defined: DESIGN.md "Readings" R1..R28.  Pins: tests/test_oracle_*.py.
+// Parity unpinned (beyond GPU==oracle): status- and event-code numbering, aux/arg
+// payload choice, one-shot fault consumption (R18), the NO_FREE_BLOCKS /
+// NO_HOST_SPACE refusal policy (R7, R26), the victim order inside a group (R23).
 #include <cstdint>
 #include <cstring>
 #include <cstdlib>
