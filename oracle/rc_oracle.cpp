@@ -134,6 +134,7 @@ struct Claim {
   u64 chain = 0;
   std::vector<u8> host;       // claim-scoped host copy (nb*blk bytes)
   std::vector<Key> hkeys;     // dedup mode (NEXT-2): the claim's blocks as keys into the content-addressed store
+  bool in_flight = false;     // split form: between rco_restore_begin and rco_restore_end the claim answers BAD_STATE (rc.h)
 };
 
 struct Verdict { u32 flags, bad; };                     // flags: 1 = served, 2 = locally ok; bad = first bad block / 0xFFFFFFFF
@@ -325,7 +326,7 @@ static void restore_verify(Ctx* c, u32 n, const u64* ids, int32_t* st, std::vect
     Claim& cl = it->second;
     bool dup = false;
     for (u32 j = 0; j < k; ++j) if (served[j] == &cl) dup = true;
-    if (cl.state != CS_OFFLOADED || dup) { st[k] = ST_BAD_STATE; continue; }
+    if (cl.state != CS_OFFLOADED || dup || cl.in_flight) { st[k] = ST_BAD_STATE; continue; }
     if (full || need + cl.nb > nfree) { full = true; st[k] = ST_NO_FREE_BLOCKS; continue; }
     need += cl.nb; served[k] = &cl; st[k] = ST_OK;
   }
@@ -601,7 +602,7 @@ int rco_restore_begin(void* h, u64 request_id, u32 n, const u64* id, int32_t* st
   if (c->tp_pending) return E_INVALID;
   std::vector<Claim*> served;
   restore_verify(c, n, id, st, served, c->split_v);
-  for (u32 k = 0; k < n; ++k) if (served[k]) st[k] = -1;      // pending: decided by _end
+  for (u32 k = 0; k < n; ++k) if (served[k]) { st[k] = -1; served[k]->in_flight = true; }   // pending: decided by _end
   c->tp_ids.assign(id, id + n);
   c->tp_served.assign(served.begin(), served.end());
   c->split_request = request_id;
@@ -613,7 +614,7 @@ int rco_restore_end(void* h, int32_t* st) {
   if (!c->tp_pending) return E_INVALID;
   const u32 n = (u32)c->tp_ids.size();
   std::vector<Claim*> served(n);
-  for (u32 k = 0; k < n; ++k) served[k] = (Claim*)c->tp_served[k];
+  for (u32 k = 0; k < n; ++k) { served[k] = (Claim*)c->tp_served[k]; if (served[k]) served[k]->in_flight = false; }
   restore_commit(c, n, c->tp_ids.data(), st, served, c->split_v, c->split_request);
   c->tp_pending = false;
   return E_OK;
@@ -643,6 +644,7 @@ int rco_release(void* h, u32 n, const u64* id, int32_t* st) {
   for (u32 k = 0; k < n; ++k) {
     auto it = c->claims.find(id[k]);
     if (it == c->claims.end()) { st[k] = ST_UNKNOWN_CLAIM; continue; }
+    if (it->second.in_flight) { st[k] = ST_BAD_STATE; continue; }   // a claim of a restore in flight (rc.h)
     drop_refs(c, it->second);
     drop_host(c, it->second);
     c->claims.erase(it); st[k] = ST_OK;

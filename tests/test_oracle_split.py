@@ -66,6 +66,7 @@ def test_calls_between_begin_and_end():
     assert o.stats()["host_used"] == host_before                            # the host copy is held until _end
     assert all(o.claim_info(c)["state"] == 3 for c in a)                    # still OFFLOADED: no record yet
     assert not o.offload(b).any()                                           # another call in between
+    assert o.release(a[:1]).tolist() == [3] and o.restore(a[:1]).tolist() == [3]   # a claim in flight answers BAD_STATE (rc.h)
     st = o.restore_end()
     assert [int(s) for s in st] == [0, 8, 0]
     ev = o.outcomes()
