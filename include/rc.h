@@ -139,6 +139,11 @@ int rc_destroy(rc_ctx* ctx);
 /* Allocator hand-over: blocks the caller already filled become "used" (ref 0), or go back
  * to free if no claim references them (claimed blocks are left alone). */
 int rc_mark_used(rc_ctx* ctx, uint32_t n, const uint32_t* block_ids);
+/* Convenience for callers that keep the materialization marks on the host: fill_dev[block_ids[i]] = values[i] (HOST
+ * arrays; values <= block_size, ids < pool_blocks, else RC_ERR_INVALID and nothing is written).  The bytes cross PCIe in
+ * the library's small-transfer path, not through a copy engine, so the call does not wait behind chunk copies in
+ * flight.  Complete on return.  Writing fill_dev directly (it is caller-owned device memory) is equivalent. */
+int rc_set_fill(rc_ctx* ctx, uint32_t n, const uint32_t* block_ids, const uint8_t* values);
 int rc_mark_free(rc_ctx* ctx, uint32_t n, const uint32_t* block_ids);
 
 /* a0. Records (C, P, N, block table) before any lifecycle event.  Table k is

@@ -465,6 +465,25 @@ static int mark(rc_ctx* c, u32 n, const u32* ids, int val) {
   }
   return RC_OK;
 }
+// fill_dev[ids[i]] = vals[i] from HOST arrays, through the small-transfer path (no copy engine: an admission made while
+// chunk copies are in flight does not wait behind them).  Ids are packed in front of the values in the upload buffer.
+extern "C" int rc_set_fill(rc_ctx* c, uint32_t n, const uint32_t* ids, const uint8_t* vals) {
+  GUARD();
+  if (n && (!ids || !vals)) return RC_ERR_INVALID;
+  for (u32 i = 0; i < n; ++i) if (ids[i] >= c->NB || vals[i] > c->cfg.block_size) return RC_ERR_INVALID;
+  const u32 per = (u32)std::min<u64>(c->cap_entries * 4 / 5, 1u << 30);          // 4 B id + 1 B value per entry
+  for (u32 s = 0; s < n; s += per) {
+    const u32 m = std::min(per, n - s), vb = (m + 3) & ~3u;
+    memcpy(c->h_up, ids + s, (u64)m * 4);
+    memcpy((u8*)(c->h_up + m), vals + s, m);
+    CK(to_dev(c->meta, c->d_up, c->h_up, (u64)m * 4 + vb));
+    k_fill_write<<<(m + 255) / 256, 256, 0, c->meta>>>(c->d_up, (const u8*)(c->d_up + m), m, c->fill);
+    CKL();
+    c->st.kernel_launches++;
+    CK(cudaStreamSynchronize(c->meta));
+  }
+  return RC_OK;
+}
 extern "C" int rc_mark_used(rc_ctx* c, uint32_t n, const uint32_t* ids) { return mark(c, n, ids, 1); }
 extern "C" int rc_mark_free(rc_ctx* c, uint32_t n, const uint32_t* ids) { return mark(c, n, ids, 0); }
 

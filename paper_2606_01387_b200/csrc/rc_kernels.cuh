@@ -783,6 +783,12 @@ __global__ void k_copy_words(u32* __restrict__ dst, const u32* __restrict__ src,
   for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (u64)gridDim.x * blockDim.x) dst[i] = src[i];
 }
 
+// rc_set_fill: fill[ids[i]] = vals[i] (the caller's materialization marks, sent as host arrays)
+__global__ void k_fill_write(const u32* __restrict__ ids, const u8* __restrict__ vals, u32 n, u8* __restrict__ fill) {
+  const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) fill[ids[i]] = vals[i];
+}
+
 // fault injection (CPU->GPU transfers only): flip bit 0 of the listed staged bytes
 __global__ void k_bitflip(u8* staging, const u64* __restrict__ offs, u32 n) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;

@@ -24,7 +24,7 @@ MOVER_AUTO, MOVER_LDG, MOVER_TMA = 0, 1, 2
 REQ_FLAG = 0x80000000
 POLICY_REFUSE, POLICY_DEMOTE, POLICY_EXPIRE = 0, 1, 2
 
-EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_accept", "rc_materialize", "rc_offload",
+EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_set_fill", "rc_accept", "rc_materialize", "rc_offload",
            "rc_restore", "rc_offload_begin", "rc_restore_begin", "rc_wait", "rc_test", "rc_set_policy", "rc_restore_request",
            "rc_restore_request_begin", "rc_tp_restore_verify", "rc_tp_restore_commit", "rc_tp_mailbox", "rc_tp_set_peer",
            "rc_tp_ipc_handle", "rc_tp_open_peer", "rc_protect", "rc_make_room", "rc_protected_map", "rc_outcomes", "rc_set_faults",
@@ -147,6 +147,11 @@ class RC:
     def mark_used(self, ids):
         ids = _u32(ids)
         return self.L.rc_mark_used(self.h, ids.size, _p(ids))
+
+    def set_fill(self, ids, vals):
+        ids, vals = _u32(ids), np.ascontiguousarray(vals, dtype=np.uint8)
+        assert ids.size == vals.size
+        self._ck(self.L.rc_set_fill(self.h, ids.size, _p(ids), _p(vals)), "rc_set_fill")
 
     def mark_free(self, ids):
         ids = _u32(ids)

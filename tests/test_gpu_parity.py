@@ -859,3 +859,23 @@ def test_split_forms_random_interleavings(seed):
     s = r.stats()
     assert o.link_bytes() == (s["bytes_d2h"], s["bytes_h2d"]) and o.stats()["host_used"] == s["host_used_bytes"]
     p.close()
+
+
+def test_set_fill_from_host_arrays():
+    """rc_set_fill writes exactly the named entries of the caller's fill vector and refuses bad input without writing."""
+    wl = W.make_workload(0)
+    p = Pair(wl, 1 << 30)
+    rng = np.random.default_rng(3)
+    ids = rng.choice(wl.geom.pool_blocks, 100, replace=False).astype(np.uint32)
+    vals = rng.integers(0, wl.geom.block_size + 1, 100).astype(np.uint8)
+    want = p.fill_t.cpu().numpy().copy()
+    want[ids] = vals
+    p.r.set_fill(ids, vals)
+    assert np.array_equal(p.fill_t.cpu().numpy(), want)
+    for bad_ids, bad_vals in ((np.array([wl.geom.pool_blocks], np.uint32), np.array([1], np.uint8)),
+                              (np.array([0], np.uint32), np.array([wl.geom.block_size + 1], np.uint8))):
+        with pytest.raises(rc.RcError):
+            p.r.set_fill(bad_ids, bad_vals)
+    assert np.array_equal(p.fill_t.cpu().numpy(), want)
+    p.r.set_fill(np.zeros(0, np.uint32), np.zeros(0, np.uint8))
+    p.close()
