@@ -486,10 +486,14 @@ def main():
     if roofline:
         roofline["kernel"] = "k_move_hash%s<GATHER> (K2 gather+checksum)" % ("_tma" if mover != rc.MOVER_LDG else "")
         roofline["traffic_source"] = traffic_source
+        roofline["note"] = ("measured inside the pipelined step, both copy engines active; the same kernel alone on the device: "
+                            "0.97-0.99 by CUDA events, 1.01-1.03 by ncu (profiles/r02_mover_sweep.md, r02_prof_c1.md, r02_instep_trace.md)")
     roof_sc = roof(st["ms_scatter"], st["scatter_launches"], st["scatter_blocks"])
     if roof_sc:
         roof_sc["kernel"] = "k_move_hash%s<SCATTER> (K4 scatter+checksum)" % ("_tma" if mover != rc.MOVER_LDG else "")
         roof_sc["traffic"] = None
+        roof_sc["note"] = ("measured inside the pipelined step; since the restore's last chunk is cut the main scatter runs beside "
+                           "both copy engines (DESIGN.md 6); alone on the device: 0.99-1.00")
     roof_dg = None
     if world == 1:             # M3: the checksum alone, read-only pass over one staging-sized buffer (algorithmic bytes = blk per block)
         nblk = int(min(a.chunk_mib << 20, job.host_store) // blk)
