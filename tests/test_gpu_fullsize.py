@@ -120,7 +120,7 @@ def _need(dev_bytes, host_bytes):
 
 
 class FullSize:
-    def __init__(self, index, wave_frac, host_bytes, max_claims_per_wave=None, dedup=False, n_waves=3):
+    def __init__(self, index, wave_frac, host_bytes, max_claims_per_wave=None, dedup=False, n_waves=3, layer_major=False):
         self.wl = wl = W.make_workload(index)
         self.g = g = wl.geom
         _need(g.pool_bytes + (14 << 30), host_bytes + (12 << 30))
@@ -135,7 +135,9 @@ class FullSize:
         n_max = max(len(w.claim_idx) for w in self.waves)
         self.r = rc.RC(g.layers, g.kv_heads, g.head_dim, g.elem_bytes, g.block_size, g.pool_blocks, self.pool, self.fill,
                        host_bytes, staging_chunk_bytes=2 << 30, staging_chunks=2, max_claims=max(1024, 4 * n_max),
-                       max_table_entries=max(4 * g.pool_blocks, 1 << 16), max_events=max(1 << 16, 16 * n_max), dedup=dedup)
+                       max_table_entries=max(4 * g.pool_blocks, 1 << 16), max_events=max(1 << 16, 16 * n_max), dedup=dedup,
+                       layer_major=layer_major)
+        self.lm = layer_major
         self.view = self.pool.view(2 * g.layers, g.pool_blocks, g.page_bytes)
         self.rng = np.random.default_rng(100 + index)
         wgen = torch.Generator(device=dev)
@@ -201,8 +203,9 @@ class FullSize:
             info = r.claim_info(cid)
             assert info["state"] == 3 and info["nb"] == a["nb"][cid] and info["host_bytes"] == info["nb"] * g.blk_bytes
             d, e = r.claim_digests(cid, both=True)
+            whole = r.host_read(cid).reshape(2 * g.layers, info["nb"], g.page_bytes) if self.lm else None   # [g][block][page]
             for j, i in enumerate(S):
-                hb = r.host_store(cid, i)
+                hb = np.ascontiguousarray(whole[:, i, :]).reshape(-1) if self.lm else r.host_store(cid, i)
                 assert hb is not None and np.array_equal(hb, want[j].reshape(-1)), "host bytes of claim %x block %d" % (cid, i)
                 assert int(d[i]) == rco.block_digest(hb, 2 * g.layers, 0) and int(e[i]) == rco.block_digest(hb, 2 * g.layers, 1)
             assert info["chain"] == rco.chain_of(cid, d)
@@ -345,4 +348,15 @@ def test_config4_long_context_full_size_interleaved():
     ev = fs.run()
     n = sum(len(w.claim_idx) for w in fs.waves)
     assert int((ev["code"] == 6).sum()) == n and fs.r.stats()["claims_restored"] == n
+    fs.close()
+
+
+def test_config1_full_size_layer_major():
+    """configs[1] in bench.py's launch configuration with rc_config.layer_major: the host copy is [g][block][page]; sampled
+    blocks are cut out of it by that layout and must equal the torch copy taken before the offload, their digests the
+    oracle's; round trip, fingerprints, stream as in every other full-size run."""
+    fs = FullSize(1, wave_frac=8, host_bytes=16 << 30, n_waves=4, layer_major=True)
+    ev = fs.run()
+    s = fs.r.stats()
+    assert s["bytes_d2h"] == s["gather_blocks"] * fs.g.blk_bytes and int((ev["code"] == 6).sum()) > 0
     fs.close()
