@@ -742,7 +742,7 @@ def test_split_forms_random_interleavings(seed):
     bytes are compared on the way, the whole event stream at the end.  The pool is small enough for NO_FREE_BLOCKS to occur;
     the host store is ample (an offload's host-space grant is taken at _begin: rc.h)."""
     rng = np.random.default_rng(1000 + seed)
-    wl = W.make_workload(0, n_claims=48, pool_blocks=700)
+    wl = W.make_workload(0, n_claims=48, pool_blocks=160)        # ~5 claims fit: NO_FREE_BLOCKS is common
     g = wl.geom
     p = Pair(wl, 1 << 30, chunk_blocks=41)
     o, r = p.o, p.r
@@ -756,7 +756,7 @@ def test_split_forms_random_interleavings(seed):
         nt = -(-c.P // g.block_size)
         used, _ = o.pool_state()
         free = np.nonzero(used == 0)[0].astype(np.uint32)
-        if free.size < nt + 40:
+        if free.size < nt:
             return False
         tab = rng.choice(free[free.size // 2:] if free.size // 2 >= nt else free, nt, replace=False).astype(np.uint32)
         fv = np.array([min(g.block_size, max(0, c.M - i * g.block_size)) for i in range(nt)], np.uint8)
@@ -855,7 +855,7 @@ def test_split_forms_random_interleavings(seed):
     ev = p.check_events("random interleavings")
     ok, why = V.validate(ev)
     assert ok, why
-    assert len(ev) > 150
+    assert len(ev) > 100 and n_nofree > 0 and n_busy_status > 0      # the refusals did occur
     s = r.stats()
     assert o.link_bytes() == (s["bytes_d2h"], s["bytes_h2d"]) and o.stats()["host_used"] == s["host_used_bytes"]
     p.close()
