@@ -40,7 +40,7 @@ extern "C" {
 typedef struct rc_ctx rc_ctx;
 
 enum { RC_OK = 0, RC_ERR_INVALID = -1, RC_ERR_CUDA = -2, RC_ERR_NOMEM = -3, RC_ERR_CAPACITY = -4,
-       RC_ERR_BUSY = -5 };
+       RC_ERR_BUSY = -5, RC_ERR_TOO_LARGE = -6 /* rc_digest_blocks_noalloc: beyond its fixed scratch */ };
 
 /* per-claim status */
 enum { RC_ST_OK = 0, RC_ST_PRED_FALSE = 1, RC_ST_UNKNOWN_CLAIM = 2, RC_ST_BAD_STATE = 3,
@@ -302,6 +302,22 @@ int rc_measure_link(rc_ctx* ctx, uint64_t bytes, int direction, int reps, double
  * are HOST arrays (d and e of each block; either may be NULL); ms (may be NULL) receives the device
  * time of the digest kernel. */
 int rc_digest_blocks(rc_ctx* ctx, const void* src_dev, uint32_t n_blocks, uint64_t* digests, uint64_t* digests2, float* ms);
+
+/* The one entry point that ALLOCATES NOTHING -- for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Same result as rc_digest_blocks (d and e of `n_blocks` contiguous
+ * blocks at DEVICE address src_dev, offload order: block-major, then page g = layer*2 + kv), but: no context; geometry
+ * passed in (blk = 2*layers*page_bytes, page_bytes % 4096 == 0, src_dev 16-byte aligned); d_out_dev / e_out_dev are
+ * caller-owned DEVICE arrays of n_blocks u64; the two kernels are enqueued on `stream` (a cudaStream_t, NULL = the default
+ * stream) and the call returns without synchronising -- the outputs are complete in stream order.  The scratch the pass
+ * needs (128 B of partial sums per page) lives in a fixed 4 MiB device array inside the library, which every GPU that
+ * loads the library holds until exit: n_blocks * 2 * layers <= RC_NOALLOC_MAX_PAGES, beyond that RC_ERR_TOO_LARGE and
+ * nothing is enqueued (split the range, or use rc_digest_blocks).  Calls no cudaMalloc / cudaFree / allocating routine;
+ * the first call on a device looks up the array's address on that device (the device must be current, as for every
+ * call).  Every call on a device shares the array: nothing in it has to start at zero, but calls that may overlap on
+ * the GPU (different streams, no ordering between them) race on it -- order them on one stream or by events. */
+#define RC_NOALLOC_MAX_PAGES 32768u
+int rc_digest_blocks_noalloc(const void* src_dev, uint32_t n_blocks, uint32_t layers, uint64_t page_bytes,
+                             uint64_t* d_out_dev, uint64_t* e_out_dev, void* stream);
 
 /* NEXT-1: the paper's artifact analyzer as a device pass.  Validates an event
  * array (HOST, n records in stream order; may contain the harness marker codes RC_EV_USE and

@@ -19,6 +19,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <string>
 #include <unordered_map>
 #include <unordered_set>
@@ -1735,7 +1736,66 @@ extern "C" const char* rc_strerror(int err) {
     case RC_ERR_NOMEM: return "out of memory";
     case RC_ERR_CAPACITY: return "capacity exceeded (claims, table entries, events or batch size)";
     case RC_ERR_BUSY: return "an operation of this kind is still in flight";
+    case RC_ERR_TOO_LARGE: return "size exceeds the fixed scratch of the no-allocation entry point (RC_NOALLOC_MAX_PAGES)";
     default: return "unknown error";
   }
 }
 extern "C" const char* rc_last_cuda_error(rc_ctx* c) { return c ? c->cuda_err.c_str() : ""; }
+
+
+// ---- the entry point that allocates nothing (rc.h: rc_digest_blocks_noalloc) ---------------------------------------------
+// The standalone checksum pass (k_move_hash_tma<DIGEST> + k_block_digest) needs scratch: the warp partial sums of every
+// page, 128 B each.  rc_digest_blocks takes them from a context (cudaMalloc at rc_create); this variant takes them from
+// a file-scope array, so that callers that may not allocate -- CUDA graph capture, serving loops, harnesses that forbid
+// cudaMalloc -- have one entry point that needs no context and calls no allocating routine.  Every GPU that loads the
+// library holds the 4 MiB until exit.  Every call shares the array; nothing in it has to start at zero (each partial the
+// reduction reads is written by the same call's first kernel), and two calls that overlap on the GPU race on it.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[(size_t)RC_NOALLOC_MAX_PAGES * WPC * 2 * sizeof(u64)];
+
+namespace {
+struct NoAllocDev { bool ready = false; u64* scratch = nullptr; int sms = 0; };
+constexpr int kNoAllocMaxDev = 64;
+NoAllocDev g_noalloc_dev[kNoAllocMaxDev];
+std::mutex g_noalloc_mu;
+}  // namespace
+
+extern "C" int rc_digest_blocks_noalloc(const void* src, uint32_t n_blocks, uint32_t layers, uint64_t page_bytes,
+                                        uint64_t* d_out, uint64_t* e_out, void* stream) {
+  if (n_blocks == 0) return RC_OK;
+  if (!src || ((uintptr_t)src & 15) || !d_out || !e_out || !layers || !page_bytes || page_bytes % 4096 != 0 ||
+      page_bytes > (1ull << 30) || layers > (1u << 20))
+    return RC_ERR_INVALID;
+  const u64 G = 2ull * layers, pages = (u64)n_blocks * G;
+  if (pages > RC_NOALLOC_MAX_PAGES) return RC_ERR_TOO_LARGE;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kNoAllocMaxDev) return RC_ERR_CUDA;
+  NoAllocDev nd;
+  {
+    // set-up, once per device, with that device current: in host code the array's name is a host-side stand-in, not a
+    // device address -- the kernels get the address cudaGetSymbolAddress returns for THIS device
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    NoAllocDev& slot = g_noalloc_dev[dev];
+    if (!slot.ready) {
+      void* p = nullptr;
+      if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || !p) return RC_ERR_CUDA;
+      if (cudaDeviceGetAttribute(&slot.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || slot.sms <= 0) return RC_ERR_CUDA;
+      slot.scratch = (u64*)p;
+      slot.ready = true;
+    }
+    nd = slot;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  const u32 grid = (u32)std::min<u64>(pages, 2ull * nd.sms);
+  // 8 KiB (4 KiB for pages that are no multiple of 8 KiB) tiles x 4 stages: 32 / 16 KiB of dynamic shared memory, below the
+  // 48 KiB that need no function attribute
+  if (page_bytes % 8192 == 0)
+    k_move_hash_tma<MV_DIGEST, 4, 8192, 1><<<grid, tma_threads<1>(), 4 * 8192, s>>>(
+        nullptr, (u8*)src, nullptr, nd.scratch, n_blocks, (u32)G, 0, (u32)page_bytes, nullptr, nullptr, (u32)G, 1);
+  else
+    k_move_hash_tma<MV_DIGEST, 4, 4096, 1><<<grid, tma_threads<1>(), 4 * 4096, s>>>(
+        nullptr, (u8*)src, nullptr, nd.scratch, n_blocks, (u32)G, 0, (u32)page_bytes, nullptr, nullptr, (u32)G, 1);
+  if (cudaGetLastError() != cudaSuccess) return RC_ERR_CUDA;
+  k_block_digest<<<warps_grid(n_blocks), 256, 0, s>>>(nd.scratch, nullptr, d_out, e_out, n_blocks, (u32)G, nullptr);
+  if (cudaGetLastError() != cudaSuccess) return RC_ERR_CUDA;
+  return RC_OK;
+}

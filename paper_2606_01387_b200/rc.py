@@ -29,7 +29,7 @@ EXPORTS = ["rc_create", "rc_destroy", "rc_mark_used", "rc_mark_free", "rc_set_fi
            "rc_restore_request_begin", "rc_tp_restore_verify", "rc_tp_restore_commit", "rc_tp_mailbox", "rc_tp_set_peer",
            "rc_tp_ipc_handle", "rc_tp_open_peer", "rc_protect", "rc_make_room", "rc_protected_map", "rc_outcomes", "rc_set_faults",
            "rc_release", "rc_claim_info", "rc_claim_blocks", "rc_claim_digests", "rc_host_read", "rc_host_store", "rc_sync", "rc_pool_state",
-           "rc_stats_get", "rc_stats_reset", "rc_measure_link", "rc_digest_blocks", "rc_validate_trace", "rc_strerror",
+           "rc_stats_get", "rc_stats_reset", "rc_measure_link", "rc_digest_blocks", "rc_digest_blocks_noalloc", "rc_validate_trace", "rc_strerror",
            "rc_last_cuda_error"]
 
 
@@ -372,6 +372,16 @@ class RC:
         self._ck(self.L.rc_digest_blocks(self.h, C.c_void_p(src_ptr), n_blocks, _p(d) if want else None,
                                          _p(e) if want else None, C.byref(ms)), "rc_digest_blocks")
         return ((d, e) if both else d), ms.value
+
+
+ERR_TOO_LARGE = -6
+NOALLOC_MAX_PAGES = 32768
+
+
+def digest_blocks_noalloc(src_ptr, n_blocks, layers, page_bytes, d_out_ptr, e_out_ptr, stream_ptr=0):
+    """rc_digest_blocks_noalloc: device pointers in, nothing allocated, enqueued on the given stream.  Returns the code."""
+    return lib().rc_digest_blocks_noalloc(C.c_void_p(src_ptr), C.c_uint32(n_blocks), C.c_uint32(layers), C.c_uint64(page_bytes),
+                                          C.c_void_p(d_out_ptr), C.c_void_p(e_out_ptr), C.c_void_p(stream_ptr))
 
 
 def validate_trace(events, want_claims=True):
