@@ -29,6 +29,9 @@
  * the caller's; writes the caller makes to pool_dev / fill_dev must have completed
  * (stream or device synchronise) before a call that reads them, and the library's
  * writes are complete when a synchronous call or rc_wait returns.
+ * Environment: RC_CHECK=1 at rc_create turns on checked mode -- the work items of every gather / scatter launch are
+ * validated on the device (pool block, work position, staged block in range) and rc_wait returns RC_ERR_CUDA if one was
+ * not; RC_TRACE_LAUNCHES=1 prints per-launch device times on stderr; RC_TMA_VARIANT=<i> overrides the mover variant.
  */
 #ifndef RC_H_
 #define RC_H_

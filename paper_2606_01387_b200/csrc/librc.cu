@@ -130,6 +130,7 @@ struct rc_ctx {
   Desc* d_desc[4] = {}; Res* d_res[4] = {}; u32* d_off[4] = {};
   Desc* h_desc[4] = {}; Res* h_res[4] = {};
   u32* h_up = nullptr; u64* h_flip = nullptr; u32* h_counters = nullptr;
+  bool check = false; u32 *h_check = nullptr, *d_check = nullptr;   // RC_CHECK=1: work items validated before every mover launch
   // per operation in flight: work list and block digests.  Index = op index: 0 = offload slot 0, 1 = restore, 2 = offload slot 1
   u32* d_phys[3] = {}; u64* d_dtmp[3] = {}; u64* d_etmp[3] = {};
   std::vector<u8*> staging[2]; std::vector<u64*> part[2];
@@ -235,6 +236,13 @@ template <int MODE>
 static void launch_move(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys, u64* part, u32 n_items,
                         const u32* iw = nullptr, const u32* ispos = nullptr, bool layer_major = false) {
   const u32 sw = layer_major ? 1u : c->G, sg = layer_major ? n_items : 1u;     // staged page of (item, g): w*sw + g*sg
+  if (c->check) {                                          // RC_CHECK=1: bound every access of this launch by its work items
+    const bool to_host_store = c->direct && staging == c->h_store_dev;
+    const u64 staged_limit = to_host_store ? c->host_blocks : c->chunk_blocks;
+    if (n_items > c->chunk_blocks) *c->h_check = 1u;      // the partial-sum buffer and a staging chunk hold chunk_blocks items
+    k_check_items<<<(n_items + 255) / 256, 256, 0, s>>>(MODE == MV_DIGEST ? nullptr : phys, n_items, c->NB, iw, (u32)std::min<u64>(c->cap_entries, 0xFFFFFFFFu),
+                                                         ispos, (u32)std::min<u64>(staged_limit, 0xFFFFFFFFu), c->d_check);
+  }
   if (c->mover == RC_MOVER_TMA) {
     const TmaVariant& v = kTma[c->tma_variant[MODE]];
     const u32 grid = std::min(n_items * c->G, c->tma_grid[MODE]);
@@ -259,7 +267,7 @@ extern "C" int rc_destroy(rc_ctx* c) {
     if (c->ev_body_a[i]) cudaEventDestroy(c->ev_body_a[i]);
     if (c->ev_body_b[i]) cudaEventDestroy(c->ev_body_b[i]);
   }
-  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_evbuf); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
+  FH(c->h_up); FH(c->h_flip); FH(c->h_counters); FH(c->h_check); FH(c->h_evbuf); FH(c->h_dig); FH(c->h_dig2); FH(c->h_iw); FH(c->h_ispos); FH(c->h_hpos);
   F(c->d_iw); F(c->d_ispos); F(c->d_hpos);
   FH(c->h_store);
   for (int d = 0; d < 2; ++d) {
@@ -360,6 +368,10 @@ extern "C" int rc_create(const rc_config* cfg, rc_ctx** out) {
   CC(cudaHostAlloc(&c->h_up, cap * 4, cudaHostAllocMapped), RC_ERR_NOMEM);
   CC(cudaHostAlloc(&c->h_flip, dc * 8, cudaHostAllocMapped), RC_ERR_NOMEM);
   CC(cudaHostAlloc(&c->h_counters, 16, cudaHostAllocMapped), RC_ERR_NOMEM);
+  CC(cudaHostAlloc(&c->h_check, 4, cudaHostAllocMapped), RC_ERR_NOMEM);
+  *c->h_check = 0;
+  CC(cudaHostGetDevicePointer((void**)&c->d_check, c->h_check, 0), RC_ERR_CUDA);
+  if (const char* e = getenv("RC_CHECK")) c->check = atoi(e) != 0;
   c->ev_bounce_cap = std::min<u64>(cfg->max_events, 1u << 16);
   CC(cudaHostAlloc(&c->h_evbuf, c->ev_bounce_cap * sizeof(Event), cudaHostAllocMapped), RC_ERR_NOMEM);
   c->dedup = cfg->dedup != 0;
@@ -879,6 +891,11 @@ static int collect_times(rc_ctx* c, Op& op, float& ms_k, float& ms_c) {
 
 // Completes the oldest open offload: a4 on `meta` (after the transfer: "offloaded" follows the finished copy),
 // then the host-side claim records.
+static int check_flag(rc_ctx* c) {                         // after the operation's streams have been waited for
+  if (c->check && *c->h_check) { c->poisoned = true; c->cuda_err = "RC_CHECK: a work item of a mover launch was out of range"; return RC_ERR_CUDA; }
+  return RC_OK;
+}
+
 static int wait_offload(rc_ctx* c) {
   if (!c->off_open) return RC_OK;
   const int slot = c->off_q[0], oi = off_oi(slot), set = off_set(slot);
@@ -893,6 +910,7 @@ static int wait_offload(rc_ctx* c) {
   if ((rc = emit(c, set, n, EM_OFFLOAD))) return rc;
   CK(to_host(c->meta, c->h_res[set], c->d_res[set], (u64)n * sizeof(Res)));
   CK(cudaStreamSynchronize(c->meta));
+  if ((rc = check_flag(c))) return rc;
   op.active = false;
   c->off_q[0] = c->off_q[1]; --c->off_open;
   u64 served = 0;
@@ -1096,6 +1114,7 @@ static int wait_restore(rc_ctx* c) {
   int rc;
   if ((rc = restore_tail(c))) return rc;
   CK(cudaStreamSynchronize(c->meta));
+  if ((rc = check_flag(c))) return rc;
   op.active = false;
   const Desc* hd = c->h_desc[1];
   for (u32 k = 0; k < op.n; ++k) {

@@ -783,6 +783,22 @@ __global__ void k_copy_words(u32* __restrict__ dst, const u32* __restrict__ src,
   for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += (u64)gridDim.x * blockDim.x) dst[i] = src[i];
 }
 
+// Checked mode (RC_CHECK=1; compute-sanitizer is closed on this pool): every address a mover forms derives from its work
+// items -- phys[w] (pool block), iw[w] (work position), ispos[w] (staged block) -- and the loop bounds, so validating the
+// items before each launch bounds every access of that launch.  A violation sets the mapped flag; the host refuses to
+// complete the operation.
+__global__ void k_check_items(const u32* __restrict__ phys, u32 n_items, u32 NB, const u32* __restrict__ iw, u32 iw_limit,
+                              const u32* __restrict__ ispos, u32 ispos_limit, u32* __restrict__ flag) {
+  const u32 w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= n_items) return;
+  bool bad = false;
+  u32 pw = w;
+  if (iw) { pw = iw[w]; bad |= pw >= iw_limit; }
+  if (phys && !bad) { const u32 b = phys[pw]; bad |= (b >= NB && b != SKIP); }
+  if (ispos) bad |= ispos[w] >= ispos_limit;
+  if (bad) *flag = 1u;
+}
+
 // rc_set_fill: fill[ids[i]] = vals[i] (the caller's materialization marks, sent as host arrays)
 __global__ void k_fill_write(const u32* __restrict__ ids, const u8* __restrict__ vals, u32 n, u8* __restrict__ fill) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;

@@ -879,3 +879,20 @@ def test_set_fill_from_host_arrays():
     assert np.array_equal(p.fill_t.cpu().numpy(), want)
     p.r.set_fill(np.zeros(0, np.uint32), np.zeros(0, np.uint8))
     p.close()
+
+
+@pytest.mark.parametrize("mode", ["plain", "dedup", "direct", "layer_major", "ldg"])
+def test_checked_mode_finds_no_out_of_range_work_item(mode, monkeypatch):
+    """RC_CHECK=1 (compute-sanitizer is closed on this pool): k_check_items validates the work items of every mover launch --
+    pool block, work position, staged block -- and rc_wait refuses to complete an operation whose flag is set.  The Tiny
+    wave with ragged chunks runs clean in every mover mode, and results do not change."""
+    monkeypatch.setenv("RC_CHECK", "1")
+    wl, wave = W.make_workload(0), None
+    kw = dict(dedup=mode == "dedup", direct_offload=mode == "direct", layer_major=mode == "layer_major",
+              mover=rc.MOVER_LDG if mode == "ldg" else rc.MOVER_AUTO)
+    p = Pair(wl, 1 << 30, chunk_blocks=7, **kw)
+    wave = W.plan_waves(wl, 1 << 30)[0]
+    ev, st_r = p.run_wave(wave)
+    assert V.validate(ev)[0] and st_r.count(rc.ST_RESTORE_FAILED) == 1
+    assert p.r.stats()["kernel_launches"] > 0
+    p.close()
