@@ -280,6 +280,8 @@ int rc_claim_blocks(rc_ctx* ctx, uint64_t claim_id, uint32_t* ids, uint32_t cap,
 /* d: the recorded per-block checksums (chained into `chain`); e (may be NULL): the second digests -- (d[i], e[i]) is
  * the 128-bit content key of block i (DESIGN.md "Checksum" R22). */
 int rc_claim_digests(rc_ctx* ctx, uint64_t claim_id, uint64_t* d, uint64_t* e, uint32_t cap, uint32_t* n);
+/* Copies the claim's host bytes (its own layout) to dst if cap suffices; *bytes = their size (0: none held).  RC_ERR_BUSY while
+ * the claim's offload is in flight. */
 int rc_host_read(rc_ctx* ctx, uint64_t claim_id, void* dst, uint64_t cap, uint64_t* bytes);
 /* Borrowed, READ-ONLY view of the claim's host copy: *p = the pinned-store address of the claim's block `block` (offload
  * order: block-major, then page g = layer*2 + kv), *contiguous_bytes = how many bytes from there belong to the claim and

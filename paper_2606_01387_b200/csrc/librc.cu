@@ -484,7 +484,7 @@ extern "C" int rc_set_fill(rc_ctx* c, uint32_t n, const uint32_t* ids, const uin
   GUARD();
   if (n && (!ids || !vals)) return RC_ERR_INVALID;
   for (u32 i = 0; i < n; ++i) if (ids[i] >= c->NB || vals[i] > c->cfg.block_size) return RC_ERR_INVALID;
-  const u32 per = (u32)std::min<u64>(c->cap_entries * 4 / 5, 1u << 30);          // 4 B id + 1 B value per entry
+  const u32 per = (u32)std::min<u64>(std::max<u64>(1, c->cap_entries * 4 / 5 - 1), 1u << 30);   // 4 B id + 1 B value per entry, values padded to 4 B
   for (u32 s = 0; s < n; s += per) {
     const u32 m = std::min(per, n - s), vb = (m + 3) & ~3u;
     memcpy(c->h_up, ids + s, (u64)m * 4);
@@ -1541,6 +1541,7 @@ extern "C" int rc_host_read(rc_ctx* c, uint64_t id, void* dst, uint64_t cap, uin
   auto it = c->claims.find(id);
   if (it == c->claims.end() || !bytes) return RC_ERR_INVALID;
   const Claim& cl = it->second;
+  if (cl.busy && cl.state != RC_CS_OFFLOADED) return RC_ERR_BUSY;   // its offload is in flight: the host copy is not complete yet
   *bytes = (cl.host.empty() && cl.hslots.empty()) ? 0 : (u64)cl.nb * c->blk;
   if (dst && cap >= *bytes && *bytes) {
     u8* o = (u8*)dst;

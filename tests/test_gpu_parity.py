@@ -172,6 +172,7 @@ def test_two_open_offloads_run_ahead_of_a_restore():
     assert np.array_equal(o.offload(ids[0]), r.wait(0))         # completes O0 only
     p.check_claims(ids[0], "O0", host=True)
     assert r.claim_info(ids[1][0])["state"] == 2                # O1 is open: still MATERIALIZED, blocks still referenced
+    assert r.host_read(ids[1][0]) is None and r.host_store(ids[1][0], 0) is None   # RC_ERR_BUSY: its host copy is not complete yet
     for k in range(3):
         p.poison_free()
         fl = [(ids[k][1], rc.FAULT_BITFLIP, 12345 + k)] if k != 1 else [(ids[k][2], rc.FAULT_XFER_ERROR, 0)]
