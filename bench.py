@@ -360,6 +360,29 @@ def run_oracle(index, steps, warmup):
             "claims_per_s": claims / dt, "seconds": dt, "steps": steps}
 
 
+def single_claim_latency(job, reps=12):
+    """Latency of the synchronous calls on ONE claim (the shape of the paper's running example: a reuse request that needs
+    an ordered restoration of one claim), wall clock around each call, medians.  Not part of `value`."""
+    r, p = job.r, job.prep[0]
+    job._admit(p, False)
+    k = int(np.argmin(p["P"]))
+    cid = p["ids"][k:k + 1]
+    r.set_faults([])
+    t_off, t_res = [], []
+    for _ in range(reps):
+        t0 = time.perf_counter(); r.offload(cid); t1 = time.perf_counter(); r.restore(cid); t2 = time.perf_counter()
+        t_off.append(t1 - t0); t_res.append(t2 - t1)
+        r.outcomes(cap=64)
+    info = r.claim_info(int(cid[0]))
+    r.release(p["ids"])
+    r.outcomes(cap=1 << 16)
+    nbytes = info["nb"] * job.g.blk_bytes
+    mo, mr = float(np.median(t_off[2:])), float(np.median(t_res[2:]))
+    return {"tokens": int(p["P"][k]), "blocks": info["nb"], "bytes": nbytes, "offload_ms": mo * 1e3, "restore_ms": mr * 1e3,
+            "offload_gbs": nbytes / mo / 1e9, "restore_gbs": nbytes / mr / 1e9,
+            "what": "rc_offload / rc_restore of one claim, synchronous calls, wall clock, median of %d" % (reps - 2)}
+
+
 def reduce_scalar(dist, x, op, device="cuda"):
     """Cross-rank reduction of one number (the only collective of the multi-GPU run): max for times, sum for units."""
     if dist is None:
@@ -541,6 +564,11 @@ def main():
                        "ms_per_step": ms2_max / a.steps,
                        "what": "same step through the C ABI with host arrays; fill[] sent as host arrays (rc_set_fill), "
                                "statuses and the event stream read back, inside the timed region"}
+    if world == 1:
+        try:
+            line["single_claim"] = single_claim_latency(job)
+        except Exception as e:                                                 # a side measurement must not lose the main line
+            line["single_claim"] = {"error": repr(e)[:200]}
     if world == 1 and not a.no_cpu_baseline:   # NEXT-1: device trace validator on a 200k-claim synthetic stream (not part of `value`)
         sys.path.insert(0, os.path.join(ROOT, "tests"))
         import trace_inputs                                  # input generator only (tests/trace_inputs.py)
