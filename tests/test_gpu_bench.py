@@ -44,3 +44,28 @@ def test_bench_step_on_tiny(mode):
     ok, why = V.validate(ev)
     assert ok, why
     job.close()
+
+
+def test_bench_line_contract_on_tiny():
+    """`python bench.py` prints ONE JSON line with the keys the driver reads (smallest config, seconds)."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--config", "0", "--steps", "3", "--warmup", "3",
+                          "--no-cpu-baseline", "--per-config-budget-s", "0"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    l = json.loads(lines[0])
+    assert l["metric"] == "kv_offload_restore_throughput" and l["unit"] == "GB/s" and l["higher_is_better"] is True
+    assert l["n_gpus"] == 1 and l["steps"] == 3 and l["warmup"] == 3 and l["scaling"] == "weak" and l["vs_baseline"] is None
+    assert l["dtype"] == "u8" and l["data"] == "synthetic" and l["config"]["workload"].startswith("configs[0]")
+    assert l["value"] > 0 and l["ms_per_step"] > 0 and l["gpu_launches"] > 0
+    r = l["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9 and "traffic" in r
+    e = l["e2e"]
+    assert e["value"] > 0 and e["unit"] == "GB/s" and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    assert set(l["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    assert l["single_claim"]["restore_ms"] > 0
