@@ -40,3 +40,13 @@ def test_rc_create_rejects_bad_geometry():
     cfg = rc.Config(2, 2, 64, 2, 3, 256, 64, 4096, 4096, 2, 1 << 20, 1 << 20, 256, 256, 0, 0, 0, 0, 0, 0, 0, 0, 0)  # page % 4096 != 0
     assert rc.lib().rc_create(ctypes.byref(cfg), ctypes.byref(h)) == rc.ERR_INVALID
     assert rc.lib().rc_strerror(rc.ERR_CAPACITY).decode().startswith("capacity")
+
+
+def test_noalloc_entry_point_validates_before_it_touches_the_device():
+    L = rc.lib()
+    big = rc.NOALLOC_MAX_PAGES // 4 + 1                        # layers = 2 -> 4 pages per block
+    assert rc.digest_blocks_noalloc(256, big, 2, 4096, 256, 256) == rc.ERR_TOO_LARGE
+    assert "scratch" in L.rc_strerror(rc.ERR_TOO_LARGE).decode()
+    assert rc.digest_blocks_noalloc(256, 1, 2, 4096 + 64, 256, 256) == rc.ERR_INVALID       # page % 4096
+    assert rc.digest_blocks_noalloc(264, 1, 2, 4096, 256, 256) == rc.ERR_INVALID            # source alignment
+    assert rc.digest_blocks_noalloc(0, 0, 2, 4096, 0, 0) == 0                               # empty range
