@@ -191,14 +191,15 @@ class RC:
         ids = _u64(ids)
         st = np.full(ids.size, -1, np.int32)
         self._ck(self.L.rc_offload_begin(self.h, ids.size, _p(ids), _p(st)), "rc_offload_begin")
-        self._pending.setdefault(0, []).append((ids, st))      # up to two offloads may be open (rc.h)
+        # every _begin is paired with one wait(); served entries are pending (-1) iff the library opened an operation
+        self._pending.setdefault(0, []).append((ids, st, bool((st == -1).any())))
         return st
 
     def restore_begin(self, ids):
         ids = _u64(ids)
         st = np.full(ids.size, -1, np.int32)
         self._ck(self.L.rc_restore_begin(self.h, ids.size, _p(ids), _p(st)), "rc_restore_begin")
-        self._pending[1] = [(ids, st)]
+        self._pending.setdefault(1, []).append((ids, st, bool((st == -1).any())))
         return st
 
     def restore_request(self, request_id, ids, check=True):
@@ -215,7 +216,7 @@ class RC:
         st = np.full(ids.size, -1, np.int32)
         self._ck(self.L.rc_restore_request_begin(self.h, C.c_uint64(request_id), ids.size, _p(ids), _p(st)),
                  "rc_restore_request_begin")
-        self._pending[1] = [(ids, st)]
+        self._pending.setdefault(1, []).append((ids, st, bool((st == -1).any())))
         return st
 
     def set_policy(self, ids, policy):
@@ -277,8 +278,12 @@ class RC:
         return prot
 
     def wait(self, which):
-        self._ck(self.L.rc_wait(self.h, which), "rc_wait")
+        """Completes the oldest _begin of this kind and returns its status array.  A _begin that served nothing opened no
+        operation in the library: its statuses were final at once and its wait() does not touch the library."""
         q = self._pending.get(which)
+        if q and not q[0][2]:
+            return q.pop(0)[1]
+        self._ck(self.L.rc_wait(self.h, which), "rc_wait")
         return q.pop(0)[1] if q else None
 
     def test(self, which):

@@ -165,10 +165,13 @@ def test_two_open_offloads_run_ahead_of_a_restore():
 
     ids = [admit(w) for w in waves]
     assert r.test(0) and r.test(1)                              # nothing in flight
+    st_none = r.offload_begin([987654321])                      # nothing served: no operation is opened, statuses are final
+    assert list(st_none) == [rc.ST_UNKNOWN_CLAIM] and list(o.offload([987654321])) == [rc.ST_UNKNOWN_CLAIM]
     r.offload_begin(ids[0])
     r.offload_begin(ids[1])
     rc3, _ = r._batch(r.L.rc_offload_begin, "rc_offload_begin", ids[2], check=False)
     assert rc3 == rc.ERR_BUSY                                   # a third open offload is refused and changes nothing
+    assert list(r.wait(0)) == [rc.ST_UNKNOWN_CLAIM]             # the wait of the _begin that opened nothing: no library call
     assert np.array_equal(o.offload(ids[0]), r.wait(0))         # completes O0 only
     p.check_claims(ids[0], "O0", host=True)
     assert r.claim_info(ids[1][0])["state"] == 2                # O1 is open: still MATERIALIZED, blocks still referenced
