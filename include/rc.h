@@ -180,6 +180,8 @@ int rc_restore(rc_ctx* ctx, uint32_t n, const uint64_t* claim_id, int32_t* statu
 /* Split forms (BASELINE.json configs[4]: restore of batch k overlapped with the offload of the next batches on
  * separate streams).  _begin validates, enqueues the data movement and returns; rc_wait completes the operation: the
  * status array must stay valid until rc_wait fills it in.  which: 0 = offload, 1 = restore.
+ * On return from a _begin, status[k] is final for the entries that were not served and -1 for the served ones; if no entry
+ * is -1, nothing was opened and no rc_wait is owed for this call (rc_wait always completes the oldest operation that IS open).
  *   rc_offload_begin  enqueues a1-a3 and the chain on the gather / d2h streams.  Up to TWO offloads may be open; they
  *       run back to back, so the D2H direction stays busy while a slower restore is still in flight.  The claims stay
  *       referenced (their pool blocks are not free) until the offload is completed.  RC_ERR_BUSY with two open (one
