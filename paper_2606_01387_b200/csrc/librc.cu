@@ -185,7 +185,7 @@ static cudaEvent_t get_event(rc_ctx* c) {
 // ---- small transfers ----------------------------------------------------------------------------------------
 // host_ptr is a mapped pinned buffer of the library (cudaHostAllocMapped); the words cross PCIe in a kernel on `s`, in
 // stream order, never through a copy engine (rc_kernels.cuh: k_copy_words).  bytes % 4 == 0.
-static cudaError_t small_copy(cudaStream_t s, void* dst, const void* src, u64 bytes, bool dst_is_host) {
+static cudaError_t small_copy(rc_ctx* c, cudaStream_t s, void* dst, const void* src, u64 bytes, bool dst_is_host) {
   if (!bytes) return cudaSuccess;
   void* hd = nullptr;
   cudaError_t e = cudaHostGetDevicePointer(&hd, dst_is_host ? dst : const_cast<void*>(src), 0);
@@ -194,10 +194,11 @@ static cudaError_t small_copy(cudaStream_t s, void* dst, const void* src, u64 by
   const u32 grid = (u32)std::min<u64>((n + 255) / 256, 592);
   if (dst_is_host) k_copy_words<<<grid, 256, 0, s>>>((u32*)hd, (const u32*)src, n);
   else k_copy_words<<<grid, 256, 0, s>>>((u32*)dst, (const u32*)hd, n);
+  c->st.kernel_launches++;
   return cudaGetLastError();
 }
-static inline cudaError_t to_dev(cudaStream_t s, void* d, const void* h, u64 bytes) { return small_copy(s, d, h, bytes, false); }
-static inline cudaError_t to_host(cudaStream_t s, void* h, const void* d, u64 bytes) { return small_copy(s, h, d, bytes, true); }
+static inline cudaError_t to_dev(rc_ctx* c, cudaStream_t s, void* d, const void* h, u64 bytes) { return small_copy(c, s, d, h, bytes, false); }
+static inline cudaError_t to_host(rc_ctx* c, cudaStream_t s, void* h, const void* d, u64 bytes) { return small_copy(c, s, h, d, bytes, true); }
 
 // ---- data movers -----------------------------------------------------------------------------
 template <int MODE>
@@ -242,6 +243,7 @@ static void launch_move(rc_ctx* c, cudaStream_t s, u8* staging, const u32* phys,
     if (n_items > c->chunk_blocks) *c->h_check = 1u;      // the partial-sum buffer and a staging chunk hold chunk_blocks items
     k_check_items<<<(n_items + 255) / 256, 256, 0, s>>>(MODE == MV_DIGEST ? nullptr : phys, n_items, c->NB, iw, (u32)std::min<u64>(c->cap_entries, 0xFFFFFFFFu),
                                                          ispos, (u32)std::min<u64>(staged_limit, 0xFFFFFFFFu), c->d_check);
+    c->st.kernel_launches++;
   }
   if (c->mover == RC_MOVER_TMA) {
     const TmaVariant& v = kTma[c->tma_variant[MODE]];
@@ -445,11 +447,11 @@ static int ev_room(rc_ctx* c, u64 extra) {
   return (c->ev_emitted - c->ev_drained) + c->ev_reserved + extra <= c->cfg.max_events;
 }
 static int upload_desc(rc_ctx* c, int set, u32 n) {
-  CK(to_dev(c->meta, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
+  CK(to_dev(c, c->meta, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
   return RC_OK;
 }
 static int fetch_res(rc_ctx* c, int set, u32 n) {
-  CK(to_host(c->meta, c->h_res[set], c->d_res[set], (u64)n * sizeof(Res)));
+  CK(to_host(c, c->meta, c->h_res[set], c->d_res[set], (u64)n * sizeof(Res)));
   return RC_OK;
 }
 static int emit(rc_ctx* c, int set, u32 n, int mode, u64 request_id = 0) {
@@ -470,7 +472,7 @@ static int mark(rc_ctx* c, u32 n, const u32* ids, int val) {
   for (u32 s = 0; s < n; s += (u32)c->cap_entries) {
     const u32 m = (u32)std::min<u64>(n - s, c->cap_entries);
     memcpy(c->h_up, ids + s, (u64)m * 4);
-    CK(to_dev(c->meta, c->d_up, c->h_up, (u64)m * 4));
+    CK(to_dev(c, c->meta, c->d_up, c->h_up, (u64)m * 4));
     k_mark<<<(m + 255) / 256, 256, 0, c->meta>>>(c->d_up, m, c->d_used, c->d_ref, val);
     CKL();
     c->st.kernel_launches++;
@@ -489,7 +491,7 @@ extern "C" int rc_set_fill(rc_ctx* c, uint32_t n, const uint32_t* ids, const uin
     const u32 m = std::min(per, n - s), vb = (m + 3) & ~3u;
     memcpy(c->h_up, ids + s, (u64)m * 4);
     memcpy((u8*)(c->h_up + m), vals + s, m);
-    CK(to_dev(c->meta, c->d_up, c->h_up, (u64)m * 4 + vb));
+    CK(to_dev(c, c->meta, c->d_up, c->h_up, (u64)m * 4 + vb));
     k_fill_write<<<(m + 255) / 256, 256, 0, c->meta>>>(c->d_up, (const u8*)(c->d_up + m), m, c->fill);
     CKL();
     c->st.kernel_launches++;
@@ -531,7 +533,7 @@ static int accept_run(rc_ctx* c, u32 n, const u64* id, const u32* P, const u32* 
   if (cand.empty()) return RC_OK;
   int rc;
   if ((rc = upload_desc(c, 2, n))) return rc;
-  CK(to_dev(c->meta, c->d_up, c->h_up, up * 4));
+  CK(to_dev(c, c->meta, c->d_up, c->h_up, up * 4));
   k_accept<<<std::min<u32>(n, c->accept_ctas), 256, 0, c->meta>>>(c->d_desc[2], c->d_res[2], n, c->d_up, c->d_bt, c->d_used,
                                                                  c->d_ref, c->NB, c->d_bitmaps);
   CKL();
@@ -817,7 +819,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
   int rc;
   // The head (offsets, compaction) only reads tables that completed calls wrote, so it runs on the gather stream;
   // nothing of an offload touches `meta` before rc_wait(0).
-  CK(to_dev(c->gather, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
+  CK(to_dev(c, c->gather, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
   k_offsets<<<1, 1024, 0, c->gather>>>(c->d_desc[set], n, c->d_off[set]);
   CKL();
   k_worklist<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[set], c->d_res[set], n, c->d_off[set], c->d_bt, nullptr, c->d_phys[oi], 0);
@@ -835,7 +837,7 @@ extern "C" int rc_offload_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
         for (u64 w = std::max(g.w0, w0); w < std::min(g.w0 + g.n, w1); ++w) c->h_hpos[w] = (u32)(g.hoff + (w - g.w0));
         if (g.w0 + g.n <= w1) ++si; else break;
       }
-      CK(to_dev(c->gather, c->d_hpos + w0, c->h_hpos + w0, (u64)m * 4));
+      CK(to_dev(c, c->gather, c->d_hpos + w0, c->h_hpos + w0, (u64)m * 4));
       cudaEvent_t t0 = get_event(c), t1 = get_event(c);
       CK(cudaEventRecord(t0, c->gather));
       launch_move<MV_GATHER>(c, c->gather, c->h_store_dev, c->d_phys[oi] + w0, c->part[0][slot], m, nullptr, c->d_hpos + w0);
@@ -908,7 +910,7 @@ static int wait_offload(rc_ctx* c) {
   CKL();
   c->st.kernel_launches++;
   if ((rc = emit(c, set, n, EM_OFFLOAD))) return rc;
-  CK(to_host(c->meta, c->h_res[set], c->d_res[set], (u64)n * sizeof(Res)));
+  CK(to_host(c, c->meta, c->h_res[set], c->d_res[set], (u64)n * sizeof(Res)));
   CK(cudaStreamSynchronize(c->meta));
   if ((rc = check_flag(c))) return rc;
   op.active = false;
@@ -967,10 +969,10 @@ static int restore_tail(rc_ctx* c) {
     k_tp_push<<<1, 1024, 0, c->meta>>>(c->d_verd, n, peers, c->tp_ranks, c->tp_rank, (u32)c->desc_cap, c->tp_epoch);
     CKL();
     c->st.kernel_launches += 2;
-    CK(to_host(c->meta, c->h_verd, c->d_verd, (u64)n * sizeof(TpVerdict)));
+    CK(to_host(c, c->meta, c->h_verd, c->d_verd, (u64)n * sizeof(TpVerdict)));
   } else {
     if ((rc = emit(c, 1, n, EM_RESTORE, op.request_id))) return rc;
-    CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
+    CK(to_host(c, c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
   }
   op.tail = true;
   return RC_OK;
@@ -1015,7 +1017,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
                                           c->d_counters);
   CKL();
   c->st.kernel_launches++;
-  CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
+  CK(to_host(c, c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
   CK(cudaStreamSynchronize(c->meta));                    // the grant (which claims are served) is needed to plan the copies
   std::vector<Seg> segs;
   std::vector<LmClaim> lmc;
@@ -1086,7 +1088,7 @@ extern "C" int rc_restore_begin(rc_ctx* c, uint32_t n, const uint64_t* id, int32
       ++fi;
     }
     if (nf) {
-      CK(to_dev(c->scatter, c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8));
+      CK(to_dev(c, c->scatter, c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8));
       k_bitflip<<<(nf + 63) / 64, 64, 0, c->scatter>>>(c->staging[1][slot], c->d_flip + flip_base, nf);
       CKL();
       c->st.kernel_launches++;
@@ -1204,7 +1206,7 @@ extern "C" int rc_tp_restore_verify(rc_ctx* c, uint32_t n, const uint64_t* id, i
     }
     if (n) {
       memcpy(c->h_verd, local, (u64)n * sizeof(TpVerdict));
-      CK(to_dev(c->meta, c->d_verd, c->h_verd, (u64)n * sizeof(TpVerdict)));
+      CK(to_dev(c, c->meta, c->d_verd, c->h_verd, (u64)n * sizeof(TpVerdict)));
     }
     k_tp_push<<<1, 1024, 0, c->meta>>>(c->d_verd, n, peers, c->tp_ranks, c->tp_rank, (u32)c->desc_cap, c->tp_epoch);
     CKL();
@@ -1224,13 +1226,13 @@ extern "C" int rc_tp_restore_commit(rc_ctx* c, uint32_t n, uint32_t ranks, const
   CK(cudaMemsetAsync(c->d_counters, 0, 16, c->meta));
   if (gathered) {                                          // all-gather path: [ranks][n] records from the caller
     memcpy(c->h_verd, gathered, (u64)ranks * n * sizeof(TpVerdict));
-    if (n) CK(to_dev(c->meta, c->d_gath, c->h_verd, (u64)ranks * n * sizeof(TpVerdict)));
+    if (n) CK(to_dev(c, c->meta, c->d_gath, c->h_verd, (u64)ranks * n * sizeof(TpVerdict)));
     src = c->d_gath; stride = n;
   } else {                                                 // NVLink path: the peers wrote into this rank's mailbox
     k_tp_ready<<<1, 32, 0, c->meta>>>((const u64*)c->d_mailbox, ranks, c->tp_epoch, c->d_counters);
     CKL();
     c->st.kernel_launches++;
-    CK(to_host(c->meta, c->h_counters, c->d_counters, 16));
+    CK(to_host(c, c->meta, c->h_counters, c->d_counters, 16));
     CK(cudaStreamSynchronize(c->meta));
     if (c->h_counters[0]) return RC_ERR_BUSY;              // some peer has not published this epoch yet: barrier first
     src = (const TpVerdict*)(c->d_mailbox + TP_MAX_RANKS * 8); stride = (u32)c->desc_cap;
@@ -1243,7 +1245,7 @@ extern "C" int rc_tp_restore_commit(rc_ctx* c, uint32_t n, uint32_t ranks, const
   k_tp_merge<<<(n + 255) / 256, 256, 0, c->meta>>>(c->d_res[1], n, src, stride, ranks, c->d_counters + 1);
   CKL();
   c->st.kernel_launches++;
-  CK(to_host(c->meta, c->h_counters, c->d_counters, 16));
+  CK(to_host(c, c->meta, c->h_counters, c->d_counters, 16));
   CK(cudaStreamSynchronize(c->meta));
   if (c->h_counters[1]) return RC_ERR_INVALID;             // a rank disagrees on which claims were served: nothing applied
   k_tp_apply<<<warps_grid(n), 256, 0, c->meta>>>(c->d_desc[1], c->d_res[1], n, c->d_bt, c->d_used, c->d_ref, c->fill,
@@ -1252,7 +1254,7 @@ extern "C" int rc_tp_restore_commit(rc_ctx* c, uint32_t n, uint32_t ranks, const
   c->st.kernel_launches++;
   int rc;
   if ((rc = emit(c, 1, n, EM_RESTORE, 0))) return rc;
-  CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
+  CK(to_host(c, c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
   op.status = st;
   c->tp_pending = false;
   return wait_restore(c);
@@ -1371,7 +1373,7 @@ extern "C" int rc_make_room(rc_ctx* c, uint64_t request_id, uint32_t need, int32
   k_vic_decide<<<1, 1024, 0, c->meta>>>(c->d_gain, n, U, need, c->d_used, c->NB, c->d_counters);
   CKL();
   c->st.kernel_launches++;
-  CK(to_host(c->meta, c->h_counters, c->d_counters, 16));
+  CK(to_host(c, c->meta, c->h_counters, c->d_counters, 16));
   CK(cudaStreamSynchronize(c->meta));
   const u32 oc = c->h_counters[0], lo = c->h_counters[1], hi = c->h_counters[2];
   if (oc == VO_FITS) { *status = RC_ST_OK; return RC_OK; }
@@ -1441,7 +1443,7 @@ extern "C" int rc_outcomes(rc_ctx* c, rc_event* buf, uint64_t cap, uint64_t* n_o
     u64 part = std::min<u64>(m - done, c->ev_bounce_cap), got = 0;
     while (got < part) {
       const u64 at = (c->ev_drained + done + got) % E, l = std::min(part - got, E - at);
-      CK(to_host(c->util, c->h_evbuf + got, c->d_ring + at, l * sizeof(Event)));
+      CK(to_host(c, c->util, c->h_evbuf + got, c->d_ring + at, l * sizeof(Event)));
       got += l;
     }
     CK(cudaStreamSynchronize(c->util));

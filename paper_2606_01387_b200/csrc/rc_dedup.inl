@@ -80,7 +80,7 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
   for (auto& od : old_dg) if (od.second) c->dg_alloc.release(od.first, od.second);
   op.n = n; op.status = st; op.blocks = T; op.copy_bytes = 0; op.launches = 0;
   int rc;
-  CK(to_dev(c->gather, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
+  CK(to_dev(c, c->gather, c->d_desc[set], c->h_desc[set], (u64)n * sizeof(Desc)));
   k_offsets<<<1, 1024, 0, c->gather>>>(c->d_desc[set], n, c->d_off[set]);
   CKL();
   k_worklist<<<warps_grid(n), 256, 0, c->gather>>>(c->d_desc[set], c->d_res[set], n, c->d_off[set], c->d_bt, nullptr, c->d_phys[oi], 0);
@@ -101,8 +101,8 @@ static int offload_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     k_block_digest<<<warps_grid(m), 256, 0, c->gather>>>(c->part[0][slot], nullptr, c->d_dtmp[oi] + w0, c->d_etmp[oi] + w0, m, c->G, nullptr);
     CKL();
     c->st.kernel_launches++;
-    CK(to_host(c->gather, c->h_dig + w0, c->d_dtmp[oi] + w0, (u64)m * 8));
-    CK(to_host(c->gather, c->h_dig2 + w0, c->d_etmp[oi] + w0, (u64)m * 8));
+    CK(to_host(c, c->gather, c->h_dig + w0, c->d_dtmp[oi] + w0, (u64)m * 8));
+    CK(to_host(c, c->gather, c->h_dig2 + w0, c->d_etmp[oi] + w0, (u64)m * 8));
     CK(cudaEventRecord(c->ev_ready[0][slot], c->gather));
     CK(cudaStreamSynchronize(c->gather));                  // the keys decide which blocks cross the link
     CK(cudaStreamWaitEvent(c->d2h, c->ev_ready[0][slot], 0));
@@ -180,7 +180,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
                                           c->d_counters);
   CKL();
   c->st.kernel_launches++;
-  CK(to_host(c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
+  CK(to_host(c, c->meta, c->h_res[1], c->d_res[1], (u64)n * sizeof(Res)));
   CK(cudaStreamSynchronize(c->meta));
   // staged blocks in first-appearance order; items = (work position, staged block)
   std::vector<u32> su;                                     // staged index -> host slot
@@ -231,8 +231,8 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
     return a.first / c->chunk_blocks < b.first / c->chunk_blocks; });
   for (size_t j = 0; j < items.size(); ++j) { c->h_iw[j] = items[j].second; c->h_ispos[j] = (u32)(items[j].first % c->chunk_blocks); }
   if (!items.empty()) {
-    CK(to_dev(c->meta, c->d_iw, c->h_iw, items.size() * 4));
-    CK(to_dev(c->meta, c->d_ispos, c->h_ispos, items.size() * 4));
+    CK(to_dev(c, c->meta, c->d_iw, c->h_iw, items.size() * 4));
+    CK(to_dev(c, c->meta, c->d_ispos, c->h_ispos, items.size() * 4));
   }
   CK(cudaEventRecord(c->ev_plan[1], c->meta));
   CK(cudaStreamWaitEvent(c->scatter, c->ev_plan[1], 0));
@@ -268,7 +268,7 @@ static int restore_begin_dedup(rc_ctx* c, uint32_t n, const uint64_t* id, int32_
       ++fi;
     }
     if (nf) {
-      CK(to_dev(c->scatter, c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8));
+      CK(to_dev(c, c->scatter, c->d_flip + flip_base, c->h_flip + flip_base, (u64)nf * 8));
       k_bitflip<<<(nf + 63) / 64, 64, 0, c->scatter>>>(c->staging[1][slot], c->d_flip + flip_base, nf);
       CKL();
       c->st.kernel_launches++;
